@@ -1,0 +1,149 @@
+/* gc.h -- C ABI of libgeoclaw_b200.so: the per-level time step of GPU GeoClaw on one B200.
+ *
+ * Source of the operations: "Efficient Tsunami Modeling on Adaptive Grids with GPUs"
+ * (arXiv 1901.06798; /root/reference/PAPER.md, cited as P:<line>), AMR steps 1-5 (P:140-146,
+ * section 3.1), regridding (section 3.2), the wave-propagation update
+ * (eqs. 4-14) and the CFL condition (eq. 15).  Everything the paper leaves
+ * open is fixed in DESIGN.md section 3 ("readings").
+ *
+ * Conventions
+ *  - plain C, extern "C"; every call returns int: 0 = GC_OK, < 0 = GC_ERR_*; nothing throws or aborts.
+ *  - DEVICE vs HOST pointers are stated per argument.  All device work is enqueued on the CUDA
+ *    stream given to gc_ctx_create (caller-owned) and is asynchronous unless the call returns a
+ *    host scalar / fills a host struct (then the call synchronises that stream).
+ *  - Ownership: the caller owns every array it passes and the stream.  The library takes device
+ *    memory only through the allocator callbacks given to gc_ctx_create (so PyTorch can own it);
+ *    with NULL callbacks it falls back to cudaMalloc / cudaFree.
+ *  - Layout: a level is one pool; each patch stores (nx+4) x (ny+4) doubles per field, row-major,
+ *    x fastest, ghost width 2 (interior cell (i,j) of the patch at storage (i+2, j+2)).  Fields are
+ *    SoA planes h, hu, hv (two buffers each: "new" = current, "old" = previous step) and b.
+ *  - Indices are 0-based global cell indices of the level; patches must not overlap; for level > 1
+ *    patch boxes are aligned to coarse cells (i0, j0, nx, ny multiples of ratio_to_coarser).
+ *  - fp64 throughout; device code is compiled with -fmad=false and uses IEEE divide / sqrt, so results
+ *    are bit-identical to a plain C evaluation of DESIGN.md section 3 in the stated order.
+ */
+#ifndef GC_H
+#define GC_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GC_OK = 0, GC_ERR_BADARG = -1, GC_ERR_NOMEM = -2, GC_ERR_CUDA = -3, GC_ERR_NAN = -4,
+       GC_ERR_NEGDEPTH = -5, GC_ERR_STATE = -6 };
+enum { GC_FIELD_H = 0, GC_FIELD_HU = 1, GC_FIELD_HV = 2, GC_FIELD_B = 3 };
+enum { GC_NEW = 0, GC_OLD = 1 };
+
+typedef struct gc_ctx gc_ctx;
+typedef struct gc_level gc_level;
+
+typedef struct {
+    int coord;            /* 0 Cartesian (metres), 1 spherical lon/lat (degrees), capacity form */
+    double g;             /* gravity, 9.81 */
+    double dry_tol;       /* dry tolerance epsilon: a cell with h <= dry_tol is dry ("handling dry states") */
+    double sea_level;     /* eta_sea used by the flagging criterion */
+    double earth_radius;  /* metres; used when coord == 1 */
+    int limiter;          /* 0 none (first-order Godunov, eq. 4), 1 MC */
+    int bc[4];            /* xlo, xhi, ylo, yhi: 0 zero-order extrapolation, 1 reflecting wall */
+} gc_params;
+
+typedef struct { int32_t i0, j0, nx, ny; } gc_patch;   /* interior box of a patch */
+
+typedef struct {
+    double tol_eta;       /* flag wet cells with |h + b - sea_level| > tol_eta; <= 0: off */
+    double tol_slope;     /* flag wet cells whose central-difference surface slope per cell > tol_slope; <= 0: off */
+    int offshore_only;    /* wave criteria apply only where b < 0 */
+    int buffer;           /* dilation by this many cells, Chebyshev distance */
+    int nboxes;           /* forced space-time regions */
+    const double *boxes;  /* HOST, 6 per box: x0, x1, y0, y1, t0, t1 */
+} gc_flag_params;
+
+typedef struct {
+    double cfl_max;       /* nu = dt * s_over_dx_max (eq. 15) */
+    double s_over_dx_max; /* max over both sweeps, all patches, interior lines, of |s| / (kappa dx) */
+    double clipped_mass;  /* sum over interior cells of (-h) * area for cells with h < 0 set to 0 by the clean-up */
+    int64_t n_clipped;    /* number of such cells */
+    int32_t nan_seen;     /* 1 if any updated value is NaN */
+} gc_step_stats;
+
+/* Allocator callbacks: alloc returns a DEVICE pointer (>= 256-byte aligned) or NULL. */
+typedef void *(*gc_alloc_fn)(size_t bytes, void *user);
+typedef void (*gc_free_fn)(void *ptr, void *user);
+
+/* Context: parameters + the CUDA stream (cudaStream_t passed as void*; NULL = legacy default stream). */
+int gc_ctx_create(const gc_params *params /*HOST*/, void *cuda_stream, gc_alloc_fn alloc, gc_free_fn free_,
+                  void *user, gc_ctx **out);
+int gc_ctx_destroy(gc_ctx *);
+const char *gc_last_error(const gc_ctx *);
+
+/* A1: one level = one device pool with all its patches, a patch-descriptor table,
+ * per-row metric tables and the host-built work lists for ghost filling.  level is 1-based; level 1
+ * covers the domain.  xlo, ylo: lower-left corner of the DOMAIN; dx, dy: cell size of THIS level;
+ * nx_level, ny_level: domain size in cells of this level.  patches: HOST array.  State is zero. */
+int gc_level_create(gc_ctx *, int level, double xlo, double ylo, double dx, double dy,
+                    int64_t nx_level, int64_t ny_level, int ratio_to_coarser,
+                    int npatch, const gc_patch *patches, gc_level **out);
+int gc_level_destroy(gc_level *);
+int64_t gc_level_ncells(const gc_level *);   /* interior cells of the level */
+
+/* Field transfer.  Per patch: arrays shaped like the storage, (ny+4) rows of (nx+4), leading dimension
+ * ld (elements).  Global: the array covers global cells [gi0, gi0+gnx) x [gj0, gj0+gny) of the level with
+ * leading dimension ld; set writes every storage cell (ghosts included) that falls inside, get reads
+ * interior cells.  src/dst are DEVICE pointers if is_device != 0, else HOST (the call then stages through
+ * a device buffer and synchronises).  which: GC_NEW (current state) or GC_OLD (before the last step). */
+int gc_level_set_field(gc_level *, int patch, int field, const double *src, int is_device, int64_t ld);
+int gc_level_get_field(const gc_level *, int patch, int field, int which, double *dst, int is_device, int64_t ld);
+int gc_level_set_global(gc_level *, int field, const double *src, int is_device, int64_t ld,
+                        int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
+int gc_level_get_global(const gc_level *, int field, int which, double *dst, int is_device, int64_t ld,
+                        int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
+
+/* A2-A4 (P:143 step 2): fill the ghost cells of the current state.  Order: same-level
+ * copy incl. corners; remaining in-domain ghosts from `coarser` interpolated in space (limited linear in
+ * eta, u, v) and time (alpha = (t - t_coarse_old) / dt_coarse, linear between coarser's OLD and NEW buffers,
+ * whose own ghosts must be filled); physical boundary (x faces, then y faces).  coarser == NULL: level 1.
+ * gc_fill_ghost_b does same-level copy + physical boundary for the bathymetry (once per regrid). */
+int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha);
+int gc_fill_ghost_b(gc_level *L);
+
+/* A5-A7 (P:142 step 1; eqs. 13-15): x-sweep then y-sweep over every patch of the level, dry clean-up,
+ * exact order-independent max reduction of the wave speeds, swap NEW/OLD.  dt == 0 is a probe: state and
+ * buffers unchanged, speeds returned.  out: HOST struct, or NULL = keep the statistics on the device (no
+ * synchronisation; read them later with gc_level_stats). */
+int gc_level_step(gc_level *L, double dt, gc_step_stats *out);
+/* Same with dt held in device memory: dt_used = *dt_dev (DEVICE double, read by the kernels); after the
+ * step the library writes the next dt = cfl_target / s_over_dx_max into *dt_dev.  No host sync; CUDA-graph
+ * capturable. */
+int gc_level_step_auto(gc_level *L, double *dt_dev, double cfl_target);
+int gc_level_stats(const gc_level *, gc_step_stats *out /*HOST*/);
+
+/* wet mask (h > dry_tol) of the current state: one byte per interior cell, patch after patch, row-major. */
+int gc_wet_mask(const gc_level *, uint8_t *mask, int is_device);
+/* sum of h * cell area over interior cells, fixed-order (deterministic) reduction; returns NaN on error. */
+double gc_level_mass(const gc_level *);
+
+/* A10: refinement flags of the current state, one byte per interior cell (layout as
+ * gc_wet_mask); ghost cells must be filled if tol_slope > 0.  nflag (HOST, nullable) receives the count. */
+int gc_flag_cells(const gc_level *L, const gc_flag_params *, double t, uint8_t *flags, int is_device, int64_t *nflag);
+
+/* A9 (P:145 step 4): every coarse cell covered by fine cells <- average of the r*r fine cells. */
+int gc_average_down(gc_level *coarse, const gc_level *fine);
+/* A11: interior of the new fine level <- copy from oldfine where it overlapped (nullable), else
+ * interpolation from coarse's NEW buffer (ghosts filled).  b of newfine must be set already. */
+int gc_level_init_from(gc_level *newfine, const gc_level *oldfine, const gc_level *coarse);
+
+/* A8 (P:146 step 5): flux registers on the boundary of the fine region.  attach builds and zeroes them
+ * (and makes both levels record what the registers need during gc_level_step); fixup applies
+ * Q_C += side * delta / area to the uncovered coarse neighbours, then the clean-up rule, and re-zeroes. */
+int gc_flux_attach(gc_level *coarse, gc_level *fine);
+int gc_flux_fixup(gc_level *coarse, gc_level *fine);
+
+/* Measured fp64 ALU throughput of this device (DFMA micro-benchmark, flop/s); for the "alu" roofline. */
+int gc_probe_fp64_peak(gc_ctx *, double *flops_out /*HOST*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

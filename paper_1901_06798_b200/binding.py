@@ -1,0 +1,253 @@
+"""Thin Python binding of libgeoclaw_b200.so (include/gc.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory (through
+the allocator callbacks), the stream and nothing else.  There is NO CPU fallback: importing works without a
+GPU (so the symbols can be checked), but creating a Context without a CUDA device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgeoclaw_b200.so")
+
+SYMBOLS = [
+    "gc_ctx_create", "gc_ctx_destroy", "gc_last_error", "gc_level_create", "gc_level_destroy", "gc_level_ncells",
+    "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
+    "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
+    "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
+]
+
+
+class Params(C.Structure):
+    _fields_ = [("coord", C.c_int), ("g", C.c_double), ("dry_tol", C.c_double), ("sea_level", C.c_double),
+                ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4)]
+
+
+class FlagParams(C.Structure):
+    _fields_ = [("tol_eta", C.c_double), ("tol_slope", C.c_double), ("offshore_only", C.c_int),
+                ("buffer", C.c_int), ("nboxes", C.c_int), ("boxes", C.POINTER(C.c_double))]
+
+
+class StepStats(C.Structure):
+    _fields_ = [("cfl_max", C.c_double), ("s_over_dx_max", C.c_double), ("clipped_mass", C.c_double),
+                ("n_clipped", C.c_int64), ("nan_seen", C.c_int32)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+_lib = None
+
+
+def lib():
+    """Loads the extension; raises if it has not been built (python -m paper_1901_06798_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("CUDA extension missing: %s (run `python -m paper_1901_06798_b200.build`); "
+                           "there is no CPU fallback" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, i, d, i64 = C.c_void_p, C.c_int, C.c_double, C.c_int64
+    L.gc_ctx_create.argtypes = [vp, vp, ALLOC_FN, FREE_FN, vp, vp]
+    L.gc_ctx_destroy.argtypes = [vp]
+    L.gc_last_error.argtypes = [vp]; L.gc_last_error.restype = C.c_char_p
+    L.gc_level_create.argtypes = [vp, i, d, d, d, d, i64, i64, i, i, vp, vp]
+    L.gc_level_destroy.argtypes = [vp]
+    L.gc_level_ncells.argtypes = [vp]; L.gc_level_ncells.restype = i64
+    L.gc_level_set_field.argtypes = [vp, i, i, vp, i, i64]
+    L.gc_level_get_field.argtypes = [vp, i, i, i, vp, i, i64]
+    L.gc_level_set_global.argtypes = [vp, i, vp, i, i64, i64, i64, i64, i64]
+    L.gc_level_get_global.argtypes = [vp, i, i, vp, i, i64, i64, i64, i64, i64]
+    L.gc_fill_ghost.argtypes = [vp, vp, d]
+    L.gc_fill_ghost_b.argtypes = [vp]
+    L.gc_level_step.argtypes = [vp, d, vp]
+    L.gc_level_step_auto.argtypes = [vp, vp, d]
+    L.gc_level_stats.argtypes = [vp, vp]
+    L.gc_wet_mask.argtypes = [vp, vp, i]
+    L.gc_level_mass.argtypes = [vp]; L.gc_level_mass.restype = d
+    L.gc_flag_cells.argtypes = [vp, vp, d, vp, i, vp]
+    L.gc_average_down.argtypes = [vp, vp]
+    L.gc_level_init_from.argtypes = [vp, vp, vp]
+    L.gc_flux_attach.argtypes = [vp, vp]
+    L.gc_flux_fixup.argtypes = [vp, vp]
+    L.gc_probe_fp64_peak.argtypes = [vp, vp]
+    _lib = L
+    return L
+
+
+FIELDS = {"h": 0, "hu": 1, "hv": 2, "b": 3}
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+class Level:
+    def __init__(self, ctx, level, xlo, ylo, dx, dy, nxl, nyl, ratio, patches):
+        self.ctx = ctx
+        self.level, self.xlo, self.ylo, self.dx, self.dy = level, xlo, ylo, dx, dy
+        self.nxl, self.nyl, self.ratio = int(nxl), int(nyl), int(ratio)
+        self.patches = np.ascontiguousarray(patches, dtype=np.int32).reshape(-1, 4)
+        h = C.c_void_p()
+        ctx._chk(lib().gc_level_create(ctx.h, level, xlo, ylo, dx, dy, nxl, nyl, ratio, len(self.patches),
+                                       self.patches.ctypes.data, C.byref(h)), "gc_level_create")
+        self.h = h
+        self.ncells = int(lib().gc_level_ncells(h))
+
+    def destroy(self):
+        if self.h:
+            lib().gc_level_destroy(self.h)
+            self.h = None
+
+    def _src(self, arr):
+        if _is_torch(arr):
+            assert arr.is_cuda and arr.dtype.is_floating_point and arr.element_size() == 8 and arr.stride(-1) == 1
+            return arr, arr.data_ptr(), 1, arr.stride(0)
+        a = np.ascontiguousarray(arr, dtype=np.float64)
+        return a, a.ctypes.data, 0, a.shape[1]
+
+    def set_field(self, p, field, arr):
+        a, ptr, dev, ld = self._src(arr)
+        self.ctx._chk(lib().gc_level_set_field(self.h, p, FIELDS[field], ptr, dev, ld), "gc_level_set_field")
+
+    def get_field(self, p, field, which=0):
+        nx, ny = int(self.patches[p, 2]), int(self.patches[p, 3])
+        a = np.empty((ny + 4, nx + 4))
+        self.ctx._chk(lib().gc_level_get_field(self.h, p, FIELDS[field], which, a.ctypes.data, 0, nx + 4), "gc_level_get_field")
+        return a
+
+    def set_global(self, field, arr, gi0=0, gj0=0):
+        a, ptr, dev, ld = self._src(arr)
+        self.ctx._chk(lib().gc_level_set_global(self.h, FIELDS[field], ptr, dev, ld, gi0, gj0, a.shape[1], a.shape[0]),
+                      "gc_level_set_global")
+
+    def get_global(self, field, which=0, gi0=0, gj0=0, gnx=None, gny=None, fill=np.nan, out=None):
+        gnx = self.nxl if gnx is None else gnx
+        gny = self.nyl if gny is None else gny
+        if out is not None:  # device tensor supplied by the caller
+            self.ctx._chk(lib().gc_level_get_global(self.h, FIELDS[field], which, out.data_ptr(), 1, out.stride(0),
+                                                    gi0, gj0, gnx, gny), "gc_level_get_global")
+            return out
+        a = np.full((gny, gnx), fill)
+        self.ctx._chk(lib().gc_level_get_global(self.h, FIELDS[field], which, a.ctypes.data, 0, gnx, gi0, gj0, gnx, gny),
+                      "gc_level_get_global")
+        return a
+
+    def fill_ghost_b(self):
+        self.ctx._chk(lib().gc_fill_ghost_b(self.h), "gc_fill_ghost_b")
+
+    def fill_ghost(self, coarser=None, alpha=1.0):
+        self.ctx._chk(lib().gc_fill_ghost(self.h, coarser.h if coarser is not None else None, alpha), "gc_fill_ghost")
+
+    def step(self, dt, sync=True):
+        if not sync:
+            self.ctx._chk(lib().gc_level_step(self.h, dt, None), "gc_level_step")
+            return None
+        st = StepStats()
+        self.ctx._chk(lib().gc_level_step(self.h, dt, C.byref(st)), "gc_level_step")
+        return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
+                    n_clipped=st.n_clipped, nan_seen=st.nan_seen)
+
+    def step_auto(self, dt_dev, cfl):
+        """dt_dev: 1-element float64 CUDA tensor holding dt; updated in place to the next dt."""
+        self.ctx._chk(lib().gc_level_step_auto(self.h, dt_dev.data_ptr(), cfl), "gc_level_step_auto")
+
+    def stats(self):
+        st = StepStats()
+        self.ctx._chk(lib().gc_level_stats(self.h, C.byref(st)), "gc_level_stats")
+        return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
+                    n_clipped=st.n_clipped, nan_seen=st.nan_seen)
+
+    def wet_mask(self):
+        m = np.zeros(self.ncells, dtype=np.uint8)
+        self.ctx._chk(lib().gc_wet_mask(self.h, m.ctypes.data, 0), "gc_wet_mask")
+        return m
+
+    def mass(self):
+        return lib().gc_level_mass(self.h)
+
+    def flag(self, tol_eta=0.0, tol_slope=0.0, offshore_only=0, buffer=0, boxes=(), t=0.0):
+        fp = FlagParams()
+        bx = np.ascontiguousarray(np.array(boxes, dtype=np.float64).reshape(-1, 6))
+        fp.tol_eta, fp.tol_slope, fp.offshore_only, fp.buffer, fp.nboxes = tol_eta, tol_slope, offshore_only, buffer, len(bx)
+        fp.boxes = bx.ctypes.data_as(C.POINTER(C.c_double))
+        fl = np.zeros(self.ncells, dtype=np.uint8)
+        n = C.c_int64(0)
+        self.ctx._chk(lib().gc_flag_cells(self.h, C.byref(fp), t, fl.ctypes.data, 0, C.byref(n)), "gc_flag_cells")
+        return fl, n.value
+
+    def average_down_from(self, fine):
+        self.ctx._chk(lib().gc_average_down(self.h, fine.h), "gc_average_down")
+
+    def init_from(self, old, coarse):
+        self.ctx._chk(lib().gc_level_init_from(self.h, old.h if old is not None else None, coarse.h), "gc_level_init_from")
+
+    def flux_attach(self, fine):
+        self.ctx._chk(lib().gc_flux_attach(self.h, fine.h), "gc_flux_attach")
+
+    def flux_fixup(self, fine):
+        self.ctx._chk(lib().gc_flux_fixup(self.h, fine.h), "gc_flux_fixup")
+
+
+class Context:
+    """The CUDA backend: Context(**params).level_create(...) -> Level.  Device memory comes from torch."""
+    name = "b200"
+
+    def __init__(self, coord=0, g=9.81, dry_tol=1e-3, sea_level=0.0, earth_radius=6367500.0, limiter=1,
+                 bc=(1, 1, 1, 1), device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1901_06798_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._bufs = {}
+        self._alloc_cb = ALLOC_FN(self._alloc)
+        self._free_cb = FREE_FN(self._free)
+        p = Params()
+        p.coord, p.g, p.dry_tol, p.sea_level, p.earth_radius, p.limiter = coord, g, dry_tol, sea_level, earth_radius, limiter
+        for k in range(4):
+            p.bc[k] = int(bc[k])
+        self.params = p
+        h = C.c_void_p()
+        rc = lib().gc_ctx_create(C.byref(p), C.c_void_p(self.stream.cuda_stream), self._alloc_cb, self._free_cb, None, C.byref(h))
+        if rc != 0:
+            raise RuntimeError("gc_ctx_create failed: %d" % rc)
+        self.h = h
+
+    def _alloc(self, nbytes, user):
+        try:
+            with self.torch.cuda.stream(self.stream):
+                t = self.torch.empty(int(nbytes), dtype=self.torch.uint8, device=self.device)
+        except Exception:
+            return None
+        self._bufs[t.data_ptr()] = t
+        return t.data_ptr()
+
+    def _free(self, ptr, user):
+        self._bufs.pop(ptr, None)
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            msg = lib().gc_last_error(self.h)
+            raise RuntimeError("%s failed: %d (%s)" % (what, rc, msg.decode() if msg else ""))
+
+    def level_create(self, level, xlo, ylo, dx, dy, nxl, nyl, ratio, patches):
+        return Level(self, level, xlo, ylo, dx, dy, nxl, nyl, ratio, patches)
+
+    def fp64_peak(self):
+        v = C.c_double(0.0)
+        self._chk(lib().gc_probe_fp64_peak(self.h, C.byref(v)), "gc_probe_fp64_peak")
+        return v.value
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def destroy(self):
+        if self.h:
+            lib().gc_ctx_destroy(self.h)
+            self.h = None

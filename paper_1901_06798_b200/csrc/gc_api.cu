@@ -1,0 +1,474 @@
+// gc_api.cu -- C ABI entry points (include/gc.h) and the host-side level runtime: pool layout, patch
+// descriptors, metric tables, work lists.  All arithmetic of the method runs in the kernels; the host only
+// builds index lists ("only clustering and bookkeeping stay on the host") and the per-row metric tables
+// (sin/cos evaluated once on the host).
+#include <math.h>
+#include <string.h>
+#include <algorithm>
+#include <atomic>
+#include "gc_internal.h"
+
+static std::atomic<uint64_t> g_gen{1};
+
+int gc_fail(gc_ctx *c, int code, const char *msg) { if (c) c->err = msg; return code; }
+
+int gc_cuda_check(gc_ctx *c, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
+        return GC_ERR_CUDA;
+    }
+    return GC_OK;
+}
+
+void *gc_dev_alloc(gc_ctx *c, size_t bytes)
+{
+    if (bytes == 0) bytes = 8;
+    if (c->alloc) return c->alloc(bytes, c->user);
+    void *p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+void gc_dev_free(gc_ctx *c, void *p)
+{
+    if (!p) return;
+    if (c->free_) c->free_(p, c->user); else if (!c->alloc) cudaFree(p);
+}
+
+extern "C" const char *gc_last_error(const gc_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc, gc_free_fn free_, void *user, gc_ctx **out)
+{
+    if (!P || !out) return GC_ERR_BADARG;
+    if (!(P->g > 0.0) || !(P->dry_tol >= 0.0) || (P->coord != 0 && P->coord != 1)) return GC_ERR_BADARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return GC_ERR_CUDA; }   // no CPU fallback
+    gc_ctx *c = new gc_ctx();
+    c->P = *P; c->stream = (cudaStream_t)stream; c->alloc = alloc; c->free_ = free_; c->user = user;
+    *out = c;
+    return GC_OK;
+}
+extern "C" int gc_ctx_destroy(gc_ctx *c) { delete c; return GC_OK; }
+
+template <class T> static T *upload(gc_level *L, const std::vector<T> &v)
+{
+    T *d = (T *)gc_dev_alloc(L->ctx, v.size() * sizeof(T));
+    if (!d) return nullptr;
+    L->allocs.push_back(d);
+    if (!v.empty()) cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, L->ctx->stream);
+    return d;
+}
+
+static inline int64_t bkey(int64_t bx, int64_t by) { return (bx << 32) ^ (by & 0xffffffffll); }
+
+int gc_find_patch_host(const gc_level *L, int64_t gi, int64_t gj)
+{
+    if (gi < 0 || gj < 0 || gi >= L->nxl || gj >= L->nyl) return -1;
+    auto it = L->buckets.find(bkey(gi / L->bsize, gj / L->bsize));
+    if (it == L->buckets.end()) return -1;
+    for (int32_t q : it->second) {
+        const gc_patch &Q = L->pat[q];
+        if (gi >= Q.i0 && gi < (int64_t)Q.i0 + Q.nx && gj >= Q.j0 && gj < (int64_t)Q.j0 + Q.ny) return q;
+    }
+    return -1;
+}
+
+// DESIGN.md 3.5 metric tables over global rows -2..ny+1 (index +2) and edges -2..ny+2
+static void build_metric(gc_level *L)
+{
+    const gc_params &P = L->ctx->P;
+    int64_t ny = L->nyl, nr = ny + 4, ne = ny + 5;
+    L->kappa.assign(nr, 1.0); L->rdx.assign(nr, 0.0); L->rdy.assign(nr, 0.0); L->ey.assign(ne, 1.0);
+    L->ex = 1.0;
+    if (P.coord == 1) {
+        const double pi = 3.14159265358979323846;
+        const double d2r = pi / 180.0;
+        double R = P.earth_radius;
+        L->ex = R * d2r;
+        for (int64_t j = -2; j <= ny + 2; j++) {
+            double lat = (L->ylo + (double)j * L->dy) * d2r;
+            L->ey[j + 2] = R * cos(lat) * d2r;
+        }
+        for (int64_t j = -2; j <= ny + 1; j++) {
+            double lat0 = (L->ylo + (double)j * L->dy) * d2r;
+            double lat1 = (L->ylo + (double)(j + 1) * L->dy) * d2r;
+            L->kappa[j + 2] = d2r * (R * R) * (sin(lat1) - sin(lat0)) / L->dy;
+        }
+        if (P.bc[2] == 1) { L->kappa[1] = L->kappa[2]; L->kappa[0] = L->kappa[3]; L->ey[1] = L->ey[3]; L->ey[0] = L->ey[4]; }
+        if (P.bc[3] == 1) {
+            L->kappa[ny + 2] = L->kappa[ny + 1]; L->kappa[ny + 3] = L->kappa[ny];
+            L->ey[ny + 3] = L->ey[ny + 1]; L->ey[ny + 4] = L->ey[ny];
+        }
+    }
+    for (int64_t j = 0; j < nr; j++) {
+        L->rdx[j] = 1.0 / (L->kappa[j] * L->dx);
+        L->rdy[j] = 1.0 / (L->kappa[j] * L->dy);
+    }
+}
+
+static void build_tiles(gc_level *L, std::vector<SweepTile> &xt, std::vector<SweepTile> &yt)
+{
+    const int B = 256, YW = 8;
+    for (int p = 0; p < L->np; p++) {
+        const gc_patch &P = L->pat[p];
+        // x-sweep: all rows 0..ny+3; whole rows if nx+3 <= B, else balanced chunks of <= B-3 cells
+        int nchunk = (P.nx + (B - 3) - 1) / (B - 3);
+        for (int c = 0; c < nchunk; c++) {
+            int c0 = (int)((int64_t)P.nx * c / nchunk), c1 = (int)((int64_t)P.nx * (c + 1) / nchunk);
+            int nc = c1 - c0, R = B / (nc + 3);
+            for (int r0 = 0; r0 < P.ny + 4; r0 += R)
+                xt.push_back(SweepTile{p, r0, std::min(R, P.ny + 4 - r0), 2 + c0, nc});
+        }
+        // y-sweep: interior columns in groups of YW, segments of <= B/YW - 3 cells along y
+        int E = B / YW, nseg = (P.ny + (E - 3) - 1) / (E - 3);
+        for (int s = 0; s < nseg; s++) {
+            int r0 = (int)((int64_t)P.ny * s / nseg), r1 = (int)((int64_t)P.ny * (s + 1) / nseg);
+            for (int i0 = 0; i0 < P.nx; i0 += YW)
+                yt.push_back(SweepTile{p, 2 + i0, std::min(YW, P.nx - i0), 2 + r0, r1 - r0});
+        }
+    }
+}
+
+extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, double dx, double dy,
+                               int64_t nxl, int64_t nyl, int ratio, int np, const gc_patch *pat, gc_level **out)
+{
+    if (!ctx || !out || np < 0 || (np > 0 && !pat) || nxl < 1 || nyl < 1 || !(dx > 0.0) || !(dy > 0.0) || ratio < 1 || level < 1)
+        return gc_fail(ctx, GC_ERR_BADARG, "gc_level_create: bad argument");
+    if (nxl > 2000000000ll || nyl > 2000000000ll) return gc_fail(ctx, GC_ERR_BADARG, "gc_level_create: level too large");
+    int maxdim = 1;
+    for (int p = 0; p < np; p++) {
+        const gc_patch &P = pat[p];
+        if (P.nx < 2 || P.ny < 2 || P.i0 < 0 || P.j0 < 0 || (int64_t)P.i0 + P.nx > nxl || (int64_t)P.j0 + P.ny > nyl)
+            return gc_fail(ctx, GC_ERR_BADARG, "gc_level_create: patch outside the level or smaller than 2 cells");
+        if (level > 1 && (P.i0 % ratio || P.j0 % ratio || P.nx % ratio || P.ny % ratio))
+            return gc_fail(ctx, GC_ERR_BADARG, "gc_level_create: fine patch not aligned with coarse cells");
+        maxdim = std::max(maxdim, std::max(P.nx, P.ny));
+    }
+    gc_level *L = new gc_level();
+    L->ctx = ctx; L->level = level; L->ratio = ratio; L->np = np; L->cur = 0;
+    L->xlo = xlo; L->ylo = ylo; L->dx = dx; L->dy = dy; L->nxl = nxl; L->nyl = nyl;
+    L->gen = g_gen.fetch_add(1);
+    L->pat.assign(pat, pat + np);
+    L->bsize = std::max(maxdim, 8);
+    L->hpat.resize(np);
+    int64_t off = 0, ioff = 0;
+    for (int p = 0; p < np; p++) {
+        const gc_patch &P = L->pat[p];
+        PatchDesc &D = L->hpat[p];
+        D.i0 = P.i0; D.j0 = P.j0; D.nx = P.nx; D.ny = P.ny; D.off = off; D.ioff = ioff; D.pitch = P.nx + 4;
+        D.bcmask = (P.i0 - 2 < 0 ? 1 : 0) | ((int64_t)P.i0 + P.nx + 2 > nxl ? 2 : 0) | (P.j0 - 2 < 0 ? 4 : 0) | ((int64_t)P.j0 + P.ny + 2 > nyl ? 8 : 0);
+        off += (int64_t)(P.nx + 4) * (P.ny + 4);
+        ioff += (int64_t)P.nx * P.ny;
+        for (int64_t by = P.j0 / L->bsize; by <= (P.j0 + P.ny - 1) / L->bsize; by++)
+            for (int64_t bx = P.i0 / L->bsize; bx <= (P.i0 + P.nx - 1) / L->bsize; bx++)
+                L->buckets[bkey(bx, by)].push_back(p);
+    }
+    L->tot = off; L->ncells = ioff;
+    // overlap check (patches of a level are disjoint)
+    for (int p = 0; p < np; p++) {
+        const gc_patch &P = L->pat[p];
+        for (int64_t by = P.j0 / L->bsize; by <= (P.j0 + P.ny - 1) / L->bsize; by++)
+            for (int64_t bx = P.i0 / L->bsize; bx <= (P.i0 + P.nx - 1) / L->bsize; bx++)
+                for (int32_t q : L->buckets[bkey(bx, by)]) {
+                    if (q <= p) continue;
+                    const gc_patch &Q = L->pat[q];
+                    if (std::max(P.i0, Q.i0) < std::min(P.i0 + P.nx, Q.i0 + Q.nx) && std::max(P.j0, Q.j0) < std::min(P.j0 + P.ny, Q.j0 + Q.ny)) {
+                        delete L;
+                        return gc_fail(ctx, GC_ERR_BADARG, "gc_level_create: patches overlap");
+                    }
+                }
+    }
+    // pool: q[0][3], q[1][3], b, qs[3] = 10 planes, one allocation
+    int64_t plane = ((L->tot + 31) / 32) * 32 + 32;
+    L->pool = (double *)gc_dev_alloc(ctx, (size_t)plane * 10 * sizeof(double));
+    if (!L->pool) { delete L; return gc_fail(ctx, GC_ERR_NOMEM, "gc_level_create: pool allocation failed"); }
+    L->allocs.push_back(L->pool);
+    cudaMemsetAsync(L->pool, 0, (size_t)plane * 10 * sizeof(double), ctx->stream);
+    for (int w = 0; w < 2; w++) for (int f = 0; f < 3; f++) L->q[w][f] = L->pool + (int64_t)(w * 3 + f) * plane;
+    L->b = L->pool + 6 * plane;
+    for (int f = 0; f < 3; f++) L->qs[f] = L->pool + (int64_t)(7 + f) * plane;
+
+    build_metric(L);
+    L->d_kappa = upload(L, L->kappa); L->d_rdx = upload(L, L->rdx); L->d_rdy = upload(L, L->rdy); L->d_ey = upload(L, L->ey);
+    L->d_pat = upload(L, L->hpat);
+    std::vector<SweepTile> xt, yt;
+    build_tiles(L, xt, yt);
+    L->nxt = (int)xt.size(); L->nyt = (int)yt.size();
+    L->d_xt = upload(L, xt); L->d_yt = upload(L, yt);
+
+    // same-level copy rectangles: grown box of p  x  interior of q (A2, incl. corners)
+    std::vector<CopyRect> rects;
+    std::vector<int32_t> bcp;
+    std::vector<uint8_t> mask;
+    for (int p = 0; p < np; p++) {
+        const gc_patch &P = L->pat[p];
+        const PatchDesc &D = L->hpat[p];
+        if (D.bcmask) bcp.push_back(p);
+        int64_t gx0 = (int64_t)P.i0 - 2, gx1 = (int64_t)P.i0 + P.nx + 2, gy0 = (int64_t)P.j0 - 2, gy1 = (int64_t)P.j0 + P.ny + 2;
+        bool need_mask = level > 1;
+        if (need_mask) mask.assign((size_t)D.pitch * (P.ny + 4), 0);
+        size_t first = rects.size();
+        int64_t bx0 = std::max<int64_t>(gx0, 0) / L->bsize, bx1 = std::min<int64_t>(gx1 - 1, nxl - 1) / L->bsize;
+        int64_t by0 = std::max<int64_t>(gy0, 0) / L->bsize, by1 = std::min<int64_t>(gy1 - 1, nyl - 1) / L->bsize;
+        for (int64_t by = by0; by <= by1; by++) for (int64_t bx = bx0; bx <= bx1; bx++) {
+            auto it = L->buckets.find(bkey(bx, by));
+            if (it == L->buckets.end()) continue;
+            for (int32_t q : it->second) {
+                if (q == p) continue;
+                const gc_patch &Q = L->pat[q];
+                int64_t x0 = std::max<int64_t>(gx0, Q.i0), x1 = std::min<int64_t>(gx1, (int64_t)Q.i0 + Q.nx);
+                int64_t y0 = std::max<int64_t>(gy0, Q.j0), y1 = std::min<int64_t>(gy1, (int64_t)Q.j0 + Q.ny);
+                if (x0 >= x1 || y0 >= y1) continue;
+                const PatchDesc &DQ = L->hpat[q];
+                CopyRect r;
+                r.dst = D.off + (y0 - P.j0 + 2) * D.pitch + (x0 - P.i0 + 2);
+                r.src = DQ.off + (y0 - Q.j0 + 2) * DQ.pitch + (x0 - Q.i0 + 2);
+                r.w = (int)(x1 - x0); r.h = (int)(y1 - y0); r.dpitch = D.pitch; r.spitch = DQ.pitch;
+                // a patch spanning several buckets is met more than once: keep the first
+                bool dup = false;
+                for (size_t k = first; k < rects.size(); k++) if (rects[k].dst == r.dst) { dup = true; break; }
+                if (dup) continue;
+                rects.push_back(r);
+                if (need_mask)
+                    for (int64_t y = y0; y < y1; y++) for (int64_t x = x0; x < x1; x++)
+                        mask[(size_t)(y - P.j0 + 2) * D.pitch + (x - P.i0 + 2)] = 1;
+            }
+        }
+        if (need_mask) {   // in-domain ghost cells without a same-level source come from the coarser level (A3)
+            for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < D.pitch; i++) {
+                if (i >= 2 && i < P.nx + 2 && j >= 2 && j < P.ny + 2) continue;
+                int64_t gi = (int64_t)P.i0 + i - 2, gj = (int64_t)P.j0 + j - 2;
+                if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
+                if (mask[(size_t)j * D.pitch + i]) continue;
+                L->coarse_ghost.push_back(D.off + (int64_t)j * D.pitch + i);
+                L->coarse_ghost_ij.push_back((int32_t)gi); L->coarse_ghost_ij.push_back((int32_t)gj);
+            }
+        }
+    }
+    L->ncopy = (int)rects.size(); L->d_copy = upload(L, rects);
+    L->nbcp = (int)bcp.size(); L->d_bcp = upload(L, bcp);
+    L->d_stats = (DevStats *)gc_dev_alloc(ctx, sizeof(DevStats)); L->allocs.push_back(L->d_stats);
+    L->d_partial = (double *)gc_dev_alloc(ctx, sizeof(double) * (np > 0 ? np : 1)); L->allocs.push_back(L->d_partial);
+    L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->ncf = 0;
+    L->reg_fine = nullptr; L->reg_coarse = nullptr; L->d_reg = nullptr; L->nreg = 0;
+    L->d_delta = nullptr; L->d_base = nullptr; L->d_fixcell = nullptr; L->d_fixstart = nullptr; L->d_fixreg = nullptr; L->nfix = 0;
+    if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_copy || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
+        gc_level_destroy(L);
+        return gc_fail(ctx, GC_ERR_NOMEM, "gc_level_create: table allocation failed");
+    }
+    gc_launch_stats_reset(L);
+    cudaStreamSynchronize(ctx->stream);   // host vectors used by the uploads go out of scope
+    int rc = gc_cuda_check(ctx, "gc_level_create");
+    if (rc) { gc_level_destroy(L); return rc; }
+    *out = L;
+    return GC_OK;
+}
+
+extern "C" int gc_level_destroy(gc_level *L)
+{
+    if (!L) return GC_OK;
+    cudaStreamSynchronize(L->ctx->stream);
+    for (void *p : L->allocs) gc_dev_free(L->ctx, p);
+    delete L;
+    return GC_OK;
+}
+
+extern "C" int64_t gc_level_ncells(const gc_level *L) { return L ? L->ncells : 0; }
+
+static double *plane_of(const gc_level *L, int field, int which)
+{
+    if (field == GC_FIELD_B) return L->b;
+    return L->q[which == GC_NEW ? L->cur : 1 - L->cur][field];
+}
+
+extern "C" int gc_level_set_field(gc_level *L, int p, int field, const double *src, int is_device, int64_t ld)
+{
+    if (!L || p < 0 || p >= L->np || field < 0 || field > 3 || !src || ld < L->pat[p].nx + 4) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_set_field: bad argument");
+    const PatchDesc &D = L->hpat[p];
+    double *dst = plane_of(L, field, GC_NEW) + D.off;
+    cudaMemcpy2DAsync(dst, (size_t)D.pitch * 8, src, (size_t)ld * 8, (size_t)D.pitch * 8, D.ny + 4,
+                      is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, L->ctx->stream);
+    if (!is_device) cudaStreamSynchronize(L->ctx->stream);
+    return gc_cuda_check(L->ctx, "gc_level_set_field");
+}
+
+extern "C" int gc_level_get_field(const gc_level *L, int p, int field, int which, double *dst, int is_device, int64_t ld)
+{
+    if (!L || p < 0 || p >= L->np || field < 0 || field > 3 || !dst || ld < L->pat[p].nx + 4) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_get_field: bad argument");
+    const PatchDesc &D = L->hpat[p];
+    const double *src = plane_of(L, field, which) + D.off;
+    cudaMemcpy2DAsync(dst, (size_t)ld * 8, src, (size_t)D.pitch * 8, (size_t)D.pitch * 8, D.ny + 4,
+                      is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, L->ctx->stream);
+    if (!is_device) cudaStreamSynchronize(L->ctx->stream);
+    return gc_cuda_check(L->ctx, "gc_level_get_field");
+}
+
+extern "C" int gc_level_set_global(gc_level *L, int field, const double *src, int is_device, int64_t ld,
+                                   int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
+{
+    if (!L || field < 0 || field > 3 || !src || gnx < 1 || gny < 1 || ld < gnx) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_set_global: bad argument");
+    gc_ctx *c = L->ctx;
+    const double *dsrc = src; int64_t dld = ld; double *tmp = nullptr;
+    if (!is_device) {
+        tmp = (double *)gc_dev_alloc(c, (size_t)gnx * gny * 8);
+        if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_level_set_global: staging allocation failed");
+        cudaMemcpy2DAsync(tmp, (size_t)gnx * 8, src, (size_t)ld * 8, (size_t)gnx * 8, gny, cudaMemcpyHostToDevice, c->stream);
+        dsrc = tmp; dld = gnx;
+    }
+    gc_launch_set_global(L, plane_of(L, field, GC_NEW), dsrc, dld, gi0, gj0, gnx, gny);
+    if (tmp) { cudaStreamSynchronize(c->stream); gc_dev_free(c, tmp); }
+    return gc_cuda_check(c, "gc_level_set_global");
+}
+
+extern "C" int gc_level_get_global(const gc_level *L, int field, int which, double *dst, int is_device, int64_t ld,
+                                   int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
+{
+    if (!L || field < 0 || field > 3 || !dst || gnx < 1 || gny < 1 || ld < gnx) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_get_global: bad argument");
+    gc_ctx *c = L->ctx;
+    double *ddst = dst; int64_t dld = ld; double *tmp = nullptr;
+    if (!is_device) {
+        tmp = (double *)gc_dev_alloc(c, (size_t)gnx * gny * 8);
+        if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_level_get_global: staging allocation failed");
+        // cells not covered by a patch keep the caller's values
+        cudaMemcpy2DAsync(tmp, (size_t)gnx * 8, dst, (size_t)ld * 8, (size_t)gnx * 8, gny, cudaMemcpyHostToDevice, c->stream);
+        ddst = tmp; dld = gnx;
+    }
+    gc_launch_get_global(L, plane_of(L, field, which), ddst, dld, gi0, gj0, gnx, gny);
+    if (tmp) {
+        cudaMemcpy2DAsync(dst, (size_t)ld * 8, tmp, (size_t)gnx * 8, (size_t)gnx * 8, gny, cudaMemcpyDeviceToHost, c->stream);
+        cudaStreamSynchronize(c->stream);
+        gc_dev_free(c, tmp);
+    }
+    return gc_cuda_check(c, "gc_level_get_global");
+}
+
+extern "C" int gc_fill_ghost_b(gc_level *L)
+{
+    if (!L) return GC_ERR_BADARG;
+    gc_launch_copy_rects(L, L->b, nullptr, nullptr, 1);
+    gc_launch_bc(L, L->b, nullptr, nullptr, 1, 0);
+    return gc_cuda_check(L->ctx, "gc_fill_ghost_b");
+}
+
+int gc_fill_coarse_ghosts(gc_level *L, const gc_level *C, double alpha);   // gc_api_amr.cu
+int gc_flux_after_step(gc_level *L, double dt, const double *dt_dev);     // gc_api_amr.cu
+
+extern "C" int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha)
+{
+    if (!L) return GC_ERR_BADARG;
+    double **q = L->q[L->cur];
+    gc_launch_copy_rects(L, q[0], q[1], q[2], 3);
+    if (coarser) {
+        int rc = gc_fill_coarse_ghosts(L, coarser, alpha);
+        if (rc) return rc;
+    } else if (!L->coarse_ghost.empty()) {
+        return gc_fail(L->ctx, GC_ERR_STATE, "gc_fill_ghost: ghost cells need a coarser level");
+    }
+    gc_launch_bc(L, q[0], q[1], q[2], 3, 1);
+    return gc_cuda_check(L->ctx, "gc_fill_ghost");
+}
+
+extern "C" int gc_level_stats(const gc_level *L, gc_step_stats *out)
+{
+    if (!L || !out) return GC_ERR_BADARG;
+    DevStats s;
+    cudaMemcpyAsync(&s, L->d_stats, sizeof s, cudaMemcpyDeviceToHost, L->ctx->stream);
+    cudaStreamSynchronize(L->ctx->stream);
+    int rc = gc_cuda_check(L->ctx, "gc_level_stats");
+    if (rc) return rc;
+    double sdx; memcpy(&sdx, &s.sdx_bits, 8);
+    out->s_over_dx_max = sdx; out->cfl_max = 0.0; out->clipped_mass = s.clipped; out->n_clipped = (int64_t)s.nclip; out->nan_seen = s.nan_seen;
+    return GC_OK;
+}
+
+extern "C" int gc_level_step(gc_level *L, double dt, gc_step_stats *out)
+{
+    if (!L || !(dt >= 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step: bad argument");
+    gc_launch_stats_reset(L);
+    gc_launch_sweeps(L, dt, nullptr, dt > 0.0 ? 1 : 0);
+    if (dt > 0.0) {
+        L->cur = 1 - L->cur;
+        int rc = gc_flux_after_step(L, dt, nullptr);
+        if (rc) return rc;
+    }
+    int rc = gc_cuda_check(L->ctx, "gc_level_step");
+    if (rc) return rc;
+    if (out) {
+        rc = gc_level_stats(L, out);
+        if (rc) return rc;
+        out->cfl_max = dt * out->s_over_dx_max;
+        if (out->nan_seen) return gc_fail(L->ctx, GC_ERR_NAN, "gc_level_step: NaN in the updated state");
+    }
+    return GC_OK;
+}
+
+extern "C" int gc_level_step_auto(gc_level *L, double *dt_dev, double cfl_target)
+{
+    if (!L || !dt_dev || !(cfl_target > 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step_auto: bad argument");
+    gc_launch_stats_reset(L);
+    gc_launch_sweeps(L, 0.0, dt_dev, 1);
+    L->cur = 1 - L->cur;
+    int rc = gc_flux_after_step(L, 0.0, dt_dev);
+    if (rc) return rc;
+    gc_launch_next_dt(L, dt_dev, cfl_target);
+    return gc_cuda_check(L->ctx, "gc_level_step_auto");
+}
+
+extern "C" int gc_wet_mask(const gc_level *L, uint8_t *mask, int is_device)
+{
+    if (!L || !mask) return GC_ERR_BADARG;
+    gc_ctx *c = L->ctx;
+    uint8_t *d = mask;
+    if (!is_device) { d = (uint8_t *)gc_dev_alloc(c, (size_t)L->ncells); if (!d) return gc_fail(c, GC_ERR_NOMEM, "gc_wet_mask: allocation failed"); }
+    gc_launch_wet_mask(L, d);
+    if (!is_device) {
+        cudaMemcpyAsync(mask, d, (size_t)L->ncells, cudaMemcpyDeviceToHost, c->stream);
+        cudaStreamSynchronize(c->stream);
+        gc_dev_free(c, d);
+    }
+    return gc_cuda_check(c, "gc_wet_mask");
+}
+
+extern "C" double gc_level_mass(const gc_level *L)
+{
+    if (!L) return NAN;
+    gc_launch_mass(L);
+    std::vector<double> part(L->np > 0 ? L->np : 1, 0.0);
+    cudaMemcpyAsync(part.data(), L->d_partial, sizeof(double) * L->np, cudaMemcpyDeviceToHost, L->ctx->stream);
+    cudaStreamSynchronize(L->ctx->stream);
+    if (gc_cuda_check(L->ctx, "gc_level_mass")) return NAN;
+    double m = 0.0;
+    for (int p = 0; p < L->np; p++) m += part[p];
+    return m;
+}
+
+extern "C" int gc_probe_fp64_peak(gc_ctx *c, double *flops_out)
+{
+    if (!c || !flops_out) return GC_ERR_BADARG;
+    double *d = (double *)gc_dev_alloc(c, 64);
+    if (!d) return gc_fail(c, GC_ERR_NOMEM, "gc_probe_fp64_peak: allocation failed");
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const int iters = 1 << 16, threads = 512, blocks = nsm * 4;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    gc_launch_fp64_probe(c->stream, d, 1024, blocks, threads);   // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; rep++) {
+        cudaEventRecord(e0, c->stream);
+        gc_launch_fp64_probe(c->stream, d, iters, blocks, threads);
+        cudaEventRecord(e1, c->stream);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    gc_dev_free(c, d);
+    int rc = gc_cuda_check(c, "gc_probe_fp64_peak");
+    if (rc) return rc;
+    *flops_out = 2.0 * 8.0 * (double)iters * threads * blocks / (best * 1e-3);
+    return GC_OK;
+}

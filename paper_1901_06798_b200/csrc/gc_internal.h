@@ -1,0 +1,138 @@
+// gc_internal.h -- internals of libgeoclaw_b200.so (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <unordered_map>
+#include <vector>
+#include "../../include/gc.h"
+
+#define GC_G 2  // ghost width
+
+// patch descriptor as the kernels see it (A1): interior box, element offset of the patch in a field plane, row pitch
+struct PatchDesc {
+    int32_t i0, j0, nx, ny;
+    int64_t off;     // element offset in every field plane of the pool
+    int64_t ioff;    // offset in interior-packed arrays (masks, flags)
+    int32_t pitch;   // nx + 4
+    int32_t bcmask;  // bit0 touches xlo, bit1 xhi, bit2 ylo, bit3 yhi
+};
+
+// work item of a sweep kernel: a group of lines (rows for x, columns for y) times a segment along the sweep
+struct SweepTile {
+    int32_t patch;
+    int32_t line0, nlines;  // rows [line0, line0+nlines) (x-sweep) or columns (y-sweep), storage indices
+    int32_t c0, nc;         // cells [c0, c0+nc) along the sweep direction, storage indices (edges c0-1 .. c0+nc+1 are solved)
+};
+
+// same-level ghost copy: rectangle of w x h cells
+struct CopyRect {
+    int64_t dst, src;       // element offsets in a field plane
+    int32_t w, h, dpitch, spitch;
+};
+
+// one fine cell to be interpolated from the coarser level (ghost fill A3 / regrid transfer A11)
+struct CoarseFillItem {
+    int64_t dst;            // element offset in the fine plane
+    int64_t csrc;           // element offset of the coarse cell (I,J) in the coarse plane
+    int32_t cpitch;         // pitch of that coarse patch
+    int16_t ii, jj;         // position of the fine cell inside the coarse cell, 0..r-1
+};
+
+struct AvgItem {            // average-down A9: one covered coarse cell
+    int64_t cdst;           // coarse plane offset
+    int64_t fsrc;           // fine plane offset of the lower-left fine cell
+    int32_t fpitch;
+    int32_t frow;           // global fine row of the lower-left fine cell (for kappa weights)
+};
+
+struct FluxReg {            // A8, one register (coarse edge on the boundary of the fine region)
+    int64_t ccell;          // coarse plane offset of the uncovered coarse cell C
+    int64_t fcell;          // fine plane offset of the first adjacent fine cell
+    int32_t cpitch, fpitch;
+    int32_t crow, frow;     // global rows (coarse cell / first fine cell) for metric tables
+    int32_t dir, side;      // dir 0: x-edge, 1: y-edge; side +1: fine region on the high side of C
+};
+
+struct DevStats {
+    unsigned long long sdx_bits;   // max of s/(kappa dx) as the bit image of a non-negative double
+    unsigned long long nclip;
+    double clipped;
+    int nan_seen;
+    int pad;
+};
+
+struct gc_ctx {
+    gc_params P;
+    cudaStream_t stream;
+    gc_alloc_fn alloc;
+    gc_free_fn free_;
+    void *user;
+    std::string err;
+};
+
+struct gc_level {
+    gc_ctx *ctx;
+    int level, ratio, np, cur;
+    double xlo, ylo, dx, dy, ex;
+    int64_t nxl, nyl, ncells, tot;
+    std::vector<gc_patch> pat;
+    std::unordered_map<int64_t, std::vector<int32_t>> buckets; int bsize;   // spatial hash of patch interiors (host lookups)
+    std::vector<PatchDesc> hpat;
+    std::vector<double> kappa, rdx, rdy, ey;        // host copies of the metric tables
+    // device pool: q[2][3], b, qs[3] are planes of `tot` doubles inside one allocation
+    double *pool;
+    double *q[2][3];
+    double *b;
+    double *qs[3];
+    PatchDesc *d_pat;
+    double *d_kappa, *d_rdx, *d_rdy, *d_ey;
+    SweepTile *d_xt, *d_yt; int nxt, nyt;
+    CopyRect *d_copy; int ncopy;
+    int32_t *d_bcp; int nbcp;                       // patches touching the physical boundary
+    std::vector<int64_t> coarse_ghost;              // plane offsets + global indices of ghosts to be filled from the coarser level
+    std::vector<int32_t> coarse_ghost_ij;           // (gi, gj) pairs
+    // cached coarse-fill list for a given coarser level (rebuilt when the coarser level changes)
+    const gc_level *cf_for; uint64_t cf_gen; CoarseFillItem *d_cf; int64_t ncf;
+    uint64_t gen;                                   // unique id of this level object
+    DevStats *d_stats;
+    double *d_partial;                              // np doubles (mass partials)
+    std::vector<void *> allocs;
+    // flux registers (this level as the coarse side) + capture slots
+    const gc_level *reg_fine; gc_level *reg_coarse;
+    FluxReg *d_reg; int nreg; int r_reg;
+    double *d_delta, *d_base;                       // nreg*3, nreg*4
+    int64_t *d_fixcell; int32_t *d_fixstart; int nfix;  // registers grouped by coarse cell for the fix-up
+    int32_t *d_fixreg;
+};
+
+// ---- helpers (gc_api.cu)
+void *gc_dev_alloc(gc_ctx *c, size_t bytes);
+void gc_dev_free(gc_ctx *c, void *p);
+int gc_fail(gc_ctx *c, int code, const char *msg);
+int gc_cuda_check(gc_ctx *c, const char *what);
+int gc_find_patch_host(const gc_level *L, int64_t gi, int64_t gj);
+
+// ---- kernel launch wrappers
+// gc_sweep.cu
+void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out);
+void gc_launch_stats_reset(gc_level *L);
+void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl_target);
+void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, int threads);
+// gc_ghost.cu
+void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);
+void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int is_state);
+void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
+void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
+void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *src, int64_t sld, int w, int h);
+void gc_launch_wet_mask(const gc_level *L, uint8_t *mask);
+void gc_launch_mass(const gc_level *L);
+// gc_amr.cu
+void gc_launch_coarse_fill(gc_level *L, const gc_level *C, const CoarseFillItem *items, int64_t n, double alpha, int use_old);
+void gc_launch_average_down(gc_level *C, const gc_level *F, const AvgItem *items, int64_t n);
+void gc_launch_flags(const gc_level *L, const gc_flag_params *fp, const double *d_boxes, double t, uint8_t *raw, uint8_t *flags,
+                     const int32_t *nbr_start, const int32_t *nbr_list);
+void gc_launch_copy_overlap(gc_level *N, const gc_level *O, const CopyRect *rects, int n);
+void gc_launch_flux_coarse(gc_level *C, double dt);
+void gc_launch_flux_fine(gc_level *F, double dt);
+void gc_launch_flux_fixup(gc_level *C);

@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element on the same
+seeded inputs.  Bars (BASELINE.json north_star): wet masks bit-exact; dt within 1e-14 relative per step;
+h, hu, hv within 1e-12 relative per step and 1e-9 max|eta| at the end.  The design is bit-reproducible
+(-fmad=false on the device, -ffp-contract=off on the host), so the expected difference is exactly 0 and
+the tests assert that where noted."""
+import numpy as np
+import pytest
+
+import workloads
+from paper_1901_06798_b200 import driver
+
+pytestmark = pytest.mark.gpu
+G = 9.81
+
+
+def unpack(L, packed):
+    """interior-packed per-patch array -> level-global 2-D array"""
+    out = np.full((L.nyl, L.nxl), 255, dtype=packed.dtype)
+    o = 0
+    for i0, j0, nx, ny in L.patches:
+        out[j0:j0 + ny, i0:i0 + nx] = packed[o:o + nx * ny].reshape(ny, nx)
+        o += nx * ny
+    return out
+
+
+def lockstep(Lg, Lo, nsteps, cfl, eta_scale, exact=True, hmax=None):
+    """Advance both backends with their own dt control; compare every step."""
+    dtg = driver.probe_dt(Lg, cfl)
+    dto = driver.probe_dt(Lo, cfl)
+    worst = dict(dt=0.0, h=0.0, hu=0.0, hv=0.0)
+    for n in range(nsteps):
+        assert abs(dtg - dto) <= 1e-14 * dto, (n, dtg, dto)
+        Lg.fill_ghost(None, 1.0); Lo.fill_ghost(None, 1.0)
+        sg = Lg.step(dtg); so = Lo.step(dto)
+        worst["dt"] = max(worst["dt"], abs(dtg - dto) / dto)
+        assert sg["n_clipped"] == so["n_clipped"], n
+        assert abs(sg["clipped_mass"] - so["clipped_mass"]) <= 1e-12 * abs(so["clipped_mass"]) + 1e-300
+        assert sg["nan_seen"] == 0 and so["nan_seen"] == 0
+        assert abs(sg["s_over_dx_max"] - so["s_over_dx_max"]) <= 1e-14 * so["s_over_dx_max"]
+        assert np.array_equal(unpack(Lg, Lg.wet_mask()), unpack(Lo, Lo.wet_mask())), "wet mask differs at step %d" % n
+        ho = Lo.get_global("h")
+        hscale = np.nanmax(np.abs(ho))
+        mscale = max(np.nanmax(np.abs(Lo.get_global("hu"))), np.nanmax(np.abs(Lo.get_global("hv"))), eta_scale * np.sqrt(G * hscale))
+        for f, sc in (("h", hscale), ("hu", mscale), ("hv", mscale)):
+            a, c = Lg.get_global(f), Lo.get_global(f)
+            assert np.array_equal(np.isnan(a), np.isnan(c))
+            d = np.nanmax(np.abs(a - c))
+            worst[f] = max(worst[f], d / sc)
+            assert d <= 1e-12 * sc, (f, n, d, sc)
+        dtg = cfl / sg["s_over_dx_max"]; dto = cfl / so["s_over_dx_max"]
+    if exact:
+        assert worst["h"] == 0.0 and worst["hu"] == 0.0 and worst["hv"] == 0.0 and worst["dt"] == 0.0, worst
+    return worst
+
+
+def both(gc, gco, wl, patches_g=None, patches_o=None, **kw):
+    cg = gc.Context(**wl.params); co = gco.Context(**wl.params)
+    Lg = driver.setup_level(cg, wl, patches=patches_g, **kw)
+    Lo = driver.setup_level(co, wl, patches=patches_o, **kw)
+    return Lg, Lo
+
+
+def test_config1_100_steps(gc, gco):
+    wl = workloads.cfg1()
+    Lg, Lo = both(gc, gco, wl)
+    lockstep(Lg, Lo, 100, wl.cfl, 1.0)
+    assert abs(Lg.mass() - Lo.mass()) <= 1e-13 * Lo.mass()
+    for f in ("h", "hu", "hv", "b"):  # ghost cells too (physical boundary A4)
+        Lg.fill_ghost(None, 1.0); Lo.fill_ghost(None, 1.0)
+        assert np.array_equal(Lg.get_field(0, f), Lo.get_field(0, f))
+
+
+def test_config2_wet_dry_reduced(gc, gco):
+    """config 2 at 128 x 128 (same recipe), 300 steps of run-up; masks bit-exact every step."""
+    wl = workloads.cfg2(128)
+    Lg, Lo = both(gc, gco, wl)
+    w = Lo.wet_mask()
+    assert 0 < w.sum() < w.size
+    lockstep(Lg, Lo, 300, wl.cfl, 2.0)
+
+
+@pytest.mark.parametrize("bc", [(1, 1, 1, 1), (0, 0, 0, 0), (1, 0, 0, 1)])
+def test_tilings_match_single_patch_oracle(gc, gco, bc):
+    """A2 + A4: any partition of the level into patches (ragged sizes, several tiles, corners) gives the bits of
+    the oracle's single-patch run."""
+    n = 48
+    wl = workloads.cfg2(n)
+    wl.params = dict(wl.params, bc=bc)
+    tilings = [
+        workloads.tile(n, n, 16),
+        np.array([[0, 0, 20, 48], [20, 0, 28, 10], [20, 10, 28, 38]], dtype=np.int32),
+        workloads.tile(n, n, 2),
+        workloads.tile(n, n, 6),
+    ]
+    for pats in tilings:
+        Lg, Lo = both(gc, gco, wl, patches_g=pats)
+        lockstep(Lg, Lo, 30, wl.cfl, 2.0)
+
+
+def test_long_rows_and_columns_chunking(gc, gco):
+    """patch wider than one x-tile (nx + 3 > 256) and taller than one y-segment; odd sizes."""
+    wl = workloads.cfg2(64)
+    wl.nx, wl.ny = 301, 37
+    Lg, Lo = both(gc, gco, wl)
+    lockstep(Lg, Lo, 20, wl.cfl, 2.0)
+    wl.nx, wl.ny = 11, 277
+    Lg, Lo = both(gc, gco, wl)
+    lockstep(Lg, Lo, 20, wl.cfl, 2.0)
+
+
+def test_config5_reduced_spherical_tilings(gc, gco):
+    """config 5 recipe at 256 x 256 (0.5 arcmin, spherical, extrapolation): tilings 16, 32, 64, 128, 256 against the
+    oracle's single patch (tiling invariance makes them comparable)."""
+    n = 256
+    wl = workloads.cfg5(n)
+    for side in (16, 32, 64, 128, 256):
+        Lg, Lo = both(gc, gco, wl, patches_g=workloads.tile(n, n, side))
+        lockstep(Lg, Lo, 8, wl.cfl, 1.0)
+
+
+def test_spherical_walls(gc, gco):
+    n = 40
+    wl = workloads.cfg3(n)
+    wl.params = dict(wl.params, bc=(1, 1, 1, 1))
+    Lg, Lo = both(gc, gco, wl, patches_g=workloads.tile(n, n, 10))
+    lockstep(Lg, Lo, 20, wl.cfl, 0.5)
+
+
+def test_first_order_mode(gc, gco):
+    wl = workloads.cfg2(64)
+    wl.params = dict(wl.params, limiter=0)
+    Lg, Lo = both(gc, gco, wl)
+    lockstep(Lg, Lo, 40, wl.cfl, 2.0)
+
+
+def test_step_auto_device_dt_chain(gc, gco):
+    """gc_level_step_auto keeps dt on the device: same states and dt sequence as the host-controlled loop."""
+    import torch
+    wl = workloads.cfg1()
+    Lg, Lo = both(gc, gco, wl)
+    dto = driver.probe_dt(Lo, wl.cfl)
+    dtg = driver.probe_dt(Lg, wl.cfl)
+    dt_dev = torch.tensor([dtg], dtype=torch.float64, device="cuda")
+    for n in range(25):
+        Lg.fill_ghost(None, 1.0); Lo.fill_ghost(None, 1.0)
+        Lg.step_auto(dt_dev, wl.cfl)
+        so = Lo.step(dto)
+        dto = wl.cfl / so["s_over_dx_max"]
+    assert dt_dev.item() == dto
+    for f in ("h", "hu", "hv"):
+        assert np.array_equal(Lg.get_global(f), Lo.get_global(f))
+
+
+def test_empty_level_and_bad_arguments(gc):
+    ctx = gc.Context(coord=0)
+    L = ctx.level_create(1, 0.0, 0.0, 1.0, 1.0, 16, 16, 1, np.zeros((0, 4), dtype=np.int32))
+    L.fill_ghost(None, 1.0)
+    st = L.step(1.0)
+    assert st["s_over_dx_max"] == 0.0 and L.ncells == 0
+    with pytest.raises(RuntimeError):
+        ctx.level_create(1, 0.0, 0.0, 1.0, 1.0, 16, 16, 1, np.array([[0, 0, 8, 8], [4, 4, 8, 8]], dtype=np.int32))  # overlap
+    with pytest.raises(RuntimeError):
+        ctx.level_create(1, 0.0, 0.0, 1.0, 1.0, 16, 16, 1, np.array([[10, 0, 8, 8]], dtype=np.int32))  # outside
+    with pytest.raises(RuntimeError):
+        ctx.level_create(2, 0.0, 0.0, 1.0, 1.0, 16, 16, 4, np.array([[2, 0, 8, 8]], dtype=np.int32))  # not aligned
+
+
+def test_device_tensor_io(gc):
+    import torch
+    wl = workloads.cfg1(32)
+    ctx = gc.Context(**wl.params)
+    L = ctx.level_create(1, 0.0, 0.0, wl.dx, wl.dy, 32, 32, 1, workloads.tile(32, 32, 16))
+    b, h, hu, hv = wl.fields()
+    L.set_global("h", torch.from_numpy(h).cuda())
+    out = torch.full((32, 32), float("nan"), dtype=torch.float64, device="cuda")
+    L.get_global("h", out=out)
+    assert np.array_equal(out.cpu().numpy(), h)
