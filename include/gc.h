@@ -140,6 +140,16 @@ int gc_level_init_from(gc_level *newfine, const gc_level *oldfine, const gc_leve
 int gc_flux_attach(gc_level *coarse, gc_level *fine);
 int gc_flux_fixup(gc_level *coarse, gc_level *fine);
 
+/* Kernel accounting.  gc_launch_count: kernels launched by this context so far.  gc_profile_enable(on): bracket
+ * every kernel group with CUDA events on the context's stream; gc_profile_read synchronises, returns per slot the
+ * summed milliseconds and the number of bracketed groups since the last read (arrays of GC_PROFILE_SLOTS), and clears.
+ * Slots: 0 same-level copy, 1 physical BC, 2 x-sweep, 3 y-sweep, 4 coarse fill, 5 average-down / regrid transfer,
+ * 6 flags, 7 flux registers, 8 misc (stats, dt), 9 fused sweep. */
+#define GC_PROFILE_SLOTS 10
+int64_t gc_launch_count(const gc_ctx *);
+int gc_profile_enable(gc_ctx *, int on);
+int gc_profile_read(gc_ctx *, double *ms /*HOST*/, int64_t *count /*HOST*/);
+
 /* Measured fp64 ALU throughput of this device (DFMA micro-benchmark, flop/s); for the "alu" roofline. */
 int gc_probe_fp64_peak(gc_ctx *, double *flops_out /*HOST*/);
 

@@ -17,6 +17,7 @@ SYMBOLS = [
     "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
+    "gc_launch_count", "gc_profile_enable", "gc_profile_read",
 ]
 
 
@@ -74,6 +75,9 @@ def lib():
     L.gc_flux_attach.argtypes = [vp, vp]
     L.gc_flux_fixup.argtypes = [vp, vp]
     L.gc_probe_fp64_peak.argtypes = [vp, vp]
+    L.gc_launch_count.argtypes = [vp]; L.gc_launch_count.restype = i64
+    L.gc_profile_enable.argtypes = [vp, i]
+    L.gc_profile_read.argtypes = [vp, vp, vp]
     _lib = L
     return L
 
@@ -243,6 +247,19 @@ class Context:
         v = C.c_double(0.0)
         self._chk(lib().gc_probe_fp64_peak(self.h, C.byref(v)), "gc_probe_fp64_peak")
         return v.value
+
+    def launch_count(self):
+        return int(lib().gc_launch_count(self.h))
+
+    def profile(self, on):
+        self._chk(lib().gc_profile_enable(self.h, 1 if on else 0), "gc_profile_enable")
+
+    def profile_read(self):
+        """-> {slot name: (milliseconds, groups)} since the last read"""
+        ms = (C.c_double * 10)(); cnt = (C.c_int64 * 10)()
+        self._chk(lib().gc_profile_read(self.h, ms, cnt), "gc_profile_read")
+        names = ["copy", "bc", "xsweep", "ysweep", "coarse", "avg", "flag", "flux", "misc", "fused"]
+        return {n: (ms[k], cnt[k]) for k, n in enumerate(names)}
 
     def synchronize(self):
         self.stream.synchronize()

@@ -51,6 +51,25 @@ extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc
 }
 extern "C" int gc_ctx_destroy(gc_ctx *c) { delete c; return GC_OK; }
 
+extern "C" int64_t gc_launch_count(const gc_ctx *c) { return c ? (int64_t)c->launches : 0; }
+extern "C" int gc_profile_enable(gc_ctx *c, int on) { if (!c) return GC_ERR_BADARG; c->prof = on != 0; return GC_OK; }
+extern "C" int gc_profile_read(gc_ctx *c, double *ms, int64_t *count)
+{
+    if (!c || !ms || !count) return GC_ERR_BADARG;
+    cudaStreamSynchronize(c->stream);
+    for (int s = 0; s < GC_NSLOT; s++) {
+        ms[s] = 0.0; count[s] = (int64_t)c->ev[s].size();
+        for (auto &p : c->ev[s]) {
+            float t = 0.f;
+            cudaEventElapsedTime(&t, p.first, p.second);
+            ms[s] += t;
+            cudaEventDestroy(p.first); cudaEventDestroy(p.second);
+        }
+        c->ev[s].clear();
+    }
+    return gc_cuda_check(c, "gc_profile_read");
+}
+
 template <class T> static T *upload(gc_level *L, const std::vector<T> &v)
 {
     T *d = (T *)gc_dev_alloc(L->ctx, v.size() * sizeof(T));

@@ -26,6 +26,7 @@ void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int n
     if (L->ncopy == 0) return;
     int threads = 256;
     int64_t blocks = ((int64_t)L->ncopy * 32 + threads - 1) / threads;
+    ProfScope ps(L->ctx, GC_SLOT_COPY);
     k_copy_rects<<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->ncopy, f0, f1, f2, nf);
 }
 
@@ -81,6 +82,7 @@ void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int i
 {
     if (L->nbcp == 0) return;
     const int *bc = L->ctx->P.bc;
+    ProfScope ps(L->ctx, GC_SLOT_BC, 2);
     for (int pass = 0; pass < 2; pass++)
         k_bc<<<L->nbcp, 128, 0, L->ctx->stream>>>(L->d_pat, L->d_bcp, f0, f1, f2, nf, is_state, pass, L->nxl, L->nyl,
                                                   bc[0], bc[1], bc[2], bc[3]);
@@ -115,10 +117,12 @@ __global__ void k_get_global(const PatchDesc *pat, const double *plane, double *
 
 void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
     if (L->np) k_set_global<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, plane, src, ld, gi0, gj0, gnx, gny);
 }
 void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
     if (L->np) k_get_global<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, plane, dst, ld, gi0, gj0, gnx, gny);
 }
 
@@ -149,6 +153,7 @@ __global__ void k_wet_mask(const PatchDesc *pat, const double *h, double eps, ui
 }
 void gc_launch_wet_mask(const gc_level *L, uint8_t *mask)
 {
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
     if (L->np) k_wet_mask<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->ctx->P.dry_tol, mask);
 }
 
@@ -174,5 +179,6 @@ __global__ void k_mass(const PatchDesc *pat, const double *h, const double *kapp
 }
 void gc_launch_mass(const gc_level *L)
 {
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
     if (L->np) k_mass<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->d_kappa, L->dx * L->dy, L->d_partial);
 }

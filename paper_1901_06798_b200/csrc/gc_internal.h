@@ -62,6 +62,10 @@ struct DevStats {
     int pad;
 };
 
+// profiling slots (gc_profile_read): kernels grouped by the SURVEY 8(a) row they implement
+enum { GC_SLOT_COPY = 0, GC_SLOT_BC = 1, GC_SLOT_XSWEEP = 2, GC_SLOT_YSWEEP = 3, GC_SLOT_COARSE = 4, GC_SLOT_AVG = 5,
+       GC_SLOT_FLAG = 6, GC_SLOT_FLUX = 7, GC_SLOT_MISC = 8, GC_SLOT_FUSED = 9, GC_NSLOT = 10 };
+
 struct gc_ctx {
     gc_params P;
     cudaStream_t stream;
@@ -69,6 +73,20 @@ struct gc_ctx {
     gc_free_fn free_;
     void *user;
     std::string err;
+    bool prof = false;
+    unsigned long long launches = 0;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];
+};
+
+// counts kernel launches; when profiling is on, brackets them with CUDA events on the launching stream
+struct ProfScope {
+    gc_ctx *c; int slot; cudaEvent_t e0, e1;
+    ProfScope(gc_ctx *c_, int slot_, int nlaunch = 1) : c(c_), slot(slot_), e0(nullptr), e1(nullptr)
+    {
+        c->launches += nlaunch;
+        if (c->prof) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventRecord(e0, c->stream); }
+    }
+    ~ProfScope() { if (e0) { cudaEventRecord(e1, c->stream); c->ev[slot].push_back({e0, e1}); } }
 };
 
 struct gc_level {

@@ -187,9 +187,9 @@ __global__ void k_next_dt(const DevStats *s, double *dt_dev, double cfl)
     *dt_dev = cfl / sdx;
 }
 
-void gc_launch_stats_reset(gc_level *L) { k_stats_reset<<<1, 1, 0, L->ctx->stream>>>(L->d_stats); }
+void gc_launch_stats_reset(gc_level *L) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_stats_reset<<<1, 1, 0, L->ctx->stream>>>(L->d_stats); }
 
-void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl) { k_next_dt<<<1, 1, 0, L->ctx->stream>>>(L->d_stats, dt_dev, cfl); }
+void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_next_dt<<<1, 1, 0, L->ctx->stream>>>(L->d_stats, dt_dev, cfl); }
 
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out)
 {
@@ -202,11 +202,11 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     // x-sweep: Q^n -> Q*
     a.tiles = L->d_xt; a.h = L->q[cur][0]; a.hu = L->q[cur][1]; a.hv = L->q[cur][2];
     a.oh = L->qs[0]; a.ohu = L->qs[1]; a.ohv = L->qs[2]; a.rd = L->d_rdx;
-    if (L->nxt > 0) k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a);
+    if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
     // y-sweep: Q* -> Q^{n+1}
     a.tiles = L->d_yt; a.h = L->qs[0]; a.hu = L->qs[1]; a.hv = L->qs[2];
     a.oh = L->q[nxt][0]; a.ohu = L->q[nxt][1]; a.ohv = L->q[nxt][2]; a.rd = L->d_rdy;
-    if (L->nyt > 0) k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a);
+    if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
 }
 
 // ---- fp64 ALU peak probe: dependent DFMA chains, 8 independent accumulators per thread
