@@ -1,0 +1,91 @@
+// gc_scheme.cuh -- the per-edge arithmetic of the wave-propagation scheme shared by every kernel that needs
+// a flux-like quantity at an edge (sweep kernels A5/A6, flux registers A8).
+//
+// P:65-105 (eqs. 4-11) in f-wave form; (1) Riemann solve (gc_riemann.cuh), (2) edge scaling
+// on the sphere, (3) fluctuations A-dQ / A+dQ (eq. 5-6, tie S-4), (4) MC-limited waves
+// (eq. 10-11, S-1), (5) correction flux (eq. 9), (6) fm = F~ + A-dQ, fp = F~ - A+dQ.
+// Every expression is written in the order of DESIGN.md so that, with -fmad=false, all users get the same bits.
+#pragma once
+#include "gc_riemann.cuh"
+
+struct Waves { double Z[3][3]; double s[3]; };
+
+// (1)+(2): solve the edge between two cells given as raw (h, p, t, b) and scale by the edge factor ef
+__device__ __forceinline__ void gc_solve_edge(double g, double eps, RState L, RState R, int coord, double ef, Waves &W)
+{
+    gc_prim(L, g, eps);
+    gc_prim(R, g, eps);
+    gc_riemann(g, eps, L, R, W.Z, W.s);
+    if (coord == 1) {
+#pragma unroll
+        for (int w = 0; w < 3; w++) { W.s[w] = W.s[w] * ef; W.Z[w][0] = W.Z[w][0] * ef; W.Z[w][1] = W.Z[w][1] * ef; W.Z[w][2] = W.Z[w][2] * ef; }
+    }
+}
+
+// same with the primitive variables of both sides already computed (gc_prim applied by the caller)
+__device__ __forceinline__ void gc_solve_edge_prim(double g, double eps, const RState &L, const RState &R, int coord, double ef, Waves &W)
+{
+    gc_riemann(g, eps, L, R, W.Z, W.s);
+    if (coord == 1) {
+#pragma unroll
+        for (int w = 0; w < 3; w++) { W.s[w] = W.s[w] * ef; W.Z[w][0] = W.Z[w][0] * ef; W.Z[w][1] = W.Z[w][1] * ef; W.Z[w][2] = W.Z[w][2] * ef; }
+    }
+}
+
+// MC limiter value for one family: zi = Z_I . Z_e, zz = Z_e . Z_e (zz != 0)
+__device__ __forceinline__ double gc_mc(double zi, double zz)
+{
+    double theta = zi / zz;                                                     // eq. 10 (S-1)
+    return dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));        // MC
+}
+
+// (3)-(6) for edge e.  ZN(w, c, up) returns component c of family w of the neighbour edge: up = -1 -> edge e-1,
+// up = +1 -> edge e+1 (eq. 11: I = e-1 if s > 0, e+1 if s < 0).  rdL, rdR = 1/(kappa dx) of the left / right cell.
+template <class NB>
+__device__ __forceinline__ void gc_edge_flux(const Waves &W, NB ZN, int limiter, double dt, double rdL, double rdR,
+                                             double (&fm)[3], double (&fp)[3])
+{
+    double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int w = 0; w < 3; w++) {
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            if (W.s[w] < 0.0) am[c] = am[c] + W.Z[w][c];
+            else if (W.s[w] > 0.0) ap[c] = ap[c] + W.Z[w][c];
+            else { am[c] = am[c] + 0.5 * W.Z[w][c]; ap[c] = ap[c] + 0.5 * W.Z[w][c]; }
+        }
+    }
+    if (limiter != 0) {
+        double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+#pragma unroll
+        for (int w = 0; w < 3; w++) {
+            double sw = W.s[w];
+            if (sw != 0.0) {
+                double zz = (W.Z[w][0] * W.Z[w][0] + W.Z[w][1] * W.Z[w][1]) + W.Z[w][2] * W.Z[w][2];
+                double phi = 1.0;
+                if (zz != 0.0) {
+                    int up = (sw > 0.0) ? -1 : 1;
+                    double zi = (ZN(w, 0, up) * W.Z[w][0] + ZN(w, 1, up) * W.Z[w][1]) + ZN(w, 2, up) * W.Z[w][2];
+                    phi = gc_mc(zi, zz);
+                }
+                double coef = ((sw > 0.0) ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
+#pragma unroll
+                for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[w][c]);   // eq. 9
+            }
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
+}
+
+// eq. 15: right-going waves enter the right cell, left-going waves the left cell
+__device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double rdR)
+{
+    double m = 0.0;
+#pragma unroll
+    for (int w = 0; w < 3; w++) {
+        m = dmax(m, dmax(W.s[w], 0.0) * rdR);
+        m = dmax(m, dmax(-W.s[w], 0.0) * rdL);
+    }
+    return m;
+}
