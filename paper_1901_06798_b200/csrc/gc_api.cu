@@ -3,6 +3,7 @@
 // builds index lists ("only clustering and bookkeeping stay on the host") and the per-row metric tables
 // (sin/cos evaluated once on the host).
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 #include <algorithm>
 #include <atomic>
@@ -149,6 +150,28 @@ static void build_tiles(gc_level *L, std::vector<SweepTile> &xt, std::vector<Swe
     }
 }
 
+// marching lines (k_march): every row (x) / interior column (y) of every patch, cut into balanced segments of about
+// `seg` cells whose boundaries are multiples of 4 cells, so that an x segment starts on a 32-byte boundary of its row
+static void build_lines(gc_level *L, int seg, std::vector<LineDesc> &xl, std::vector<LineDesc> &yl)
+{
+    for (int p = 0; p < L->np; p++) {
+        const gc_patch &P = L->pat[p];
+        for (int dir = 0; dir < 2; dir++) {
+            int n = dir == 0 ? P.nx : P.ny;                     // cells along the sweep
+            int nlines = dir == 0 ? P.ny + 4 : P.nx;            // x: all rows (S-5); y: interior columns
+            int line0 = dir == 0 ? 0 : 2;
+            int nch = std::max(1, (n + seg - 1) / seg);
+            for (int k = 0; k < nch; k++) {
+                int b0 = k == 0 ? 0 : (int)(((int64_t)n * k / nch + 3) / 4 * 4);
+                int b1 = k == nch - 1 ? n : (int)(((int64_t)n * (k + 1) / nch + 3) / 4 * 4);
+                b0 = std::min(b0, n); b1 = std::min(b1, n);
+                if (b1 <= b0) continue;
+                for (int l = 0; l < nlines; l++) (dir == 0 ? xl : yl).push_back(LineDesc{p, line0 + l, 2 + b0, b1 - b0});
+            }
+        }
+    }
+}
+
 extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, double dx, double dy,
                                int64_t nxl, int64_t nyl, int ratio, int np, const gc_patch *pat, gc_level **out)
 {
@@ -175,9 +198,9 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     for (int p = 0; p < np; p++) {
         const gc_patch &P = L->pat[p];
         PatchDesc &D = L->hpat[p];
-        D.i0 = P.i0; D.j0 = P.j0; D.nx = P.nx; D.ny = P.ny; D.off = off; D.ioff = ioff; D.pitch = P.nx + 4;
+        D.i0 = P.i0; D.j0 = P.j0; D.nx = P.nx; D.ny = P.ny; D.off = off; D.ioff = ioff; D.pitch = ((P.nx + 4 + 3) / 4) * 4;
         D.bcmask = (P.i0 - 2 < 0 ? 1 : 0) | ((int64_t)P.i0 + P.nx + 2 > nxl ? 2 : 0) | (P.j0 - 2 < 0 ? 4 : 0) | ((int64_t)P.j0 + P.ny + 2 > nyl ? 8 : 0);
-        off += (int64_t)(P.nx + 4) * (P.ny + 4);
+        off += (int64_t)D.pitch * (P.ny + 4);   // multiple of 4 elements: every row starts 32-byte aligned
         ioff += (int64_t)P.nx * P.ny;
         for (int64_t by = P.j0 / L->bsize; by <= (P.j0 + P.ny - 1) / L->bsize; by++)
             for (int64_t bx = P.i0 / L->bsize; bx <= (P.i0 + P.nx - 1) / L->bsize; bx++)
@@ -215,6 +238,20 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     build_tiles(L, xt, yt);
     L->nxt = (int)xt.size(); L->nyt = (int)yt.size();
     L->d_xt = upload(L, xt); L->d_yt = upload(L, yt);
+    {   // sweep kernel family: marching lines for large levels, edge-parallel tiles for small ones (GC_SWEEP=edge|march overrides)
+        const char *mode = getenv("GC_SWEEP");
+        L->use_march = L->ncells >= (int64_t)GC_MARCH_MIN_CELLS;
+        if (mode && !strcmp(mode, "edge")) L->use_march = 0;
+        if (mode && !strcmp(mode, "march")) L->use_march = 1;
+        int seg = (int)std::min<int64_t>(128, std::max<int64_t>(16, (L->ncells / 400000 + 3) / 4 * 4));
+        const char *sg = getenv("GC_MARCH_SEG");
+        if (sg && atoi(sg) >= 4) seg = atoi(sg) / 4 * 4;
+        std::vector<LineDesc> xl, yl;
+        if (L->use_march) build_lines(L, seg, xl, yl);
+        L->nxl_lines = (int64_t)xl.size(); L->nyl_lines = (int64_t)yl.size();
+        L->d_xl = upload(L, xl); L->d_yl = upload(L, yl);
+        cudaStreamSynchronize(ctx->stream);
+    }
 
     // same-level copy rectangles: grown box of p  x  interior of q (A2, incl. corners)
     std::vector<CopyRect> rects;
@@ -255,7 +292,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
             }
         }
         if (need_mask) {   // in-domain ghost cells without a same-level source come from the coarser level (A3)
-            for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < D.pitch; i++) {
+            for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < P.nx + 4; i++) {
                 if (i >= 2 && i < P.nx + 2 && j >= 2 && j < P.ny + 2) continue;
                 int64_t gi = (int64_t)P.i0 + i - 2, gj = (int64_t)P.j0 + j - 2;
                 if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
@@ -272,7 +309,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->ncf = 0;
     L->reg_fine = nullptr; L->reg_coarse = nullptr; L->d_reg = nullptr; L->nreg = 0;
     L->d_delta = nullptr; L->d_base = nullptr; L->d_fixcell = nullptr; L->d_fixstart = nullptr; L->d_fixreg = nullptr; L->nfix = 0;
-    if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_copy || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
+    if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_xl || !L->d_yl || !L->d_copy || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
         gc_level_destroy(L);
         return gc_fail(ctx, GC_ERR_NOMEM, "gc_level_create: table allocation failed");
     }
@@ -306,7 +343,7 @@ extern "C" int gc_level_set_field(gc_level *L, int p, int field, const double *s
     if (!L || p < 0 || p >= L->np || field < 0 || field > 3 || !src || ld < L->pat[p].nx + 4) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_set_field: bad argument");
     const PatchDesc &D = L->hpat[p];
     double *dst = plane_of(L, field, GC_NEW) + D.off;
-    cudaMemcpy2DAsync(dst, (size_t)D.pitch * 8, src, (size_t)ld * 8, (size_t)D.pitch * 8, D.ny + 4,
+    cudaMemcpy2DAsync(dst, (size_t)D.pitch * 8, src, (size_t)ld * 8, (size_t)(D.nx + 4) * 8, D.ny + 4,
                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, L->ctx->stream);
     if (!is_device) cudaStreamSynchronize(L->ctx->stream);
     return gc_cuda_check(L->ctx, "gc_level_set_field");
@@ -317,7 +354,7 @@ extern "C" int gc_level_get_field(const gc_level *L, int p, int field, int which
     if (!L || p < 0 || p >= L->np || field < 0 || field > 3 || !dst || ld < L->pat[p].nx + 4) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_get_field: bad argument");
     const PatchDesc &D = L->hpat[p];
     const double *src = plane_of(L, field, which) + D.off;
-    cudaMemcpy2DAsync(dst, (size_t)ld * 8, src, (size_t)D.pitch * 8, (size_t)D.pitch * 8, D.ny + 4,
+    cudaMemcpy2DAsync(dst, (size_t)ld * 8, src, (size_t)D.pitch * 8, (size_t)(D.nx + 4) * 8, D.ny + 4,
                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, L->ctx->stream);
     if (!is_device) cudaStreamSynchronize(L->ctx->stream);
     return gc_cuda_check(L->ctx, "gc_level_get_field");

@@ -58,8 +58,9 @@ __global__ void k_bc(const PatchDesc *pat, const int32_t *list, double *f0, doub
             }
         }
     } else {
-        for (int t = threadIdx.x; t < pd.pitch * 4; t += blockDim.x) {
-            int c = t / pd.pitch, i = t - c * pd.pitch;
+        const int W = pd.nx + 4;
+        for (int t = threadIdx.x; t < W * 4; t += blockDim.x) {
+            int c = t / W, i = t - c * W;
             int j = (c < 2) ? c : pd.ny + c;
             int64_t gj = (int64_t)pd.j0 + j - 2;
             int wall; int64_t gs;
@@ -93,12 +94,13 @@ __global__ void k_set_global(const PatchDesc *pat, double *plane, const double *
                              int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
     PatchDesc pd = pat[blockIdx.x];
-    int n = pd.pitch * (pd.ny + 4);
+    const int W = pd.nx + 4;
+    int n = W * (pd.ny + 4);
     for (int t = threadIdx.x; t < n; t += blockDim.x) {
-        int j = t / pd.pitch, i = t - j * pd.pitch;
+        int j = t / W, i = t - j * W;
         int64_t gi = (int64_t)pd.i0 + i - 2 - gi0, gj = (int64_t)pd.j0 + j - 2 - gj0;
         if (gi < 0 || gi >= gnx || gj < 0 || gj >= gny) continue;
-        plane[pd.off + t] = src[gj * ld + gi];
+        plane[pd.off + (int64_t)j * pd.pitch + i] = src[gj * ld + gi];
     }
 }
 

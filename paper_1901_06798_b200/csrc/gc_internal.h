@@ -8,13 +8,14 @@
 #include "../../include/gc.h"
 
 #define GC_G 2  // ghost width
+#define GC_MARCH_MIN_CELLS 2000000   // levels at least this large use the line-marching sweep kernels
 
 // patch descriptor as the kernels see it (A1): interior box, element offset of the patch in a field plane, row pitch
 struct PatchDesc {
     int32_t i0, j0, nx, ny;
     int64_t off;     // element offset in every field plane of the pool
     int64_t ioff;    // offset in interior-packed arrays (masks, flags)
-    int32_t pitch;   // nx + 4
+    int32_t pitch;   // row pitch in elements: nx + 4 rounded up to a multiple of 4 (32-byte aligned rows)
     int32_t bcmask;  // bit0 touches xlo, bit1 xhi, bit2 ylo, bit3 yhi
 };
 
@@ -23,6 +24,12 @@ struct SweepTile {
     int32_t patch;
     int32_t line0, nlines;  // rows [line0, line0+nlines) (x-sweep) or columns (y-sweep), storage indices
     int32_t c0, nc;         // cells [c0, c0+nc) along the sweep direction, storage indices (edges c0-1 .. c0+nc+1 are solved)
+};
+
+// work item of a marching sweep kernel: ONE thread walks cells [c0-2, c0+nc+2) of a line (row for x, column for y),
+// solving edges c0-1 .. c0+nc+1 and updating cells c0 .. c0+nc-1 (storage indices along the sweep)
+struct LineDesc {
+    int32_t patch, line, c0, nc;
 };
 
 // same-level ghost copy: rectangle of w x h cells
@@ -105,7 +112,9 @@ struct gc_level {
     double *qs[3];
     PatchDesc *d_pat;
     double *d_kappa, *d_rdx, *d_rdy, *d_ey;
-    SweepTile *d_xt, *d_yt; int nxt, nyt;
+    SweepTile *d_xt, *d_yt; int nxt, nyt;            // edge-parallel tiles (small levels)
+    LineDesc *d_xl, *d_yl; int64_t nxl_lines, nyl_lines;   // marching lines (large levels)
+    int use_march;
     CopyRect *d_copy; int ncopy;
     int32_t *d_bcp; int nbcp;                       // patches touching the physical boundary
     std::vector<int64_t> coarse_ghost;              // plane offsets + global indices of ghosts to be filled from the coarser level

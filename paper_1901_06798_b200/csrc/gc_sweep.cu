@@ -4,15 +4,26 @@
 // filled) and writes Q* for columns 2..nx+1 on ALL rows; the y-sweep reads Q*, writes Q^{n+1} on the interior
 // and applies the dry clean-up.  Thread <-> edge for the Riemann solve and the limiter, then thread <-> cell
 // for the update (the paper's re-assignment), neighbour waves through shared memory.
+//
+// Two kernel families compute the same bits:
+//  * k_sweep  (edge-parallel): thread <-> edge, neighbour waves through shared memory.  Much parallelism per
+//    cell, used for small levels where the GPU would otherwise be empty.
+//  * k_march  (line-marching): thread <-> line segment, walking along the sweep with the waves of the previous
+//    edge, the primitive variables of the previous cell and the pending fluxes in registers.  No shared
+//    memory, no barriers, each cell's primitive variables computed once, 3 redundant edges per segment only.
+//    The x-sweep reads 4 cells of its row per 256-bit load (rows are 32-byte aligned); the y-sweep reads
+//    one row of 32 adjacent columns per warp (coalesced).  Used for large levels (fp64-pipe bound).
 #include "gc_internal.h"
-#include "gc_riemann.cuh"
+#include "gc_scheme.cuh"
 
 #define SW_BLOCK 256
+#define MARCH_BLOCK 128
 #define SW_YW 8       // columns per y-sweep block (8 doubles = 2 full 32-byte sectors per row access)
 
 struct SweepArgs {
     const PatchDesc *pat;
     const SweepTile *tiles;
+    const LineDesc *lines; int64_t nlines;
     const double *h, *hu, *hv, *b;   // input planes
     double *oh, *ohu, *ohv;          // output planes
     const double *rd;                // rdx (x-sweep) or rdy (y-sweep), per global row (+2)
@@ -179,6 +190,136 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
     }
 }
 
+// ---- line-marching sweep ------------------------------------------------------------------------------------
+__device__ __forceinline__ void ld4(const double *p, double &x, double &y, double &z, double &w)
+{
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
+}
+
+template <int DIR>
+__global__ void __launch_bounds__(MARCH_BLOCK) k_march(SweepArgs a)
+{
+    __shared__ double sred[MARCH_BLOCK / 32];
+    __shared__ unsigned long long sclip[MARCH_BLOCK / 32];
+    __shared__ double sclipm[MARCH_BLOCK / 32];
+
+    const int64_t lid = (int64_t)blockIdx.x * MARCH_BLOCK + threadIdx.x;
+    const bool active = lid < a.nlines;
+    LineDesc ln; ln.patch = 0; ln.line = 0; ln.c0 = 2; ln.nc = -4;
+    if (active) { int4 v = *reinterpret_cast<const int4 *>(a.lines + lid); ln.patch = v.x; ln.line = v.y; ln.c0 = v.z; ln.nc = v.w; }
+    const PatchDesc pd = a.pat[ln.patch];
+    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
+    const int nst = ln.nc + 4;                                   // cells read by this line
+    const int nst_warp = __reduce_max_sync(0xffffffffu, nst);
+    const int cfirst = ln.c0 - 2;                                // storage index (along the sweep) of the first cell read
+    int64_t base; int64_t str;
+    if (DIR == 0) { base = pd.off + (int64_t)ln.line * pd.pitch + cfirst; str = 1; }
+    else          { base = pd.off + (int64_t)cfirst * pd.pitch + ln.line; str = pd.pitch; }
+    const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
+    const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
+
+    Waves Wc; gc_waves_zero(Wc);                                 // waves of the previous edge (r-1)
+    double dlo[3] = {0.0, 0.0, 0.0};                             // Z_{r-2} . Z_{r-1}
+    double fpp[3] = {0.0, 0.0, 0.0};                             // fp of edge r-2
+    RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
+    double q1h = 0.0, q1p = 0.0, q1t = 0.0, q2h = 0.0, q2p = 0.0, q2t = 0.0;   // raw state of cells r-1, r-2
+    double rd1 = 0.0, rd2 = 0.0;                                 // 1/(kappa dx) of cells r-1, r-2
+    double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
+
+    double vh[4], vp[4], vt[4], vb[4];                           // x-sweep: the 4 cells of the current 256-bit group
+    double nh_ = 0.0, np_ = 0.0, nt_ = 0.0, nb_ = 0.0;           // y-sweep: next row, loaded one step ahead
+    if (DIR == 1 && nst > 0) {
+        nh_ = a.h[base]; nb_ = a.b[base]; np_ = a.hv[base]; nt_ = a.hu[base];
+    }
+
+#pragma unroll 1
+    for (int r = 0; r < nst_warp; r++) {
+        const bool live = r < nst;
+        double qh, qp, qt, qb;
+        if (DIR == 0) {
+            if ((r & 3) == 0) {
+                if (live) {
+                    const int64_t o = base + r;
+                    ld4(a.h + o, vh[0], vh[1], vh[2], vh[3]); ld4(a.hu + o, vp[0], vp[1], vp[2], vp[3]);
+                    ld4(a.hv + o, vt[0], vt[1], vt[2], vt[3]); ld4(a.b + o, vb[0], vb[1], vb[2], vb[3]);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; k++) { vh[k] = 0.0; vp[k] = 0.0; vt[k] = 0.0; vb[k] = 0.0; }
+                }
+            }
+            qh = vh[0]; qp = vp[0]; qt = vt[0]; qb = vb[0];
+#pragma unroll
+            for (int k = 0; k < 3; k++) { vh[k] = vh[k + 1]; vp[k] = vp[k + 1]; vt[k] = vt[k + 1]; vb[k] = vb[k + 1]; }
+        } else {
+            qh = nh_; qp = np_; qt = nt_; qb = nb_;
+            if (r + 1 < nst) {
+                const int64_t o = base + (int64_t)(r + 1) * str;
+                nh_ = a.h[o]; nb_ = a.b[o]; np_ = a.hv[o]; nt_ = a.hu[o];
+            }
+        }
+        const int c = cfirst + r;                                // storage index of this cell = index of the edge on its low side
+        double rd0, ef;
+        if (DIR == 0) { rd0 = rdrow; ef = a.ex; }
+        else          { rd0 = live ? a.rd[pd.j0 + c] : 0.0; ef = live ? a.ey[pd.j0 + c] : 1.0; }
+
+        RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
+        gc_prim(R, a.g, a.eps);
+        Waves Wn;
+        if (r >= 1 && live) gc_solve_edge_prim(a.g, a.eps, Lst, R, a.coord, ef, Wn);    // edge r (between cells r-1, r)
+        else gc_waves_zero(Wn);
+        double dhi[3];
+        gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
+        double fm[3], fp[3];
+        gc_edge_flux(Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);                    // edge r-1
+        if (live && r >= 3 && count) cflm = dmax(cflm, gc_edge_cfl(Wc, rd2, rd1));
+        if (live && r >= 4) {                                                           // cell r-2
+            const double dtdx = dt * rd2;
+            double uh = q2h - dtdx * (fm[0] - fpp[0]);
+            double up = q2p - dtdx * (fm[1] - fpp[1]);
+            double ut = q2t - dtdx * (fm[2] - fpp[2]);
+            const int64_t o = base + (int64_t)(r - 2) * str;
+            if (DIR == 0) {
+                a.oh[o] = uh; a.ohu[o] = up; a.ohv[o] = ut;
+            } else {
+                if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
+                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[pd.j0 + c - 2] * a.dxdy); }
+                    uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
+                }
+                if (uh != uh || up != up || ut != ut) nanf = 1;
+                if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; k++) { fpp[k] = fp[k]; dlo[k] = dhi[k]; }
+        Wc = Wn; Lst = R;
+        q2h = q1h; q2p = q1p; q2t = q1t; q1h = qh; q1p = qp; q1t = qt;
+        rd2 = rd1; rd1 = rd0;
+    }
+
+    cflm = warp_max(cflm);
+    if (DIR == 1) {
+        nclip = __reduce_add_sync(0xffffffffu, nclip);
+        nanf = __any_sync(0xffffffffu, nanf);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) clipm += __shfl_xor_sync(0xffffffffu, clipm, o);
+    }
+    const int k = threadIdx.x;
+    if ((k & 31) == 0) { sred[k >> 5] = cflm; if (DIR == 1) { sclip[k >> 5] = nclip; sclipm[k >> 5] = clipm; if (nanf) a.stats->nan_seen = 1; } }
+    __syncthreads();
+    if (k == 0) {
+        double m = sred[0];
+#pragma unroll
+        for (int w = 1; w < MARCH_BLOCK / 32; w++) m = dmax(m, sred[w]);
+        if (m > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(m));
+        if (DIR == 1) {
+            unsigned long long n = 0; double cm = 0.0;
+#pragma unroll
+            for (int w = 0; w < MARCH_BLOCK / 32; w++) { n += sclip[w]; cm += sclipm[w]; }
+            if (n) { atomicAdd(&a.stats->nclip, n); atomicAdd(&a.stats->clipped, cm); }
+        }
+    }
+}
+
 __global__ void k_stats_reset(DevStats *s) { s->sdx_bits = 0ull; s->nclip = 0ull; s->clipped = 0.0; s->nan_seen = 0; }
 
 __global__ void k_next_dt(const DevStats *s, double *dt_dev, double cfl)
@@ -198,15 +339,22 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     SweepArgs a;
     a.pat = L->d_pat; a.g = P.g; a.eps = P.dry_tol; a.dt = dt; a.dt_dev = dt_dev;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out; a.stats = L->d_stats;
+    a.lines = nullptr; a.nlines = 0;
     a.ex = L->ex; a.ey = L->d_ey; a.dxdy = L->dx * L->dy; a.kappa = L->d_kappa; a.b = L->b;
     // x-sweep: Q^n -> Q*
     a.tiles = L->d_xt; a.h = L->q[cur][0]; a.hu = L->q[cur][1]; a.hv = L->q[cur][2];
     a.oh = L->qs[0]; a.ohu = L->qs[1]; a.ohv = L->qs[2]; a.rd = L->d_rdx;
-    if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
+    if (L->use_march) {
+        a.lines = L->d_xl; a.nlines = L->nxl_lines;
+        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_march<0><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, 0, L->ctx->stream>>>(a); }
+    } else if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
     // y-sweep: Q* -> Q^{n+1}
     a.tiles = L->d_yt; a.h = L->qs[0]; a.hu = L->qs[1]; a.hv = L->qs[2];
     a.oh = L->q[nxt][0]; a.ohu = L->q[nxt][1]; a.ohv = L->q[nxt][2]; a.rd = L->d_rdy;
-    if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
+    if (L->use_march) {
+        a.lines = L->d_yl; a.nlines = L->nyl_lines;
+        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_march<1><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, 0, L->ctx->stream>>>(a); }
+    } else if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
 }
 
 // ---- fp64 ALU peak probe: dependent DFMA chains, 8 independent accumulators per thread

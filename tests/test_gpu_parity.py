@@ -13,6 +13,14 @@ pytestmark = pytest.mark.gpu
 G = 9.81
 
 
+@pytest.fixture(autouse=True, params=["edge", "march"])
+def sweep_mode(request, monkeypatch):
+    """Both sweep kernel families (edge-parallel tiles / line-marching, DESIGN.md 5) must give the oracle's bits;
+    the library picks one by level size unless GC_SWEEP says otherwise."""
+    monkeypatch.setenv("GC_SWEEP", request.param)
+    return request.param
+
+
 def unpack(L, packed):
     """interior-packed per-patch array -> level-global 2-D array"""
     out = np.full((L.nyl, L.nxl), 255, dtype=packed.dtype)
