@@ -150,6 +150,12 @@ int64_t gc_launch_count(const gc_ctx *);
 int gc_profile_enable(gc_ctx *, int on);
 int gc_profile_read(gc_ctx *, double *ms /*HOST*/, int64_t *count /*HOST*/);
 
+/* Self-test of the branch-free correctly rounded divide / reciprocal / square root the marching kernels use
+ * (csrc/gc_math.cuh) against the IEEE operators: for each i, a[i]/b[i], 1/b[i], sqrt(a[i]) (a, b: HOST arrays of n).
+ * nmismatch = results that differ in any bit although the fast path accepted the operands (must be 0);
+ * nfallback = operations whose operands were outside the fast window (they are redone with the operators). */
+int gc_selftest_math(gc_ctx *, const double *a, const double *b, int64_t n, int64_t *nmismatch, int64_t *nfallback);
+
 /* Measured fp64 ALU throughput of this device (DFMA micro-benchmark, flop/s); for the "alu" roofline. */
 int gc_probe_fp64_peak(gc_ctx *, double *flops_out /*HOST*/);
 

@@ -10,14 +10,14 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgeoclaw_b200.so")
+LIB_PATH = os.environ.get("GC_LIB", os.path.join(_HERE, "libgeoclaw_b200.so"))   # GC_LIB: an alternative build of the same library
 
 SYMBOLS = [
     "gc_ctx_create", "gc_ctx_destroy", "gc_last_error", "gc_level_create", "gc_level_destroy", "gc_level_ncells",
     "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
-    "gc_launch_count", "gc_profile_enable", "gc_profile_read",
+    "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math",
 ]
 
 
@@ -78,6 +78,7 @@ def lib():
     L.gc_launch_count.argtypes = [vp]; L.gc_launch_count.restype = i64
     L.gc_profile_enable.argtypes = [vp, i]
     L.gc_profile_read.argtypes = [vp, vp, vp]
+    L.gc_selftest_math.argtypes = [vp, vp, vp, i64, vp, vp]
     _lib = L
     return L
 
@@ -247,6 +248,13 @@ class Context:
         v = C.c_double(0.0)
         self._chk(lib().gc_probe_fp64_peak(self.h, C.byref(v)), "gc_probe_fp64_peak")
         return v.value
+
+    def selftest_math(self, a, b):
+        """-> (mismatches, fallbacks) of the fast divide / reciprocal / sqrt against the IEEE operators"""
+        a = np.ascontiguousarray(a, dtype=np.float64); b = np.ascontiguousarray(b, dtype=np.float64)
+        nm, nf = C.c_int64(0), C.c_int64(0)
+        self._chk(lib().gc_selftest_math(self.h, a.ctypes.data, b.ctypes.data, a.size, C.byref(nm), C.byref(nf)), "gc_selftest_math")
+        return nm.value, nf.value
 
     def launch_count(self):
         return int(lib().gc_launch_count(self.h))

@@ -499,6 +499,23 @@ extern "C" double gc_level_mass(const gc_level *L)
     return m;
 }
 
+extern "C" int gc_selftest_math(gc_ctx *c, const double *a, const double *b, int64_t n, int64_t *nmismatch, int64_t *nfallback)
+{
+    if (!c || !a || !b || n < 0 || !nmismatch || !nfallback) return GC_ERR_BADARG;
+    double *d = (double *)gc_dev_alloc(c, (size_t)(2 * n + 2) * 8);
+    if (!d) return gc_fail(c, GC_ERR_NOMEM, "gc_selftest_math: allocation failed");
+    unsigned long long *cnt = (unsigned long long *)(d + 2 * n), h[2] = {0, 0};
+    cudaMemcpyAsync(d, a, (size_t)n * 8, cudaMemcpyHostToDevice, c->stream);
+    cudaMemcpyAsync(d + n, b, (size_t)n * 8, cudaMemcpyHostToDevice, c->stream);
+    cudaMemsetAsync(cnt, 0, 16, c->stream);
+    gc_launch_math_selftest(c->stream, d, d + n, n, cnt);
+    cudaMemcpyAsync(h, cnt, 16, cudaMemcpyDeviceToHost, c->stream);
+    cudaStreamSynchronize(c->stream);
+    gc_dev_free(c, d);
+    *nmismatch = (int64_t)h[0]; *nfallback = (int64_t)h[1];
+    return gc_cuda_check(c, "gc_selftest_math");
+}
+
 extern "C" int gc_probe_fp64_peak(gc_ctx *c, double *flops_out)
 {
     if (!c || !flops_out) return GC_ERR_BADARG;

@@ -145,6 +145,7 @@ int gc_find_patch_host(const gc_level *L, int64_t gi, int64_t gj);
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out);
 void gc_launch_stats_reset(gc_level *L);
 void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl_target);
+void gc_launch_math_selftest(cudaStream_t s, const double *a, const double *b, int64_t n, unsigned long long *out);
 void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, int threads);
 // gc_ghost.cu
 void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);

@@ -3,9 +3,12 @@
 // P:122 names the solver (George 2008, augmented system with topography and momentum flux) and its
 // properties; the steps R0-R8 implemented here are DESIGN.md section 3.3.  Every expression is
 // evaluated in the order DESIGN.md states (no FMA contraction: the library is built with -fmad=false;
-// '/' and sqrt are IEEE), so the result is bit-identical to a plain C evaluation.
+// '/' and sqrt are IEEE), so the result is bit-identical to a plain C evaluation.  Divides, reciprocals and
+// square roots go through a math policy M (gc_math.cuh): MathIeee = the operators, MathFast = the same
+// correctly rounded results without a branch per operation (valid inside an exponent window, else M.failed()).
 #pragma once
 #include <cuda_runtime.h>
+#include "gc_math.cuh"
 
 #define GC_TAU 1.0e-6
 #define GC_SQRT_TAU 1.0e-3
@@ -16,21 +19,23 @@ __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : 
 struct RState { double h, p, t, b, u, v, phi, c; };   // depth, normal/transverse momentum, bathymetry, velocities, momentum flux, celerity
 
 // R2: primitive variables of one side (h <= eps: dry, everything zero)
-__device__ __forceinline__ void gc_prim(RState &S, double g, double eps)
+template <class M>
+__device__ __forceinline__ void gc_prim(M &m, RState &S, double g, double eps)
 {
     if (S.h < 0.0) { S.h = 0.0; S.p = 0.0; S.t = 0.0; }      // R0
     if (S.h <= eps) {
         S.h = 0.0; S.p = 0.0; S.t = 0.0; S.u = 0.0; S.v = 0.0; S.phi = 0.0;
     } else {
-        double rh = 1.0 / S.h;
+        double rh = m.rcp(S.h);
         S.u = S.p * rh; S.v = S.t * rh;
         S.phi = S.p * S.u + 0.5 * g * (S.h * S.h);
     }
-    S.c = sqrt(g * S.h);
+    S.c = m.sqrt_(g * S.h);
 }
 
 // R5: flat-bottom two-wave middle state M(hL, hR, uL, uR) -> (hm, sigma1, sigma2)
-__device__ __forceinline__ void gc_middle(double g, double eps, double hL, double hR, double uL, double uR,
+template <class M>
+__device__ __forceinline__ void gc_middle(M &m, double g, double eps, double hL, double hR, double uL, double uR,
                                           double cL, double cR, double &hm, double &s1m, double &s2m)
 {
     double hmin = dmin(hL, hR), hmax = dmax(hL, hR);
@@ -43,30 +48,30 @@ __device__ __forceinline__ void gc_middle(double g, double eps, double hL, doubl
     double cmin = (hL < hR) ? cL : cR;
     double cmax = (hL < hR) ? cR : cL;
     double Fmin = du + 2.0 * (cmin - cmax);
-    double Fmax = du + (hmax - hmin) * sqrt(0.5 * g * (hmax + hmin) / (hmax * hmin));
+    double Fmax = du + (hmax - hmin) * m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin));
     if (Fmin > 0.0) {                       // two rarefactions
         double cm = 0.25 * dmax(0.0, 2.0 * (cL + cR) - du);
-        hm = cm * cm / g;
+        hm = m.div(cm * cm, g);
         s1m = (uL + 2.0 * cL) - 3.0 * cm;
         s2m = (uR - 2.0 * cR) + 3.0 * cm;
     } else if (Fmax <= 0.0) {               // two shocks: one Newton step in sqrt(h) from hmax
         double h0 = hmax;
-        double gL = sqrt(0.5 * g * (1.0 / h0 + 1.0 / hL));
-        double gR = sqrt(0.5 * g * (1.0 / h0 + 1.0 / hR));
+        double gL = m.sqrt_(0.5 * g * (m.rcp(h0) + m.rcp(hL)));
+        double gR = m.sqrt_(0.5 * g * (m.rcp(h0) + m.rcp(hR)));
         double F0 = du + (h0 - hL) * gL + (h0 - hR) * gR;
-        double dfdh = (gL - g * (h0 - hL) / (4.0 * (h0 * h0) * gL))
-                    + (gR - g * (h0 - hR) / (4.0 * (h0 * h0) * gR));
-        double sq0 = sqrt(h0);
+        double dfdh = (gL - m.div(g * (h0 - hL), 4.0 * (h0 * h0) * gL))
+                    + (gR - m.div(g * (h0 - hR), 4.0 * (h0 * h0) * gR));
+        double sq0 = m.sqrt_(h0);
         double slope = 2.0 * sq0 * dfdh;
-        double sq = sq0 - F0 / slope;
+        double sq = sq0 - m.div(F0, slope);
         double h1 = sq * sq;
-        double u1m = uL - (h1 - hL) * sqrt(0.5 * g * (1.0 / h1 + 1.0 / hL));
-        double u2m = uR + (h1 - hR) * sqrt(0.5 * g * (1.0 / h1 + 1.0 / hR));
-        double cm = sqrt(g * h1);
+        double u1m = uL - (h1 - hL) * m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hL)));
+        double u2m = uR + (h1 - hR) * m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hR)));
+        double cm = m.sqrt_(g * h1);
         hm = h1; s1m = u1m - cm; s2m = u2m + cm;
     } else {                                // shock + rarefaction: one secant step from hmin
-        double h1 = hmin - Fmin * (hmax - hmin) / (Fmax - Fmin);
-        double cm = sqrt(g * h1);
+        double h1 = hmin - m.div(Fmin * (hmax - hmin), Fmax - Fmin);
+        double cm = m.sqrt_(g * h1);
         hm = h1;
         if (hL > hR) { s1m = (uL + 2.0 * cL) - 3.0 * cm; s2m = (uL + 2.0 * cL) - cm; }
         else         { s2m = (uR - 2.0 * cR) + 3.0 * cm; s1m = (uR - 2.0 * cR) + cm; }
@@ -75,7 +80,8 @@ __device__ __forceinline__ void gc_middle(double g, double eps, double hL, doubl
 
 // Full solve.  L and R must have gone through gc_prim.  Z[p][k]: f-wave of family p, component k
 // (0: h, 1: normal momentum, 2: transverse momentum); s[p]: speeds.
-__device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RState R, double (&Z)[3][3], double (&s)[3])
+template <class M>
+__device__ __forceinline__ void gc_riemann(M &m, double g, double eps, RState L, RState R, double (&Z)[3][3], double (&s)[3])
 {
 #pragma unroll
     for (int p = 0; p < 3; p++) { s[p] = 0.0; Z[p][0] = 0.0; Z[p][1] = 0.0; Z[p][2] = 0.0; }
@@ -84,7 +90,7 @@ __device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RStat
     bool m0 = true, m1 = true, m2 = true;                      // R3 wall mask
     if (R.h <= eps) {
         double hw, a1, a2;
-        gc_middle(g, eps, L.h, L.h, L.u, -L.u, L.c, L.c, hw, a1, a2);
+        gc_middle(m, g, eps, L.h, L.h, L.u, -L.u, L.c, L.c, hw, a1, a2);
         double htest = dmax(L.h, hw);
         if (htest + L.b < R.b) {
             m1 = false; m2 = false;
@@ -94,7 +100,7 @@ __device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RStat
         }
     } else if (L.h <= eps) {
         double hw, a1, a2;
-        gc_middle(g, eps, R.h, R.h, -R.u, R.u, R.c, R.c, hw, a1, a2);
+        gc_middle(m, g, eps, R.h, R.h, -R.u, R.u, R.c, R.c, hw, a1, a2);
         double htest = dmax(R.h, hw);
         if (htest + R.b < L.b) {
             m0 = false; m1 = false;
@@ -106,14 +112,14 @@ __device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RStat
 
     // R4 Einfeldt speeds
     double sL = L.u - L.c, sR = R.u + R.c;
-    double uhat = (L.c * L.u + R.c * R.u) / (L.c + R.c);
-    double chat = sqrt(g * (0.5 * (L.h + R.h)));
+    double uhat = m.div(L.c * L.u + R.c * R.u, L.c + R.c);
+    double chat = m.sqrt_(g * (0.5 * (L.h + R.h)));
     double sE1 = dmin(sL, uhat - chat);
     double sE2 = dmax(sR, uhat + chat);
 
     // R5, R6
     double hm, s1m, s2m;
-    gc_middle(g, eps, L.h, R.h, L.u, R.u, L.c, R.c, hm, s1m, s2m);
+    gc_middle(m, g, eps, L.h, R.h, L.u, R.u, L.c, R.c, hm, s1m, s2m);
     double l1 = dmin(sE1, s2m);
     double l3 = dmax(sE2, s1m);
     double l2 = 0.5 * (l1 + l3);
@@ -141,19 +147,19 @@ __device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RStat
         dh = -delb;
         dphi = -ghbar * delb;
     } else {
-        double q = ghbar / pbar;
+        double q = m.div(ghbar, pbar);
         dh = delb * q;
         dphi = -delb * (q * ptil);
     }
     if (l1 < -GC_TAU && l3 > GC_TAU) {
-        dh = dmin(dh, hsd / l3);
-        dh = dmax(dh, hsd / l1);
+        dh = dmin(dh, m.div(hsd, l3));
+        dh = dmax(dh, m.div(hsd, l1));
     } else if (l1 >= GC_TAU) {
-        dh = dmin(dh, hsd / l1);
+        dh = dmin(dh, m.div(hsd, l1));
         dh = dmax(dh, -L.h);
     } else if (l3 <= -GC_TAU) {
         dh = dmin(dh, R.h);
-        dh = dmax(dh, hsd / l3);
+        dh = dmax(dh, m.div(hsd, l3));
     }
     {
         double a = -L.h * delb, c = -R.h * delb;
@@ -165,7 +171,7 @@ __device__ __forceinline__ void gc_riemann(double g, double eps, RState L, RStat
     double d1 = (R.h - L.h) - dh;
     double d2 = R.p - L.p;
     double d3 = (R.phi - L.phi) - dphi;
-    double rdl = 1.0 / (l3 - l1);
+    double rdl = m.rcp(l3 - l1);
     double l1sq = l1 * l1, l3sq = l3 * l3;
     double b1 = (l3 * d1 - d2) * rdl;
     double b3 = (d2 - l1 * d1) * rdl;

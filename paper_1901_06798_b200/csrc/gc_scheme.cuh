@@ -17,9 +17,10 @@ __device__ __forceinline__ void gc_waves_zero(Waves &W)
 }
 
 // (1)+(2) with the primitive variables of both sides already computed (gc_prim applied by the caller)
-__device__ __forceinline__ void gc_solve_edge_prim(double g, double eps, const RState &L, const RState &R, int coord, double ef, Waves &W)
+template <class M>
+__device__ __forceinline__ void gc_solve_edge_prim(M &m, double g, double eps, const RState &L, const RState &R, int coord, double ef, Waves &W)
 {
-    gc_riemann(g, eps, L, R, W.Z, W.s);
+    gc_riemann(m, g, eps, L, R, W.Z, W.s);
     if (coord == 1) {
 #pragma unroll
         for (int w = 0; w < 3; w++) { W.s[w] = W.s[w] * ef; W.Z[w][0] = W.Z[w][0] * ef; W.Z[w][1] = W.Z[w][1] * ef; W.Z[w][2] = W.Z[w][2] * ef; }
@@ -27,11 +28,12 @@ __device__ __forceinline__ void gc_solve_edge_prim(double g, double eps, const R
 }
 
 // (1)+(2): solve the edge between two cells given as raw (h, p, t, b) and scale by the edge factor ef
-__device__ __forceinline__ void gc_solve_edge(double g, double eps, RState L, RState R, int coord, double ef, Waves &W)
+template <class M>
+__device__ __forceinline__ void gc_solve_edge(M &m, double g, double eps, RState L, RState R, int coord, double ef, Waves &W)
 {
-    gc_prim(L, g, eps);
-    gc_prim(R, g, eps);
-    gc_solve_edge_prim(g, eps, L, R, coord, ef, W);
+    gc_prim(m, L, g, eps);
+    gc_prim(m, R, g, eps);
+    gc_solve_edge_prim(m, g, eps, L, R, coord, ef, W);
 }
 
 // Z_a^w . Z_b^w per family.  The product is commutative term by term, so the same three numbers serve the
@@ -43,15 +45,17 @@ __device__ __forceinline__ void gc_wave_dots(const Waves &A, const Waves &B, dou
 }
 
 // MC limiter value for one family: zi = Z_I . Z_e, zz = Z_e . Z_e (zz != 0)
-__device__ __forceinline__ double gc_mc(double zi, double zz)
+template <class M>
+__device__ __forceinline__ double gc_mc(M &m, double zi, double zz)
 {
-    double theta = zi / zz;                                                     // eq. 10 (S-1)
+    double theta = m.div(zi, zz);                                                    // eq. 10 (S-1)
     return dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));        // MC
 }
 
 // (3)-(6) for edge e.  dlo[w] = Z_{e-1}^w . Z_e^w, dhi[w] = Z_{e+1}^w . Z_e^w (eq. 11: I = e-1 if s > 0, e+1 if s < 0).
 // rdL, rdR = 1/(kappa dx) of the left / right cell.
-__device__ __forceinline__ void gc_edge_flux(const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
+template <class M>
+__device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
                                              double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
 {
     double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
@@ -72,7 +76,7 @@ __device__ __forceinline__ void gc_edge_flux(const Waves &W, const double (&dlo)
             if (sw != 0.0) {
                 double zz = (W.Z[w][0] * W.Z[w][0] + W.Z[w][1] * W.Z[w][1]) + W.Z[w][2] * W.Z[w][2];
                 double phi = 1.0;
-                if (zz != 0.0) phi = gc_mc((sw > 0.0) ? dlo[w] : dhi[w], zz);
+                if (zz != 0.0) phi = gc_mc(m, (sw > 0.0) ? dlo[w] : dhi[w], zz);
                 double coef = ((sw > 0.0) ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
 #pragma unroll
                 for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[w][c]);   // eq. 9

@@ -18,6 +18,9 @@
 
 #define SW_BLOCK 256
 #define MARCH_BLOCK 128
+#ifndef MARCH_MINB
+#define MARCH_MINB 3     // resident blocks per SM the register allocation is bounded for
+#endif
 #define SW_YW 8       // columns per y-sweep block (8 doubles = 2 full 32-byte sectors per row access)
 
 struct SweepArgs {
@@ -80,9 +83,10 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
         if (DIR == 0) { L.p = a.hu[idx - str]; L.t = a.hv[idx - str]; R.p = a.hu[idx]; R.t = a.hv[idx]; }
         else          { L.p = a.hv[idx - str]; L.t = a.hu[idx - str]; R.p = a.hv[idx]; R.t = a.hu[idx]; }
         qh = R.h; qp = R.p; qt = R.t;
-        gc_prim(L, a.g, a.eps);
-        gc_prim(R, a.g, a.eps);
-        gc_riemann(a.g, a.eps, L, R, Z, s);
+        MathIeee mi;
+        gc_prim(mi, L, a.g, a.eps);
+        gc_prim(mi, R, a.g, a.eps);
+        gc_riemann(mi, a.g, a.eps, L, R, Z, s);
         if (DIR == 0) { rdR = a.rd[pd.j0 + line]; rdL = rdR; }
         else          { rdR = a.rd[pd.j0 + ce]; rdL = a.rd[pd.j0 + ce - 1]; }
         if (a.coord == 1) {                   // scale by the edge factor
@@ -197,7 +201,7 @@ __device__ __forceinline__ void ld4(const double *p, double &x, double &y, doubl
 }
 
 template <int DIR>
-__global__ void __launch_bounds__(MARCH_BLOCK) k_march(SweepArgs a)
+__global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
 {
     __shared__ double sred[MARCH_BLOCK / 32];
     __shared__ unsigned long long sclip[MARCH_BLOCK / 32];
@@ -263,14 +267,28 @@ __global__ void __launch_bounds__(MARCH_BLOCK) k_march(SweepArgs a)
         else          { rd0 = live ? a.rd[pd.j0 + c] : 0.0; ef = live ? a.ey[pd.j0 + c] : 1.0; }
 
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
-        gc_prim(R, a.g, a.eps);
         Waves Wn;
-        if (r >= 1 && live) gc_solve_edge_prim(a.g, a.eps, Lst, R, a.coord, ef, Wn);    // edge r (between cells r-1, r)
-        else gc_waves_zero(Wn);
+        {   // fast math first; an operand outside its window (gc_math.cuh) redoes this cell + edge with the IEEE operators
+            MathFast mf;
+            RState R0 = R;
+            gc_prim(mf, R, a.g, a.eps);
+            if (r >= 1 && live) gc_solve_edge_prim(mf, a.g, a.eps, Lst, R, a.coord, ef, Wn);    // edge r (between cells r-1, r)
+            else gc_waves_zero(Wn);
+            if (mf.failed()) {
+                MathIeee mi;
+                R = R0;
+                gc_prim(mi, R, a.g, a.eps);
+                if (r >= 1 && live) gc_solve_edge_prim(mi, a.g, a.eps, Lst, R, a.coord, ef, Wn);
+            }
+        }
         double dhi[3];
         gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
         double fm[3], fp[3];
-        gc_edge_flux(Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);                    // edge r-1
+        {
+            MathFast mf;
+            gc_edge_flux(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);            // edge r-1
+            if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
+        }
         if (live && r >= 3 && count) cflm = dmax(cflm, gc_edge_cfl(Wc, rd2, rd1));
         if (live && r >= 4) {                                                           // cell r-2
             const double dtdx = dt * rd2;
@@ -355,6 +373,28 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
         a.lines = L->d_yl; a.nlines = L->nyl_lines;
         if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_march<1><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, 0, L->ctx->stream>>>(a); }
     } else if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
+}
+
+// ---- self-test of gc_math.cuh: MathFast against the IEEE operators on caller-supplied operands
+__global__ void k_math_selftest(const double *a, const double *b, int64_t n, unsigned long long *out)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double x = a[i], y = b[i];
+    MathIeee mi;
+    { MathFast mf; double q = mf.div(x, y);
+      if (mf.failed()) atomicAdd(out + 1, 1ull);
+      else if (__double_as_longlong(q) != __double_as_longlong(mi.div(x, y))) atomicAdd(out, 1ull); }
+    { MathFast mf; double q = mf.rcp(y);
+      if (mf.failed()) atomicAdd(out + 1, 1ull);
+      else if (__double_as_longlong(q) != __double_as_longlong(mi.rcp(y))) atomicAdd(out, 1ull); }
+    { MathFast mf; double q = mf.sqrt_(x);
+      if (mf.failed()) atomicAdd(out + 1, 1ull);
+      else if (__double_as_longlong(q) != __double_as_longlong(mi.sqrt_(x))) atomicAdd(out, 1ull); }
+}
+void gc_launch_math_selftest(cudaStream_t s, const double *a, const double *b, int64_t n, unsigned long long *out)
+{
+    if (n > 0) k_math_selftest<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(a, b, n, out);
 }
 
 // ---- fp64 ALU peak probe: dependent DFMA chains, 8 independent accumulators per thread
