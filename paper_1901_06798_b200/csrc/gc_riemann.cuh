@@ -185,3 +185,97 @@ __device__ __forceinline__ void gc_riemann(M &m, double g, double eps, RState L,
     if (!m1) { s[1] = 0.0; Z[1][0] = 0.0; Z[1][1] = 0.0; Z[1][2] = 0.0; }
     if (!m2) { s[2] = 0.0; Z[2][0] = 0.0; Z[2][1] = 0.0; Z[2][2] = 0.0; }
 }
+
+// ---- straight-line variants for the common case --------------------------------------------------------------
+// The same expressions in the same order as gc_prim / gc_riemann, specialised to the branch an open-ocean edge takes
+// (both sides wet, one shock + one rarefaction in R5, not near-critical in R7, subcritical clamp l1 < -tau < tau < l3)
+// and written without control flow, so that the independent divide / square-root chains can overlap.  They return
+// false when the edge is not of that kind (or a fast-math operand left its window); the caller then runs the
+// general code above.  Where both apply they produce identical bits.
+
+// R0 + R2 without branches (the reciprocal of a dry cell's depth is taken of 1 and discarded)
+__device__ __forceinline__ void gc_prim_fast(MathFast &m, RState &S, double g, double eps)
+{
+    const bool wet = S.h > eps;                       // h < 0 and h <= eps both end as the zero state
+    const double hs = wet ? S.h : 1.0;
+    const double rh = m.rcp(hs);
+    const double u = S.p * rh, v = S.t * rh;
+    const double phi = S.p * u + 0.5 * g * (S.h * S.h);
+    S.h = wet ? S.h : 0.0; S.p = wet ? S.p : 0.0; S.t = wet ? S.t : 0.0;
+    S.u = wet ? u : 0.0; S.v = wet ? v : 0.0; S.phi = wet ? phi : 0.0;
+    S.c = m.sqrt_(g * S.h);
+}
+
+__device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double eps, const RState &L, const RState &R,
+                                                double (&Z)[3][3], double (&s)[3])
+{
+    bool ok = (L.h > eps) && (R.h > eps);
+    const double hL = ok ? L.h : 1.0, hR = ok ? R.h : 1.0;         // keep the arithmetic below inside the window
+    const double cL = ok ? L.c : 1.0, cR = ok ? R.c : 1.0;
+    // R4
+    const double sL = L.u - cL, sR = R.u + cR;
+    const double uhat = m.div(cL * L.u + cR * R.u, cL + cR);
+    const double chat = m.sqrt_(g * (0.5 * (hL + hR)));
+    const double sE1 = dmin(sL, uhat - chat);
+    const double sE2 = dmax(sR, uhat + chat);
+    // R5, shock + rarefaction branch
+    const double hmin = dmin(hL, hR), hmax = dmax(hL, hR);
+    const double du = R.u - L.u;
+    const double cmin = (hL < hR) ? cL : cR;
+    const double cmax = (hL < hR) ? cR : cL;
+    const double Fmin = du + 2.0 * (cmin - cmax);
+    const double Fmax = du + (hmax - hmin) * m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin));
+    ok = ok && !(Fmin > 0.0) && !(Fmax <= 0.0);
+    const double dF = Fmax - Fmin;
+    const double h1 = hmin - m.div(Fmin * (hmax - hmin), ok ? dF : 1.0);
+    const double cm = m.sqrt_(g * (ok ? h1 : 1.0));
+    const double aL = L.u + 2.0 * cL, aR = R.u - 2.0 * cR;
+    const bool deepL = hL > hR;
+    const double s1m = deepL ? (aL - 3.0 * cm) : (aR + cm);
+    const double s2m = deepL ? (aL - cm) : (aR + 3.0 * cm);
+    // R6
+    const double l1 = dmin(sE1, s2m);
+    const double l3 = dmax(sE2, s1m);
+    const double l2 = 0.5 * (l1 + l3);
+    // R7, not near-critical, subcritical clamp
+    const double delb = R.b - L.b;
+    const double hbar = dmax(0.5 * (hL + hR), 0.0);
+    const double ghbar = g * hbar;
+    const double su = L.u + R.u;
+    const double pbar = 0.25 * (su * su) - ghbar;
+    const double ptil = dmax(0.0, L.u * R.u) - ghbar;
+    const double hsd = dmax(0.0, ((L.p - R.p) + l3 * hR) - l1 * hL);
+    bool sonic = fabs(pbar) <= GC_TAU;
+    sonic = sonic || (pbar * ptil <= GC_TAU);
+    sonic = sonic || (pbar * l1 * l3 <= GC_TAU);
+    sonic = sonic || (dmin(fabs(l1), fabs(l3)) < GC_SQRT_TAU);
+    sonic = sonic || (l1 < GC_SQRT_TAU && s1m > -GC_SQRT_TAU);
+    sonic = sonic || (l3 > -GC_SQRT_TAU && s2m < GC_SQRT_TAU);
+    sonic = sonic || ((L.u + cL) * (R.u + cR) < 0.0);
+    sonic = sonic || ((L.u - cL) * (R.u - cR) < 0.0);
+    ok = ok && !sonic && (l1 < -GC_TAU) && (l3 > GC_TAU);
+    const double q = m.div(ghbar, ok ? pbar : 1.0);
+    double dh = delb * q;
+    double dphi = -delb * (q * ptil);
+    dh = dmin(dh, m.div(hsd, ok ? l3 : 1.0));
+    dh = dmax(dh, m.div(hsd, ok ? l1 : 1.0));
+    {
+        const double a = -hL * delb, c = -hR * delb;
+        dphi = dmin(dphi, g * dmax(a, c));
+        dphi = dmax(dphi, g * dmin(a, c));
+    }
+    // R8
+    const double d1 = (hR - hL) - dh;
+    const double d2 = R.p - L.p;
+    const double d3 = (R.phi - L.phi) - dphi;
+    const double rdl = m.rcp(ok ? (l3 - l1) : 1.0);
+    const double l1sq = l1 * l1, l3sq = l3 * l3;
+    const double b1 = (l3 * d1 - d2) * rdl;
+    const double b3 = (d2 - l1 * d1) * rdl;
+    const double b2 = (d3 - l1sq * b1) - l3sq * b3;
+    Z[0][0] = b1 * l1; Z[0][1] = b1 * l1sq; Z[0][2] = L.v * Z[0][0];
+    Z[2][0] = b3 * l3; Z[2][1] = b3 * l3sq; Z[2][2] = R.v * Z[2][0];
+    Z[1][0] = 0.0;     Z[1][1] = b2;        Z[1][2] = ((R.p * R.v - L.p * L.v) - Z[0][2]) - Z[2][2];
+    s[0] = l1; s[1] = l2; s[2] = l3;
+    return ok && !m.failed();
+}

@@ -98,3 +98,36 @@ __device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double
     }
     return m;
 }
+
+// (3)-(6) without control flow (same values as gc_edge_flux: a skipped term is added as +0.0, which changes no bit
+// because the sums start at +0.0 and can therefore never be -0.0).  m.failed() afterwards: redo with gc_edge_flux.
+__device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
+                                                  double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
+{
+    double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
+    const double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+#pragma unroll
+    for (int w = 0; w < 3; w++) {
+        const double sw = W.s[w];
+        const bool neg = sw < 0.0, pos = sw > 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const double z = W.Z[w][c], hz = 0.5 * z;
+            am[c] = am[c] + (neg ? z : (pos ? 0.0 : hz));
+            ap[c] = ap[c] + (pos ? z : (neg ? 0.0 : hz));
+        }
+        if (limiter != 0) {
+            const double zz = (W.Z[w][0] * W.Z[w][0] + W.Z[w][1] * W.Z[w][1]) + W.Z[w][2] * W.Z[w][2];
+            const bool nz = zz != 0.0;
+            const double theta = m.div(pos ? dlo[w] : dhi[w], nz ? zz : 1.0);                       // eq. 10 (S-1), eq. 11
+            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));          // MC
+            const double phi = nz ? mc : 1.0;
+            const double coef = (pos ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
+            const bool on = neg || pos;                                                              // sgn(0) = 0 (S-4)
+#pragma unroll
+            for (int c = 0; c < 3; c++) { const double t = coef * (phi * W.Z[w][c]); F[c] = F[c] + (on ? t : 0.0); }   // eq. 9
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
+}

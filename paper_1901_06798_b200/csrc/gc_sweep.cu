@@ -268,17 +268,23 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
 
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
         Waves Wn;
-        {   // fast math first; an operand outside its window (gc_math.cuh) redoes this cell + edge with the IEEE operators
+        {   // straight-line code for an open-ocean edge first (gc_riemann_fast); any other kind of edge, or a fast-math
+            // operand outside its window (gc_math.cuh), redoes this cell + edge with the general code and IEEE operators
             MathFast mf;
-            RState R0 = R;
-            gc_prim(mf, R, a.g, a.eps);
-            if (r >= 1 && live) gc_solve_edge_prim(mf, a.g, a.eps, Lst, R, a.coord, ef, Wn);    // edge r (between cells r-1, r)
+            const RState R0 = R;
+            gc_prim_fast(mf, R, a.g, a.eps);
+            bool ok = !mf.failed();
+            if (r >= 1 && live) ok = gc_riemann_fast(mf, a.g, a.eps, Lst, R, Wn.Z, Wn.s) && ok;
             else gc_waves_zero(Wn);
-            if (mf.failed()) {
+            if (!ok) {
                 MathIeee mi;
                 R = R0;
                 gc_prim(mi, R, a.g, a.eps);
-                if (r >= 1 && live) gc_solve_edge_prim(mi, a.g, a.eps, Lst, R, a.coord, ef, Wn);
+                if (r >= 1 && live) gc_riemann(mi, a.g, a.eps, Lst, R, Wn.Z, Wn.s);
+            }
+            if (a.coord == 1) {                                   // scale by the edge factor
+#pragma unroll
+                for (int w = 0; w < 3; w++) { Wn.s[w] = Wn.s[w] * ef; Wn.Z[w][0] = Wn.Z[w][0] * ef; Wn.Z[w][1] = Wn.Z[w][1] * ef; Wn.Z[w][2] = Wn.Z[w][2] * ef; }
             }
         }
         double dhi[3];
@@ -286,7 +292,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         double fm[3], fp[3];
         {
             MathFast mf;
-            gc_edge_flux(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);            // edge r-1
+            gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);       // edge r-1
             if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
         }
         if (live && r >= 3 && count) cflm = dmax(cflm, gc_edge_cfl(Wc, rd2, rd1));
