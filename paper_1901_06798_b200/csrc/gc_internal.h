@@ -38,19 +38,24 @@ struct CopyRect {
     int32_t w, h, dpitch, spitch;
 };
 
-// one fine cell to be interpolated from the coarser level (ghost fill A3 / regrid transfer A11)
-struct CoarseFillItem {
-    int64_t dst;            // element offset in the fine plane
-    int64_t csrc;           // element offset of the coarse cell (I,J) in the coarse plane
-    int32_t cpitch;         // pitch of that coarse patch
-    int16_t ii, jj;         // position of the fine cell inside the coarse cell, 0..r-1
+// a rectangle of fine cells (w x h) lying inside ONE coarse patch, to be interpolated from the coarser level
+// (ghost fill A3 / regrid transfer A11).  Fine cell (x, y) of the rectangle sits at sub-position
+// ((ii0 + x) % r, (jj0 + y) % r) of the coarse cell csrc + ((jj0 + y) / r) * cpitch + (ii0 + x) / r.
+struct CoarseFillRect {
+    int64_t dst;            // element offset of the rectangle's lower-left fine cell in the fine plane
+    int64_t csrc;           // element offset, in the coarse plane, of the coarse cell holding that fine cell
+    int32_t dpitch, cpitch;
+    int32_t w, h;
+    int32_t ii0, jj0;       // sub-position of the lower-left fine cell inside its coarse cell, 0..r-1
 };
 
-struct AvgItem {            // average-down A9: one covered coarse cell
-    int64_t cdst;           // coarse plane offset
-    int64_t fsrc;           // fine plane offset of the lower-left fine cell
-    int32_t fpitch;
-    int32_t frow;           // global fine row of the lower-left fine cell (for kappa weights)
+struct AvgRect {            // average-down A9: w x h covered coarse cells under one fine patch, inside one coarse patch
+    int64_t cdst;           // coarse plane offset of the lower-left coarse cell
+    int64_t fsrc;           // fine plane offset of the lower-left fine cell under it
+    int32_t cpitch, fpitch;
+    int32_t w, h;
+    int32_t frow;           // table index (global fine row + 2) of that fine cell, for the kappa weights
+    int32_t pad;
 };
 
 struct FluxReg {            // A8, one register (coarse edge on the boundary of the fine region)
@@ -120,7 +125,7 @@ struct gc_level {
     std::vector<int64_t> coarse_ghost;              // plane offsets + global indices of ghosts to be filled from the coarser level
     std::vector<int32_t> coarse_ghost_ij;           // (gi, gj) pairs
     // cached coarse-fill list for a given coarser level (rebuilt when the coarser level changes)
-    const gc_level *cf_for; uint64_t cf_gen; CoarseFillItem *d_cf; int64_t ncf;
+    const gc_level *cf_for; uint64_t cf_gen; CoarseFillRect *d_cf; int64_t *d_cfstart; int ncf; int64_t ncfcells;
     uint64_t gen;                                   // unique id of this level object
     DevStats *d_stats;
     double *d_partial;                              // np doubles (mass partials)
@@ -129,8 +134,11 @@ struct gc_level {
     const gc_level *reg_fine; gc_level *reg_coarse;
     FluxReg *d_reg; int nreg; int r_reg;
     double *d_delta, *d_base;                       // nreg*3, nreg*4
-    int64_t *d_fixcell; int32_t *d_fixstart; int nfix;  // registers grouped by coarse cell for the fix-up
+    int32_t *d_fixstart; int nfix;                  // registers grouped by coarse cell for the fix-up: group g = d_fixreg[d_fixstart[g] .. d_fixstart[g+1])
     int32_t *d_fixreg;
+    // cached average-down list for a given fine level, cached neighbour lists for flag dilation
+    uint64_t avg_gen; AvgRect *d_avg; int64_t *d_avgstart; int navg; int64_t navgcells;
+    int nbr_buffer; int32_t *d_nbrstart, *d_nbrlist;
 };
 
 // ---- helpers (gc_api.cu)
@@ -156,11 +164,12 @@ void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *sr
 void gc_launch_wet_mask(const gc_level *L, uint8_t *mask);
 void gc_launch_mass(const gc_level *L);
 // gc_amr.cu
-void gc_launch_coarse_fill(gc_level *L, const gc_level *C, const CoarseFillItem *items, int64_t n, double alpha, int use_old);
-void gc_launch_average_down(gc_level *C, const gc_level *F, const AvgItem *items, int64_t n);
+void gc_launch_coarse_fill(gc_level *L, const gc_level *C, const CoarseFillRect *rects, const int64_t *start, int n, int64_t ncells,
+                           double alpha, int use_old, int slot);
+void gc_launch_average_down(gc_level *C, const gc_level *F, const AvgRect *rects, const int64_t *start, int n, int64_t ncells);
 void gc_launch_flags(const gc_level *L, const gc_flag_params *fp, const double *d_boxes, double t, uint8_t *raw, uint8_t *flags,
-                     const int32_t *nbr_start, const int32_t *nbr_list);
+                     const int32_t *nbr_start, const int32_t *nbr_list, unsigned long long *d_count);
 void gc_launch_copy_overlap(gc_level *N, const gc_level *O, const CopyRect *rects, int n);
-void gc_launch_flux_coarse(gc_level *C, double dt);
-void gc_launch_flux_fine(gc_level *F, double dt);
+void gc_launch_flux_coarse(gc_level *C, double dt, const double *dt_dev);
+void gc_launch_flux_fine(gc_level *F, double dt, const double *dt_dev);
 void gc_launch_flux_fixup(gc_level *C);
