@@ -306,9 +306,11 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     L->nbcp = (int)bcp.size(); L->d_bcp = upload(L, bcp);
     L->d_stats = (DevStats *)gc_dev_alloc(ctx, sizeof(DevStats)); L->allocs.push_back(L->d_stats);
     L->d_partial = (double *)gc_dev_alloc(ctx, sizeof(double) * (np > 0 ? np : 1)); L->allocs.push_back(L->d_partial);
-    L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->ncf = 0;
+    L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->d_cfstart = nullptr; L->ncf = 0; L->ncfcells = 0;
+    L->avg_gen = 0; L->d_avg = nullptr; L->d_avgstart = nullptr; L->navg = 0; L->navgcells = 0;
+    L->nbr_buffer = -1; L->d_nbrstart = nullptr; L->d_nbrlist = nullptr; L->r_reg = 1;
     L->reg_fine = nullptr; L->reg_coarse = nullptr; L->d_reg = nullptr; L->nreg = 0;
-    L->d_delta = nullptr; L->d_base = nullptr; L->d_fixcell = nullptr; L->d_fixstart = nullptr; L->d_fixreg = nullptr; L->nfix = 0;
+    L->d_delta = nullptr; L->d_base = nullptr; L->d_fixstart = nullptr; L->d_fixreg = nullptr; L->nfix = 0;
     if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_xl || !L->d_yl || !L->d_copy || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
         gc_level_destroy(L);
         return gc_fail(ctx, GC_ERR_NOMEM, "gc_level_create: table allocation failed");
@@ -321,9 +323,12 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     return GC_OK;
 }
 
+void gc_amr_on_destroy(gc_level *L);
+
 extern "C" int gc_level_destroy(gc_level *L)
 {
     if (!L) return GC_OK;
+    gc_amr_on_destroy(L);
     cudaStreamSynchronize(L->ctx->stream);
     for (void *p : L->allocs) gc_dev_free(L->ctx, p);
     delete L;
@@ -408,6 +413,7 @@ extern "C" int gc_fill_ghost_b(gc_level *L)
 }
 
 int gc_fill_coarse_ghosts(gc_level *L, const gc_level *C, double alpha);   // gc_api_amr.cu
+void gc_amr_on_destroy(gc_level *L);                                       // gc_api_amr.cu
 int gc_flux_after_step(gc_level *L, double dt, const double *dt_dev);     // gc_api_amr.cu
 
 extern "C" int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha)

@@ -131,7 +131,7 @@ struct gc_level {
     double *d_partial;                              // np doubles (mass partials)
     std::vector<void *> allocs;
     // flux registers (this level as the coarse side) + capture slots
-    const gc_level *reg_fine; gc_level *reg_coarse;
+    const gc_level *reg_fine; gc_level *reg_coarse;   // cleared by gc_level_destroy of either side
     FluxReg *d_reg; int nreg; int r_reg;
     double *d_delta, *d_base;                       // nreg*3, nreg*4
     int32_t *d_fixstart; int nfix;                  // registers grouped by coarse cell for the fix-up: group g = d_fixreg[d_fixstart[g] .. d_fixstart[g+1])

@@ -64,3 +64,258 @@ def run_single_level(L, nsteps, cfl, dt0=None, record=None):
             record(n, dt, st, L)
         dt = cfl / st["s_over_dx_max"]
     return hist
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Clustering ("Berger-Rigoutsos"): flagged cells of level l -> rectangles.  Deterministic (ties to the
+# lower index), shared by both backends AFTER their flags have been compared bit for bit (DESIGN.md 3.9 S-13).
+def _signature_cut(sig):
+    """Cut position (1..n-1) for a 1-D signature: first a hole (zero entry) nearest the centre, else the strongest
+    inflection of the discrete Laplacian; None if neither exists."""
+    n = len(sig)
+    zeros = [k for k in range(1, n - 1) if sig[k] == 0]
+    if zeros:
+        k = min(zeros, key=lambda z: (abs(z - n / 2.0), z))
+        return k
+    if n < 4:
+        return None
+    lap = sig[:-2] - 2 * sig[1:-1] + sig[2:]          # lap[k] belongs to cell k+1
+    best, bestk = 0, None
+    for k in range(len(lap) - 1):
+        if lap[k] * lap[k + 1] < 0:
+            mag = abs(int(lap[k]) - int(lap[k + 1]))
+            if mag > best or (mag == best and bestk is not None and abs(k + 2 - n / 2.0) < abs(bestk - n / 2.0)):
+                best, bestk = mag, k + 2               # cut between cells k+1 and k+2
+    return bestk
+
+
+def cluster(flags, valid=None, efficiency=0.7, max_side=64):
+    """flags: 2-D uint8 (ny, nx) of one level.  valid (optional, same shape): cells a box may contain.
+    Returns a list of (i0, j0, nx, ny) boxes (cells of that level), disjoint, covering every flagged cell,
+    sorted by (j0, i0)."""
+    out = []
+    fl = np.asarray(flags, dtype=bool)
+    stack = [(0, 0, fl.shape[1], fl.shape[0])]
+    while stack:
+        i0, j0, nx, ny = stack.pop()
+        sub = fl[j0:j0 + ny, i0:i0 + nx]
+        if not sub.any():
+            continue
+        sx = sub.sum(axis=0); sy = sub.sum(axis=1)
+        xs = np.nonzero(sx)[0]; ys = np.nonzero(sy)[0]
+        i0, nx = i0 + int(xs[0]), int(xs[-1] - xs[0] + 1)
+        j0, ny = j0 + int(ys[0]), int(ys[-1] - ys[0] + 1)
+        sub = fl[j0:j0 + ny, i0:i0 + nx]
+        sx = sub.sum(axis=0).astype(np.int64); sy = sub.sum(axis=1).astype(np.int64)
+        ok_valid = True if valid is None else bool(valid[j0:j0 + ny, i0:i0 + nx].all())
+        eff = sub.sum() / float(nx * ny)
+        if eff >= efficiency and ok_valid and nx <= max_side and ny <= max_side:
+            out.append((i0, j0, nx, ny))
+            continue
+        cut = None
+        if nx > max_side or ny > max_side:             # chop oversize boxes first, in the middle of the long side
+            cut = ("x", nx // 2) if nx >= ny else ("y", ny // 2)
+        else:
+            cx = _signature_cut(sx); cy = _signature_cut(sy)
+            hx = cx is not None and sx[cx] == 0; hy = cy is not None and sy[cy] == 0
+            if hx or hy:
+                cut = ("x", cx) if (hx and (not hy or nx >= ny)) else ("y", cy)
+            elif cx is not None or cy is not None:
+                cut = ("x", cx) if (cx is not None and (cy is None or nx >= ny)) else ("y", cy)
+            elif nx > 1 or ny > 1:
+                cut = ("x", nx // 2) if nx >= ny else ("y", ny // 2)
+        if cut is None:                                 # a single cell: accept (flagged cells are valid by construction)
+            out.append((i0, j0, nx, ny))
+            continue
+        if cut[0] == "x":
+            stack.append((i0 + cut[1], j0, nx - cut[1], ny)); stack.append((i0, j0, cut[1], ny))
+        else:
+            stack.append((i0, j0 + cut[1], nx, ny - cut[1])); stack.append((i0, j0, nx, cut[1]))
+    out.sort(key=lambda b: (b[1], b[0]))
+    return out
+
+
+def unpack_cells(L, packed, fill=0):
+    """interior-packed per-patch array (flags, masks) -> level-global 2-D array"""
+    out = np.full((L.nyl, L.nxl), fill, dtype=packed.dtype)
+    o = 0
+    for i0, j0, nx, ny in L.patches:
+        out[j0:j0 + ny, i0:i0 + nx] = packed[o:o + nx * ny].reshape(ny, nx)
+        o += nx * ny
+    return out
+
+
+def nesting_mask(L):
+    """Cells of level L whose 3x3 neighbourhood (clipped to the domain) lies inside the level: a finer patch on
+    top of them has every ghost cell over level-L interior cells (proper nesting by one coarse cell)."""
+    cov = np.zeros((L.nyl + 2, L.nxl + 2), dtype=bool)
+    cov[0, :] = cov[-1, :] = True; cov[:, 0] = cov[:, -1] = True     # outside the domain counts as fine (physical BC)
+    for i0, j0, nx, ny in L.patches:
+        cov[j0 + 1:j0 + ny + 1, i0 + 1:i0 + nx + 1] = True
+    ok = np.ones((L.nyl, L.nxl), dtype=bool)
+    for dj in (0, 1, 2):
+        for di in (0, 1, 2):
+            ok &= cov[dj:dj + L.nyl, di:di + L.nxl]
+    return ok
+
+
+class Hierarchy:
+    """The AMR recursion of P:140-146 (steps 1-5) with regridding every `regrid_interval` steps of a level,
+    driving one backend through the C-ABI calls.  Bookkeeping only."""
+
+    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7):
+        self.ctx, self.wl, self.reflux, self.eff = ctx, wl, reflux, efficiency
+        nl = 1 + len(wl.ratios) if max_levels is None else min(max_levels, 1 + len(wl.ratios))
+        self.ratios = list(wl.ratios)[:nl - 1]
+        self.levels = [setup_level(ctx, wl, patches=patches1)]
+        self.t = 0.0
+        self.alpha_now = [1.0]          # time of level l inside the last step of level l-1, as a fraction
+        self.steps = [0]
+        self.sdx = [0.0]
+        self.updates = 0
+        self.flag_log = []              # (level index, t, packed flags) of every flagging pass, for parity checks
+        self.regrids = 0
+        self._regrid(0, initial=True)
+
+    # ---- geometry of level index k (0-based)
+    def _geom(self, k):
+        R = 1
+        for r in self.ratios[:k]:
+            R *= r
+        return self.wl.dx / R, self.wl.dy / R, self.wl.nx * R, self.wl.ny * R
+
+    def _flag_boxes(self, k):
+        """flag level k, cluster -> patches of level k+1 (in cells of level k+1), or None"""
+        L = self.levels[k]
+        f = dict(self.wl.flag)
+        boxes = [b[1:] for b in self.wl.forced_boxes if b[0] == k + 1]
+        packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0), tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
+                           buffer=f.get("buffer", 0), boxes=boxes, t=self.t)
+        self.flag_log.append((k, self.t, packed.copy()))
+        if n == 0:
+            return None
+        fl = unpack_cells(L, packed).astype(bool)
+        ok = nesting_mask(L)
+        fl &= ok
+        if not fl.any():
+            return None
+        r = self.ratios[k]
+        boxes = cluster(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
+        return np.array([[b[0] * r, b[1] * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
+
+    def _regrid(self, k0, initial=False):
+        """rebuild levels k0+1.. from the flags of the level below each"""
+        self.regrids += 0 if initial else 1
+        for k in range(k0, len(self.ratios)):
+            if k >= len(self.levels):
+                break
+            C = self.levels[k]
+            pats = self._flag_boxes(k)
+            old = self.levels[k + 1] if k + 1 < len(self.levels) else None
+            if pats is None:
+                for L in self.levels[k + 1:]:
+                    L.destroy()
+                del self.levels[k + 1:]; del self.alpha_now[k + 1:]; del self.steps[k + 1:]; del self.sdx[k + 1:]
+                break
+            dx, dy, nxl, nyl = self._geom(k + 1)
+            N = self.ctx.level_create(k + 2, self.wl.xlo, self.wl.ylo, dx, dy, nxl, nyl, self.ratios[k], pats)
+            set_initial(N, self.wl, state=initial)
+            if not initial:
+                C.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
+                N.init_from(old, C)
+            if old is not None:
+                old.destroy()
+                self.levels[k + 1] = N
+            else:
+                self.levels.append(N); self.alpha_now.append(1.0); self.steps.append(0); self.sdx.append(0.0)
+            if self.reflux:
+                C.flux_attach(N)
+
+    def probe(self):
+        """dt of level 1 from dt = 0 probe steps of every level"""
+        m, R = 0.0, 1
+        for k, L in enumerate(self.levels):
+            R = R * (self.ratios[k - 1] if k > 0 else 1)
+            L.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
+            m = max(m, L.step(0.0)["s_over_dx_max"] / R)
+        return self.wl.cfl / m
+
+    def _advance(self, k, dt, alpha):
+        L = self.levels[k]
+        L.fill_ghost(self.levels[k - 1] if k > 0 else None, alpha)
+        st = L.step(dt)
+        self.sdx[k] = max(self.sdx[k], st["s_over_dx_max"])
+        self.steps[k] += 1
+        self.updates += L.ncells
+        if k + 1 < len(self.levels):
+            r = self.ratios[k]
+            for s in range(r):
+                self.alpha_now[k + 1] = (s + 1) / r
+                self._advance(k + 1, dt / r, s / r)
+        if k + 1 < len(self.levels):        # the finer level may have vanished in a regrid below
+            F = self.levels[k + 1]
+            if self.reflux:
+                L.flux_fixup(F)
+            L.average_down_from(F)
+        if k > 0 and k < len(self.ratios) and self.steps[k] % self.wl.regrid_interval == 0:
+            self._regrid(k)
+
+    def step(self, dt):
+        """one step of level 1 (and everything above it); returns the next dt of level 1"""
+        self.sdx = [0.0] * len(self.levels)
+        self.alpha_now[0] = 1.0
+        self._advance(0, dt, 1.0)
+        self.t += dt
+        if len(self.ratios) > 0 and self.steps[0] % self.wl.regrid_interval == 0:
+            self._regrid(0)
+        m, R = 0.0, 1
+        for k in range(len(self.sdx)):
+            R = R * (self.ratios[k - 1] if k > 0 else 1)
+            m = max(m, self.sdx[k] / R)
+        return self.wl.cfl / m
+
+    def run(self, nsteps=None, t_end=None, record=None):
+        dt = self.probe()
+        n = 0
+        while (nsteps is None or n < nsteps) and (t_end is None or self.t < t_end):
+            if t_end is not None and self.t + dt > t_end:
+                dt = t_end - self.t
+            dtn = self.step(dt)
+            if record is not None:
+                record(n, dt, self)
+            dt = dtn
+            n += 1
+        return n
+
+    def composite_mass(self):
+        """mass over the finest available cells: sum over levels of the mass of cells not covered by a finer level.
+        Needs get_global on every level (small test problems only)."""
+        tot = 0.0
+        for k, L in enumerate(self.levels):
+            h = L.get_global("h", fill=0.0)
+            kap = self._kappa(L)
+            w = np.ones_like(h, dtype=bool)
+            cov = np.zeros_like(w)
+            for i0, j0, nx, ny in L.patches:
+                cov[j0:j0 + ny, i0:i0 + nx] = True
+            w &= cov
+            if k + 1 < len(self.levels):
+                r = self.ratios[k]
+                for i0, j0, nx, ny in self.levels[k + 1].patches:
+                    w[j0 // r:(j0 + ny) // r, i0 // r:(i0 + nx) // r] = False
+            tot += float((h * kap[:, None] * (L.dx * L.dy))[w].sum())
+        return tot
+
+    def _kappa(self, L):
+        if self.wl.params.get("coord", 0) == 0:
+            return np.ones(L.nyl)
+        R = self.wl.params.get("earth_radius", 6367500.0)
+        d2r = np.pi / 180.0
+        lat0 = (L.ylo + np.arange(L.nyl) * L.dy) * d2r
+        lat1 = (L.ylo + (np.arange(L.nyl) + 1) * L.dy) * d2r
+        return d2r * R * R * (np.sin(lat1) - np.sin(lat0)) / L.dy
+
+    def destroy(self):
+        for L in self.levels:
+            L.destroy()
+        self.levels = []
