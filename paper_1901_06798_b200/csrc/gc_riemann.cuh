@@ -206,12 +206,13 @@ __device__ __forceinline__ void gc_prim_fast(MathFast &m, RState &S, double g, d
     S.c = m.sqrt_(g * S.h);
 }
 
+// Lanes whose edge is not of that kind compute garbage (possibly Inf / NaN: harmless, nothing traps) that the caller
+// discards; only the returned flag decides.
 __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double eps, const RState &L, const RState &R,
                                                 double (&Z)[3][3], double (&s)[3])
 {
     bool ok = (L.h > eps) && (R.h > eps);
-    const double hL = ok ? L.h : 1.0, hR = ok ? R.h : 1.0;         // keep the arithmetic below inside the window
-    const double cL = ok ? L.c : 1.0, cR = ok ? R.c : 1.0;
+    const double hL = L.h, hR = R.h, cL = L.c, cR = R.c;
     // R4
     const double sL = L.u - cL, sR = R.u + cR;
     const double uhat = m.div(cL * L.u + cR * R.u, cL + cR);
@@ -219,18 +220,17 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double sE1 = dmin(sL, uhat - chat);
     const double sE2 = dmax(sR, uhat + chat);
     // R5, shock + rarefaction branch
-    const double hmin = dmin(hL, hR), hmax = dmax(hL, hR);
+    const bool deepL = hL > hR, shalL = hL < hR;
+    const double hmin = shalL ? hL : hR, hmax = hL > hR ? hL : hR;
     const double du = R.u - L.u;
-    const double cmin = (hL < hR) ? cL : cR;
-    const double cmax = (hL < hR) ? cR : cL;
+    const double cmin = shalL ? cL : cR;
+    const double cmax = shalL ? cR : cL;
     const double Fmin = du + 2.0 * (cmin - cmax);
     const double Fmax = du + (hmax - hmin) * m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin));
     ok = ok && !(Fmin > 0.0) && !(Fmax <= 0.0);
-    const double dF = Fmax - Fmin;
-    const double h1 = hmin - m.div(Fmin * (hmax - hmin), ok ? dF : 1.0);
-    const double cm = m.sqrt_(g * (ok ? h1 : 1.0));
+    const double h1 = hmin - m.div(Fmin * (hmax - hmin), Fmax - Fmin);
+    const double cm = m.sqrt_(g * h1);
     const double aL = L.u + 2.0 * cL, aR = R.u - 2.0 * cR;
-    const bool deepL = hL > hR;
     const double s1m = deepL ? (aL - 3.0 * cm) : (aR + cm);
     const double s2m = deepL ? (aL - cm) : (aR + 3.0 * cm);
     // R6
@@ -254,11 +254,17 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     sonic = sonic || ((L.u + cL) * (R.u + cR) < 0.0);
     sonic = sonic || ((L.u - cL) * (R.u - cR) < 0.0);
     ok = ok && !sonic && (l1 < -GC_TAU) && (l3 > GC_TAU);
-    const double q = m.div(ghbar, ok ? pbar : 1.0);
-    double dh = delb * q;
+    const double q = m.div(ghbar, pbar);
+    const double dh = delb * q;
     double dphi = -delb * (q * ptil);
-    dh = dmin(dh, m.div(hsd, ok ? l3 : 1.0));
-    dh = dmax(dh, m.div(hsd, ok ? l1 : 1.0));
+    // The clamp dh <- max(min(dh, hsd / l3), hsd / l1) is the identity when dh lies inside the bounds.  That is decided
+    // without the two divides, with a margin far above the rounding of the products and of the quotients:
+    //   dh * l3 < hsd (1 - 1e-7)  =>  dh < fl(hsd / l3);   dh * l1 < hsd (1 - 1e-7)  =>  dh > fl(hsd / l1)   (l1 < 0 < l3).
+    // hsd > 1e-100 and |dh| < 1e100 keep every product away from underflow / overflow (|l| >= tau).  Otherwise: general code.
+    {
+        const double hs = hsd * 0.9999999;
+        ok = ok && (hsd > 1.0e-100) && (fabs(dh) < 1.0e100) && (dh * l3 < hs) && (dh * l1 < hs);
+    }
     {
         const double a = -hL * delb, c = -hR * delb;
         dphi = dmin(dphi, g * dmax(a, c));
@@ -268,7 +274,7 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double d1 = (hR - hL) - dh;
     const double d2 = R.p - L.p;
     const double d3 = (R.phi - L.phi) - dphi;
-    const double rdl = m.rcp(ok ? (l3 - l1) : 1.0);
+    const double rdl = m.rcp(l3 - l1);
     const double l1sq = l1 * l1, l3sq = l3 * l3;
     const double b1 = (l3 * d1 - d2) * rdl;
     const double b3 = (d2 - l1 * d1) * rdl;

@@ -131,3 +131,70 @@ __device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, c
 #pragma unroll
     for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
 }
+
+// (3)-(6) for a "standard" edge: s[0] < 0 < s[2] is known (every edge solved by gc_riemann_fast: l1 < -tau, l3 > tau, and
+// the edge factor is positive), so families 1 and 3 need no sign tests; only the corrector family 2 keeps them.
+// Same values as gc_edge_flux: the sums are formed in the same order, a skipped term is added as +0.0 (no bit changes:
+// the partial sums start at +0.0 and are therefore never -0.0), |s0| = -s0 exactly, Z[1][0] is +0.0 by construction.
+// m.failed() afterwards: redo with gc_edge_flux.
+__device__ __forceinline__ void gc_edge_flux_std(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
+                                                 double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
+{
+    const double s0 = W.s[0], s1 = W.s[1], s2 = W.s[2];
+    const bool neg1 = s1 < 0.0, pos1 = s1 > 0.0;
+    double am[3], ap[3], F[3] = {0.0, 0.0, 0.0};
+    am[0] = 0.0 + W.Z[0][0];
+    ap[0] = 0.0 + W.Z[2][0];
+#pragma unroll
+    for (int c = 1; c < 3; c++) {
+        const double z = W.Z[1][c], hz = 0.5 * z;
+        am[c] = (0.0 + W.Z[0][c]) + (neg1 ? z : (pos1 ? 0.0 : hz));
+        ap[c] = (0.0 + (pos1 ? z : (neg1 ? 0.0 : hz))) + W.Z[2][c];
+    }
+    if (limiter != 0) {
+        const double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+        {   // family 1: s < 0, upwind neighbour e+1
+            const double zz = (W.Z[0][0] * W.Z[0][0] + W.Z[0][1] * W.Z[0][1]) + W.Z[0][2] * W.Z[0][2];
+            const bool nz = zz != 0.0;
+            const double theta = m.div(dhi[0], nz ? zz : 1.0);
+            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
+            const double phi = nz ? mc : 1.0;
+            const double coef = -0.5 * (1.0 - (-s0) * dtdx_ave);
+#pragma unroll
+            for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[0][c]);
+        }
+        {   // family 2: either sign, sgn(0) = 0
+            const double zz = (W.Z[1][0] * W.Z[1][0] + W.Z[1][1] * W.Z[1][1]) + W.Z[1][2] * W.Z[1][2];
+            const bool nz = zz != 0.0;
+            const double theta = m.div(pos1 ? dlo[1] : dhi[1], nz ? zz : 1.0);
+            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
+            const double phi = nz ? mc : 1.0;
+            const double coef = (pos1 ? 0.5 : -0.5) * (1.0 - fabs(s1) * dtdx_ave);
+            const bool on = neg1 || pos1;
+#pragma unroll
+            for (int c = 0; c < 3; c++) { const double t = coef * (phi * W.Z[1][c]); F[c] = F[c] + (on ? t : 0.0); }
+        }
+        {   // family 3: s > 0, upwind neighbour e-1
+            const double zz = (W.Z[2][0] * W.Z[2][0] + W.Z[2][1] * W.Z[2][1]) + W.Z[2][2] * W.Z[2][2];
+            const bool nz = zz != 0.0;
+            const double theta = m.div(dlo[2], nz ? zz : 1.0);
+            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
+            const double phi = nz ? mc : 1.0;
+            const double coef = 0.5 * (1.0 - s2 * dtdx_ave);
+#pragma unroll
+            for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[2][c]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
+}
+
+// eq. 15 for a standard edge (s[0] < 0 < s[2]): the terms max(s0, 0) rdR and max(-s2, 0) rdL are +0
+__device__ __forceinline__ double gc_edge_cfl_std(const Waves &W, double rdL, double rdR)
+{
+    double m = (-W.s[0]) * rdL;
+    m = dmax(m, dmax(W.s[1], 0.0) * rdR);
+    m = dmax(m, dmax(-W.s[1], 0.0) * rdL);
+    m = dmax(m, W.s[2] * rdR);
+    return m;
+}

@@ -21,6 +21,9 @@
 #ifndef MARCH_MINB
 #define MARCH_MINB 3     // resident blocks per SM the register allocation is bounded for
 #endif
+#ifndef MARCH_UNROLL
+#define MARCH_UNROLL 1
+#endif
 #define SW_YW 8       // columns per y-sweep block (8 doubles = 2 full 32-byte sectors per row access)
 
 struct SweepArgs {
@@ -229,6 +232,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
     double q1h = 0.0, q1p = 0.0, q1t = 0.0, q2h = 0.0, q2p = 0.0, q2t = 0.0;   // raw state of cells r-1, r-2
     double rd1 = 0.0, rd2 = 0.0;                                 // 1/(kappa dx) of cells r-1, r-2
     double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
+    bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
 
     double vh[4], vp[4], vt[4], vb[4];                           // x-sweep: the 4 cells of the current 256-bit group
     double nh_ = 0.0, np_ = 0.0, nt_ = 0.0, nb_ = 0.0;           // y-sweep: next row, loaded one step ahead
@@ -236,7 +240,8 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         nh_ = a.h[base]; nb_ = a.b[base]; np_ = a.hv[base]; nt_ = a.hu[base];
     }
 
-#pragma unroll 1
+    constexpr int kMarchUnroll = MARCH_UNROLL;
+#pragma unroll kMarchUnroll
     for (int r = 0; r < nst_warp; r++) {
         const bool live = r < nst;
         double qh, qp, qt, qb;
@@ -268,6 +273,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
 
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
         Waves Wn;
+        bool stdn = false;
         {   // straight-line code for an open-ocean edge first (gc_riemann_fast); any other kind of edge, or a fast-math
             // operand outside its window (gc_math.cuh), redoes this cell + edge with the general code and IEEE operators
             MathFast mf;
@@ -276,6 +282,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
             bool ok = !mf.failed();
             if (r >= 1 && live) ok = gc_riemann_fast(mf, a.g, a.eps, Lst, R, Wn.Z, Wn.s) && ok;
             else gc_waves_zero(Wn);
+            stdn = ok && (r >= 1) && live;
             if (!ok) {
                 MathIeee mi;
                 R = R0;
@@ -290,12 +297,13 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         double dhi[3];
         gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
         double fm[3], fp[3];
-        {
+        {   // edge r-1: a standard edge (s[0] < 0 < s[2], solved by the fast path) needs no sign tests for families 1 and 3
             MathFast mf;
-            gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);       // edge r-1
+            if (stdc) gc_edge_flux_std(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
+            else gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
             if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
         }
-        if (live && r >= 3 && count) cflm = dmax(cflm, gc_edge_cfl(Wc, rd2, rd1));
+        if (live && r >= 3 && count) cflm = dmax(cflm, stdc ? gc_edge_cfl_std(Wc, rd2, rd1) : gc_edge_cfl(Wc, rd2, rd1));
         if (live && r >= 4) {                                                           // cell r-2
             const double dtdx = dt * rd2;
             double uh = q2h - dtdx * (fm[0] - fpp[0]);
@@ -315,7 +323,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         }
 #pragma unroll
         for (int k = 0; k < 3; k++) { fpp[k] = fp[k]; dlo[k] = dhi[k]; }
-        Wc = Wn; Lst = R;
+        Wc = Wn; Lst = R; stdc = stdn;
         q2h = q1h; q2p = q1p; q2t = q1t; q1h = qh; q1p = qp; q1t = qt;
         rd2 = rd1; rd1 = rd0;
     }
