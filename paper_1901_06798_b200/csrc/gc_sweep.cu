@@ -203,6 +203,27 @@ __device__ __forceinline__ void ld4(const double *p, double &x, double &y, doubl
     asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
 }
 
+// x-sweep staging: each thread copies the next 4 cells (32 bytes) of its row, per plane, into its own slots of a
+// two-stage shared-memory buffer with cp.async, one group ahead of their use
+__device__ __forceinline__ void cp16(const double *sdst, const double *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void stage_group(const SweepArgs &a, const double *sb, int64_t o)
+{
+    cp16(sb, a.h + o);                        cp16(sb + 2, a.h + o + 2);
+    cp16(sb + MARCH_BLOCK * 4, a.hu + o);     cp16(sb + MARCH_BLOCK * 4 + 2, a.hu + o + 2);
+    cp16(sb + 2 * MARCH_BLOCK * 4, a.hv + o); cp16(sb + 2 * MARCH_BLOCK * 4 + 2, a.hv + o + 2);
+    cp16(sb + 3 * MARCH_BLOCK * 4, a.b + o);  cp16(sb + 3 * MARCH_BLOCK * 4 + 2, a.b + o + 2);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void lds4(const double *sb, double (&v)[4])
+{
+    const double2 lo = *reinterpret_cast<const double2 *>(sb), hi = *reinterpret_cast<const double2 *>(sb + 2);
+    v[0] = lo.x; v[1] = lo.y; v[2] = hi.x; v[3] = hi.y;
+}
+#define MARCH_STAGE_BYTES (2 * 4 * MARCH_BLOCK * 4 * 8)   // [stage][plane][thread][4 cells] doubles
+
 template <int DIR>
 __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
 {
@@ -234,7 +255,9 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
     double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
     bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
 
-    double vh[4], vp[4], vt[4], vb[4];                           // x-sweep: the 4 cells of the current 256-bit group
+    double vh[4], vp[4], vt[4], vb[4];                           // x-sweep: the 4 cells of the current group
+    extern __shared__ __align__(16) double stage[];              // x-sweep: MARCH_STAGE_BYTES of staging slots
+    if (DIR == 0 && nst > 0) stage_group(a, stage + threadIdx.x * 4, base);
     double nh_ = 0.0, np_ = 0.0, nt_ = 0.0, nb_ = 0.0;           // y-sweep: next row, loaded one step ahead
     if (DIR == 1 && nst > 0) {
         nh_ = a.h[base]; nb_ = a.b[base]; np_ = a.hv[base]; nt_ = a.hu[base];
@@ -247,14 +270,17 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         double qh, qp, qt, qb;
         if (DIR == 0) {
             if ((r & 3) == 0) {
+                // the 4 cells of this group were requested one group ago (cp.async into this thread's own staging slots:
+                // no register is tied up while the request is in flight); read them, then request the next group
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                const double *sb = stage + (size_t)((r >> 2) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4;
                 if (live) {
-                    const int64_t o = base + r;
-                    ld4(a.h + o, vh[0], vh[1], vh[2], vh[3]); ld4(a.hu + o, vp[0], vp[1], vp[2], vp[3]);
-                    ld4(a.hv + o, vt[0], vt[1], vt[2], vt[3]); ld4(a.b + o, vb[0], vb[1], vb[2], vb[3]);
+                    lds4(sb, vh); lds4(sb + MARCH_BLOCK * 4, vp); lds4(sb + 2 * MARCH_BLOCK * 4, vt); lds4(sb + 3 * MARCH_BLOCK * 4, vb);
                 } else {
 #pragma unroll
                     for (int k = 0; k < 4; k++) { vh[k] = 0.0; vp[k] = 0.0; vt[k] = 0.0; vb[k] = 0.0; }
                 }
+                if (r + 4 < nst) stage_group(a, stage + (size_t)(((r >> 2) + 1) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4, base + r + 4);
             }
             qh = vh[0]; qp = vp[0]; qt = vt[0]; qb = vb[0];
 #pragma unroll
@@ -378,7 +404,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     a.oh = L->qs[0]; a.ohu = L->qs[1]; a.ohv = L->qs[2]; a.rd = L->d_rdx;
     if (L->use_march) {
         a.lines = L->d_xl; a.nlines = L->nxl_lines;
-        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_march<0><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, 0, L->ctx->stream>>>(a); }
+        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_march<0><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, MARCH_STAGE_BYTES, L->ctx->stream>>>(a); }
     } else if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
     // y-sweep: Q* -> Q^{n+1}
     a.tiles = L->d_yt; a.h = L->qs[0]; a.hu = L->qs[1]; a.hv = L->qs[2];
