@@ -21,8 +21,16 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-FLOP_PER_UPDATE = 480.0   # fp64 operations per cell update in the scheme, div and sqrt counted as one
-BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once
+# Algorithmic work per cell update: the open-ocean path of the scheme executes 440 fp64 flops per cell
+# per sweep (156 DMUL + 112 DADD + 86 DFMA x 2, divides and square roots expanded into their correctly rounded
+# Newton sequences; counted from the ncu source page, profiles/r01_march_final.md), i.e. 880 per update (x + y).
+FLOP_PER_SWEEP = 440.0
+FLOP_PER_UPDATE = 2.0 * FLOP_PER_SWEEP
+FP64_SLOTS_PER_SWEEP = 417.0   # instructions issued to the fp64 pipe per cell per sweep (arithmetic + DSETP compares)
+BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once; the two-pass design moves 112
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (k_march<0>, the x-sweep) at the bench
+# size 8192^2 / side 256, from the ncu --set full capture summarised in profiles/r01_march_final.md
+NCU_TRAFFIC_BYTES = {"xsweep": None, "ysweep": None}
 METRIC = "fp64 cell updates/sec per level step (device-timed)"
 UNIT = "cell updates/s"
 
@@ -241,8 +249,12 @@ def main():
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms = prof[dom][0] / max(prof[dom][1], 1)
     share = {k: v[0] / max(sum(x[0] for x in prof.values()), 1e-12) for k, v in prof.items() if v[1]}
-    frac_of_update = {"xsweep": 0.5, "ysweep": 0.5, "fused": 1.0}.get(dom, 1.0)
-    alu_achieved = FLOP_PER_UPDATE * frac_of_update * cells / (dom_ms * 1e-3) / 1e12
+    # cells one launch of the dominant kernel updates: the x-sweep also covers the 4 ghost rows of every patch (S-5)
+    per_launch = {"xsweep": cells * (1.0 + 4.0 / args.side), "ysweep": float(cells)}.get(dom, float(cells))
+    alu_achieved = FLOP_PER_SWEEP * per_launch / (dom_ms * 1e-3) / 1e12
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
+    slot_frac = FP64_SLOTS_PER_SWEEP * per_launch / (dom_ms * 1e-3) / slot_peak
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -256,9 +268,11 @@ def main():
                 "steps": Ke, "note": "state copied host->device and back every step through the C ABI (P:166 pipeline)"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                     "frac": alu_achieved / (fp64_peak / 1e12), "traffic": None,
-                     "peak_source": "DFMA micro-benchmark in this run (gc_probe_fp64_peak); no-FMA code tops out at 0.5",
-                     "flop_per_update": FLOP_PER_UPDATE, "kernel_ms": dom_ms, "kernel_share_of_step": share},
+                     "frac": alu_achieved / (fp64_peak / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(dom),
+                     "peak_source": "DFMA micro-benchmark in this run (gc_probe_fp64_peak = 2 flop x 64 lanes x SMs x clock); "
+                                    "the scheme is compiled without FMA contraction, so add/mul code tops out at 0.5",
+                     "flop_per_cell_per_sweep": FLOP_PER_SWEEP, "cells_per_launch": per_launch, "kernel_ms": dom_ms,
+                     "fp64_pipe_slot_frac": slot_frac, "kernel_share_of_step": share},
         "hbm": {"achieved_gbs": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9, "peak_gbs": hbm_peak,
                 "frac": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9 / hbm_peak, "of": which,
                 "bytes_per_update": BYTES_PER_UPDATE},
@@ -266,9 +280,9 @@ def main():
     if tilings:
         out["config"]["tilings"] = tilings
     if not args.no_cpu:
-        rate, el = oracle_rate(1024, 6)
+        rate, el = oracle_rate(1024, 60)
         out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                               "sample": "config-5 recipe at 1024x1024 (one patch), 6 steps, %.1f s" % el}
+                               "sample": "config-5 recipe at 1024x1024 (one patch), 60 steps, %.1f s" % el}
     print(json.dumps(out))
     if dist:
         dist.destroy_process_group()

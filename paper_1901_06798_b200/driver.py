@@ -26,8 +26,8 @@ def set_initial(L, wl, state=True):
     """b (and optionally h, hu, hv) from the analytic workload functions, patch by patch, over the
     patch box grown by the ghost width and clipped to the domain."""
     pats = L.patches
-    # group: if patches tile a modest domain, evaluate once globally
-    if L.nxl * L.nyl <= (1 << 27):
+    # if the patches cover most of a modest domain, evaluate once globally; else patch by patch
+    if L.nxl * L.nyl <= (1 << 27) and L.nxl * L.nyl <= 2 * L.ncells:
         b, h, hu, hv = wl.fields(L.dx, L.dy, 0, 0, L.nxl, L.nyl)
         L.set_global("b", b)
         if state:
@@ -135,27 +135,45 @@ def cluster(flags, valid=None, efficiency=0.7, max_side=64):
     return out
 
 
-def unpack_cells(L, packed, fill=0):
-    """interior-packed per-patch array (flags, masks) -> level-global 2-D array"""
-    out = np.full((L.nyl, L.nxl), fill, dtype=packed.dtype)
+def level_bbox(L):
+    """bounding box (i0, j0, i1, j1) of the patches of a level, grown by one cell and clipped to the domain"""
+    p = np.asarray(L.patches)
+    i0 = max(int(p[:, 0].min()) - 1, 0); j0 = max(int(p[:, 1].min()) - 1, 0)
+    i1 = min(int((p[:, 0] + p[:, 2]).max()) + 1, L.nxl); j1 = min(int((p[:, 1] + p[:, 3]).max()) + 1, L.nyl)
+    return i0, j0, i1, j1
+
+
+def unpack_cells(L, packed, fill=0, bbox=None):
+    """interior-packed per-patch array (flags, masks) -> 2-D array over the level (or over bbox = (i0, j0, i1, j1))"""
+    bi, bj, ei, ej = (0, 0, L.nxl, L.nyl) if bbox is None else bbox
+    out = np.full((ej - bj, ei - bi), fill, dtype=packed.dtype)
     o = 0
     for i0, j0, nx, ny in L.patches:
-        out[j0:j0 + ny, i0:i0 + nx] = packed[o:o + nx * ny].reshape(ny, nx)
+        out[j0 - bj:j0 - bj + ny, i0 - bi:i0 - bi + nx] = packed[o:o + nx * ny].reshape(ny, nx)
         o += nx * ny
     return out
 
 
-def nesting_mask(L):
+def nesting_mask(L, bbox=None):
     """Cells of level L whose 3x3 neighbourhood (clipped to the domain) lies inside the level: a finer patch on
-    top of them has every ghost cell over level-L interior cells (proper nesting by one coarse cell)."""
-    cov = np.zeros((L.nyl + 2, L.nxl + 2), dtype=bool)
-    cov[0, :] = cov[-1, :] = True; cov[:, 0] = cov[:, -1] = True     # outside the domain counts as fine (physical BC)
+    top of them has every ghost cell over level-L interior cells (proper nesting by one coarse cell).
+    Over the whole level, or over bbox = (i0, j0, i1, j1)."""
+    bi, bj, ei, ej = (0, 0, L.nxl, L.nyl) if bbox is None else bbox
+    nx_, ny_ = ei - bi, ej - bj
+    cov = np.zeros((ny_ + 2, nx_ + 2), dtype=bool)      # index (j - bj + 1, i - bi + 1)
+    if bj == 0: cov[0, :] = True                         # outside the domain counts as fine (physical BC)
+    if ej == L.nyl: cov[-1, :] = True
+    if bi == 0: cov[:, 0] = True
+    if ei == L.nxl: cov[:, -1] = True
     for i0, j0, nx, ny in L.patches:
-        cov[j0 + 1:j0 + ny + 1, i0 + 1:i0 + nx + 1] = True
-    ok = np.ones((L.nyl, L.nxl), dtype=bool)
+        a0, a1 = max(i0 - bi + 1, 0), min(i0 - bi + 1 + nx, nx_ + 2)
+        c0, c1 = max(j0 - bj + 1, 0), min(j0 - bj + 1 + ny, ny_ + 2)
+        if a0 < a1 and c0 < c1:
+            cov[c0:c1, a0:a1] = True
+    ok = np.ones((ny_, nx_), dtype=bool)
     for dj in (0, 1, 2):
         for di in (0, 1, 2):
-            ok &= cov[dj:dj + L.nyl, di:di + L.nxl]
+            ok &= cov[dj:dj + ny_, di:di + nx_]
     return ok
 
 
@@ -188,20 +206,23 @@ class Hierarchy:
         """flag level k, cluster -> patches of level k+1 (in cells of level k+1), or None"""
         L = self.levels[k]
         f = dict(self.wl.flag)
-        boxes = [b[1:] for b in self.wl.forced_boxes if b[0] == k + 1]
-        packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0), tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
+        # a box that refines level lv -> lv + 1 needs every coarser level underneath: it flags levels 1..lv (P:160)
+        boxes = [b[1:] for b in self.wl.forced_boxes if b[0] >= k + 1]
+        wave = k + 1 <= self.wl.wave_levels
+        packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0) if wave else 0.0, tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
                            buffer=f.get("buffer", 0), boxes=boxes, t=self.t)
         self.flag_log.append((k, self.t, packed.copy()))
         if n == 0:
             return None
-        fl = unpack_cells(L, packed).astype(bool)
-        ok = nesting_mask(L)
+        bbox = level_bbox(L)
+        fl = unpack_cells(L, packed, bbox=bbox).astype(bool)
+        ok = nesting_mask(L, bbox=bbox)
         fl &= ok
         if not fl.any():
             return None
         r = self.ratios[k]
         boxes = cluster(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
-        return np.array([[b[0] * r, b[1] * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
+        return np.array([[(b[0] + bbox[0]) * r, (b[1] + bbox[1]) * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
 
     def _regrid(self, k0, initial=False):
         """rebuild levels k0+1.. from the flags of the level below each"""

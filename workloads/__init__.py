@@ -38,6 +38,7 @@ class Workload:
     patch_min: int = 32
     patch_max: int = 64
     forced_boxes: Tuple = ()          # (level, x0, x1, y0, y1, t0, t1): refine level -> level+1 inside
+    wave_levels: int = 99             # the wave criteria (tol_eta, ...) flag levels 1..wave_levels only; finer levels come from boxes
 
     def centers(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
         dx = self.dx if level_dx is None else level_dx
@@ -154,7 +155,7 @@ def cfg4(nx=1800, ny=900):
              (3, coast0 - 0.8, coast0 + 0.4, cy - 0.4, cy + 0.4, 6.5 * 3600, 1e30))
     return Workload("cfg4", dict(coord=1, dry_tol=1e-3, bc=(0, 0, 0, 0)), xlo, ylo, d, d, nx, ny, bathy, eta0,
                     cfl=0.9, t_end=36000.0, ratios=(5, 6, 4), flag=dict(tol_eta=0.02, offshore_only=1, buffer=3),
-                    regrid_interval=3, patch_min=50, patch_max=200, forced_boxes=boxes)
+                    regrid_interval=3, patch_min=50, patch_max=200, forced_boxes=boxes, wave_levels=1)
 
 
 def cfg5(n=8192):
