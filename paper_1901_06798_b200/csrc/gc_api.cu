@@ -134,6 +134,15 @@ static void build_tiles(gc_level *L, std::vector<SweepTile> &xt, std::vector<Swe
         const gc_patch &P = L->pat[p];
         // x-sweep: all rows 0..ny+3; whole rows if nx+3 <= B, else balanced chunks of <= B-3 cells
         int nchunk = (P.nx + (B - 3) - 1) / (B - 3);
+        {   // pick the chunking with the most updated cells per thread: R rows of (nc + 3) edges fill a block of B threads
+            int best = 0;
+            for (int m = nchunk; m <= std::max(nchunk, P.nx / 8); m++) {
+                int nc = (P.nx + m - 1) / m, R = B / (nc + 3);
+                if (R < 1) continue;
+                int useful = std::min(R, P.ny + 4) * nc;
+                if (useful > best) { best = useful; nchunk = m; }
+            }
+        }
         for (int c = 0; c < nchunk; c++) {
             int c0 = (int)((int64_t)P.nx * c / nchunk), c1 = (int)((int64_t)P.nx * (c + 1) / nchunk);
             int nc = c1 - c0, R = B / (nc + 3);

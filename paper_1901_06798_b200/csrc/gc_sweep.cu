@@ -73,10 +73,12 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
     const int ce = T.c0 - 1 + e;              // storage index (along the sweep) of the cell right of / above this edge
     const double dt = a.dt_dev ? *a.dt_dev : a.dt;
 
-    double Z[3][3], s[3];
+    Waves W;
+    double (&Z)[3][3] = W.Z; double (&s)[3] = W.s;
     double rdR = 0.0, rdL = 0.0;              // 1/(kappa dx) of the right and the left cell of the edge
     int64_t idx = 0, str = 1;
     double qh = 0.0, qp = 0.0, qt = 0.0;      // state of the right cell (the one this thread updates)
+    bool stdE = false;                        // "standard" edge: solved by the straight-line open-ocean code, s[0] < 0 < s[2]
     if (active) {
         RState L, R;
         if (DIR == 0) { idx = pd.off + (int64_t)line * pd.pitch + ce; str = 1; }
@@ -86,10 +88,19 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
         if (DIR == 0) { L.p = a.hu[idx - str]; L.t = a.hv[idx - str]; R.p = a.hu[idx]; R.t = a.hv[idx]; }
         else          { L.p = a.hv[idx - str]; L.t = a.hu[idx - str]; R.p = a.hv[idx]; R.t = a.hu[idx]; }
         qh = R.h; qp = R.p; qt = R.t;
-        MathIeee mi;
-        gc_prim(mi, L, a.g, a.eps);
-        gc_prim(mi, R, a.g, a.eps);
-        gc_riemann(mi, a.g, a.eps, L, R, Z, s);
+        {   // straight-line code for an open-ocean edge first; any other edge is redone with the general code (same bits)
+            MathFast mf;
+            RState Lf = L, Rf = R;
+            gc_prim_fast(mf, Lf, a.g, a.eps);
+            gc_prim_fast(mf, Rf, a.g, a.eps);
+            stdE = gc_riemann_fast(mf, a.g, a.eps, Lf, Rf, Z, s);
+        }
+        if (!stdE) {
+            MathIeee mi;
+            gc_prim(mi, L, a.g, a.eps);
+            gc_prim(mi, R, a.g, a.eps);
+            gc_riemann(mi, a.g, a.eps, L, R, Z, s);
+        }
         if (DIR == 0) { rdR = a.rd[pd.j0 + line]; rdL = rdR; }
         else          { rdR = a.rd[pd.j0 + ce]; rdL = a.rd[pd.j0 + ce - 1]; }
         if (a.coord == 1) {                   // scale by the edge factor
@@ -98,8 +109,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
             for (int w = 0; w < 3; w++) { s[w] = s[w] * ef; Z[w][0] = Z[w][0] * ef; Z[w][1] = Z[w][1] * ef; Z[w][2] = Z[w][2] * ef; }
         }
     } else {
-#pragma unroll
-        for (int w = 0; w < 3; w++) { s[w] = 0.0; Z[w][0] = 0.0; Z[w][1] = 0.0; Z[w][2] = 0.0; }
+        gc_waves_zero(W);
     }
 #pragma unroll
     for (int w = 0; w < 3; w++) { sZ[3 * w + 0][k] = Z[w][0]; sZ[3 * w + 1][k] = Z[w][1]; sZ[3 * w + 2][k] = Z[w][2]; }
@@ -109,47 +119,18 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
     double fm[3] = {0.0, 0.0, 0.0}, fp[3] = {0.0, 0.0, 0.0};
     double cflm = 0.0;
     if (limited) {
-        double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
+        double zi[3];                                          // Z_I . Z_e with the upwind neighbour I of eq. 11
 #pragma unroll
         for (int w = 0; w < 3; w++) {
-#pragma unroll
-            for (int c = 0; c < 3; c++) {
-                if (s[w] < 0.0) am[c] = am[c] + Z[w][c];
-                else if (s[w] > 0.0) ap[c] = ap[c] + Z[w][c];
-                else { am[c] = am[c] + 0.5 * Z[w][c]; ap[c] = ap[c] + 0.5 * Z[w][c]; }
-            }
+            const int kn = (s[w] > 0.0) ? k - dk : k + dk;
+            zi[w] = (sZ[3 * w + 0][kn] * Z[w][0] + sZ[3 * w + 1][kn] * Z[w][1]) + sZ[3 * w + 2][kn] * Z[w][2];
         }
-        if (a.limiter != 0) {
-            double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
-#pragma unroll
-            for (int w = 0; w < 3; w++) {
-                double sw = s[w];
-                if (sw != 0.0) {
-                    double zz = (Z[w][0] * Z[w][0] + Z[w][1] * Z[w][1]) + Z[w][2] * Z[w][2];
-                    double phi = 1.0;
-                    if (zz != 0.0) {
-                        int kn = (sw > 0.0) ? k - dk : k + dk;                  // eq. 11
-                        double zi = (sZ[3 * w + 0][kn] * Z[w][0] + sZ[3 * w + 1][kn] * Z[w][1]) + sZ[3 * w + 2][kn] * Z[w][2];
-                        double theta = zi / zz;                                 // eq. 10 (S-1)
-                        phi = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));   // MC
-                    }
-                    double coef = ((sw > 0.0) ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
-#pragma unroll
-                    for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * Z[w][c]);        // eq. 9
-                }
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
+        bool done = false;
+        if (stdE) { MathFast mf; gc_edge_flux_std(mf, W, zi, zi, a.limiter, dt, rdL, rdR, fm, fp); done = !mf.failed(); }
+        if (!done) { MathIeee mi; gc_edge_flux(mi, W, zi, zi, a.limiter, dt, rdL, rdR, fm, fp); }
         // eq. 15: right-going waves enter the right cell, left-going the left cell; interior lines only
-        bool count = (DIR == 1) || (line >= 2 && line < pd.ny + 2);
-        if (count) {
-#pragma unroll
-            for (int w = 0; w < 3; w++) {
-                cflm = dmax(cflm, dmax(s[w], 0.0) * rdR);
-                cflm = dmax(cflm, dmax(-s[w], 0.0) * rdL);
-            }
-        }
+        const bool count = (DIR == 1) || (line >= 2 && line < pd.ny + 2);
+        if (count) cflm = stdE ? gc_edge_cfl_std(W, rdL, rdR) : gc_edge_cfl(W, rdL, rdR);
     }
     sF[0][k] = fm[0]; sF[1][k] = fm[1]; sF[2][k] = fm[2];
     __syncthreads();
