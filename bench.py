@@ -21,16 +21,16 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# Algorithmic work per cell update: the open-ocean path of the scheme executes 440 fp64 flops per cell
-# per sweep (156 DMUL + 112 DADD + 86 DFMA x 2, divides and square roots expanded into their correctly rounded
-# Newton sequences; counted from the ncu source page, profiles/r01_march_final.md), i.e. 880 per update (x + y).
-FLOP_PER_SWEEP = 440.0
+# Algorithmic work per cell update: the open-ocean path of the scheme executes 415 fp64 flops per cell
+# per sweep (147 DMUL + 106 DADD + 81 DFMA x 2, divides and square roots expanded into their correctly rounded
+# Newton sequences; counted from the ncu source page, profiles/r01_march_final.md), i.e. 830 per update (x + y).
+FLOP_PER_SWEEP = 415.0
 FLOP_PER_UPDATE = 2.0 * FLOP_PER_SWEEP
-FP64_SLOTS_PER_SWEEP = 417.0   # instructions issued to the fp64 pipe per cell per sweep (arithmetic + DSETP compares)
+FP64_SLOTS_PER_SWEEP = 394.0   # instructions issued to the fp64 pipe per cell per sweep (arithmetic + DSETP compares)
 BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once; the two-pass design moves 112
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (k_march<0>, the x-sweep) at the bench
 # size 8192^2 / side 256, from the ncu --set full capture summarised in profiles/r01_march_final.md
-NCU_TRAFFIC_BYTES = {"xsweep": None, "ysweep": None}
+NCU_TRAFFIC_BYTES = {"xsweep": 5.935e9, "ysweep": 3.922e9}
 METRIC = "fp64 cell updates/sec per level step (device-timed)"
 UNIT = "cell updates/s"
 
