@@ -17,7 +17,9 @@
 #include "gc_scheme.cuh"
 
 #define SW_BLOCK 256
+#ifndef MARCH_BLOCK
 #define MARCH_BLOCK 128
+#endif
 #ifndef MARCH_MINB
 #define MARCH_MINB 3     // resident blocks per SM the register allocation is bounded for
 #endif
@@ -188,7 +190,7 @@ __device__ __forceinline__ void ld4(const double *p, double &x, double &y, doubl
 // two-stage shared-memory buffer with cp.async, one group ahead of their use
 __device__ __forceinline__ void cp16(const double *sdst, const double *gsrc)
 {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void stage_group(const SweepArgs &a, const double *sb, int64_t o)
 {
@@ -197,11 +199,6 @@ __device__ __forceinline__ void stage_group(const SweepArgs &a, const double *sb
     cp16(sb + 2 * MARCH_BLOCK * 4, a.hv + o); cp16(sb + 2 * MARCH_BLOCK * 4 + 2, a.hv + o + 2);
     cp16(sb + 3 * MARCH_BLOCK * 4, a.b + o);  cp16(sb + 3 * MARCH_BLOCK * 4 + 2, a.b + o + 2);
     asm volatile("cp.async.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void lds4(const double *sb, double (&v)[4])
-{
-    const double2 lo = *reinterpret_cast<const double2 *>(sb), hi = *reinterpret_cast<const double2 *>(sb + 2);
-    v[0] = lo.x; v[1] = lo.y; v[2] = hi.x; v[3] = hi.y;
 }
 #define MARCH_STAGE_BYTES (2 * 4 * MARCH_BLOCK * 4 * 8)   // [stage][plane][thread][4 cells] doubles
 
@@ -236,7 +233,6 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
     double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
     bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
 
-    double vh[4], vp[4], vt[4], vb[4];                           // x-sweep: the 4 cells of the current group
     extern __shared__ __align__(16) double stage[];              // x-sweep: MARCH_STAGE_BYTES of staging slots
     if (DIR == 0 && nst > 0) stage_group(a, stage + threadIdx.x * 4, base);
     double nh_ = 0.0, np_ = 0.0, nt_ = 0.0, nb_ = 0.0;           // y-sweep: next row, loaded one step ahead
@@ -250,22 +246,16 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         const bool live = r < nst;
         double qh, qp, qt, qb;
         if (DIR == 0) {
+            // the 4 cells of a group were requested one group ago (cp.async.cg into this thread's own staging slots: no
+            // register is tied up while the request is in flight and nothing is allocated in L1, which the spilled
+            // loop invariants need); each cell is read from its slot when its turn comes
             if ((r & 3) == 0) {
-                // the 4 cells of this group were requested one group ago (cp.async into this thread's own staging slots:
-                // no register is tied up while the request is in flight); read them, then request the next group
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
-                const double *sb = stage + (size_t)((r >> 2) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4;
-                if (live) {
-                    lds4(sb, vh); lds4(sb + MARCH_BLOCK * 4, vp); lds4(sb + 2 * MARCH_BLOCK * 4, vt); lds4(sb + 3 * MARCH_BLOCK * 4, vb);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < 4; k++) { vh[k] = 0.0; vp[k] = 0.0; vt[k] = 0.0; vb[k] = 0.0; }
-                }
                 if (r + 4 < nst) stage_group(a, stage + (size_t)(((r >> 2) + 1) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4, base + r + 4);
             }
-            qh = vh[0]; qp = vp[0]; qt = vt[0]; qb = vb[0];
-#pragma unroll
-            for (int k = 0; k < 3; k++) { vh[k] = vh[k + 1]; vp[k] = vp[k + 1]; vt[k] = vt[k + 1]; vb[k] = vb[k + 1]; }
+            const double *sb = stage + (size_t)((r >> 2) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4 + (r & 3);
+            qh = live ? sb[0] : 0.0; qp = live ? sb[MARCH_BLOCK * 4] : 0.0;
+            qt = live ? sb[2 * MARCH_BLOCK * 4] : 0.0; qb = live ? sb[3 * MARCH_BLOCK * 4] : 0.0;
         } else {
             qh = nh_; qp = np_; qt = nt_; qb = nb_;
             if (r + 1 < nst) {
