@@ -13,6 +13,8 @@
 //    memory, no barriers, each cell's primitive variables computed once, 3 redundant edges per segment only.
 //    The x-sweep reads 4 cells of its row per 256-bit load (rows are 32-byte aligned); the y-sweep reads
 //    one row of 32 adjacent columns per warp (coalesced).  Used for large levels (fp64-pipe bound).
+#include <cstdlib>
+#include <cstring>
 #include "gc_internal.h"
 #include "gc_scheme.cuh"
 
@@ -349,6 +351,263 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
     }
 }
 
+// ---- line-marching sweep, parked state (k_marchp) ---------------------------------------------------------------
+// Same walk and the same arithmetic as k_march, but every value a line carries from one cell to the next and does not
+// need while the Riemann problem of the new edge is being solved -- the waves of the previous edge, the limiter dot
+// products, the pending flux, the raw state of the last two cells -- lives in this thread's own shared-memory slots
+// instead of registers (stored when produced, loaded when used; no rotation moves).  That bounds the kernel at 128
+// registers, so that 4 blocks (16 warps) are resident per SM, without the compiler's local-memory spills.
+// Slots are 16 bytes per thread, slot s of thread t at s * MARCH_BLOCK * 16 + t * 16: conflict-free 128-bit accesses.
+//   0-3 Z00 Z01 | Z02 Z11 | Z12 Z20 | Z21 Z22 (Z10 is +0 by construction)   4 s0 s1   5 s2 dlo0   6 dlo1 dlo2
+//   7 fpp0 fpp1   8 fpp2 -
+// y-sweep: 9-14 ring of the last 3 cells, (h, p) (t, rd) each; 15-18 the next row, 8 bytes per plane and stage (cp.async.ca).
+// x-sweep: 9-20 three stages of 2 cells x 4 planes (one 16-byte cp.async.cg each): the group in flight, the current one and
+//   the previous one, which still holds cell r-2; 21-26 the new values of 4 cells x 3 planes, written to the row with one
+//   256-bit store per plane (a thread's row accesses touch one sector per lane whatever their width, so wide ones are cheap).
+#ifndef PARK_MINB
+#define PARK_MINB 4
+#endif
+#define PK_SL (MARCH_BLOCK * 16u)
+#define PK_RING 9
+#define PK_STAGE 15
+#define PK_XST 9
+#define PK_XOUT 21
+#define PARK_BYTES_X ((PK_XOUT + 6) * PK_SL)
+#define PARK_BYTES_Y ((PK_STAGE + 4) * PK_SL)
+
+__device__ __forceinline__ void sts2(unsigned addr, double x, double y)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" :: "r"(addr), "d"(x), "d"(y));
+}
+__device__ __forceinline__ void lds2(unsigned addr, double &x, double &y)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
+}
+__device__ __forceinline__ double lds1(unsigned addr)
+{
+    double x; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(addr)); return x;
+}
+__device__ __forceinline__ void sts1(unsigned addr, double x)
+{
+    asm volatile("st.shared.f64 [%0], %1;" :: "r"(addr), "d"(x));
+}
+__device__ __forceinline__ void stg4(double *p, double x, double y, double z, double w)
+{
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" :: "l"(p), "d"(x), "d"(y), "d"(z), "d"(w) : "memory");
+}
+__device__ __forceinline__ void stg2(double *p, double x, double y)
+{
+    asm volatile("st.global.v2.f64 [%0], {%1, %2};" :: "l"(p), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void cpa16(unsigned sdst, const double *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sdst), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cpa8(unsigned sdst, const double *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
+}
+
+template <int DIR>
+__global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
+{
+    __shared__ double sred[MARCH_BLOCK / 32];
+    __shared__ unsigned long long sclip[MARCH_BLOCK / 32];
+    __shared__ double sclipm[MARCH_BLOCK / 32];
+    extern __shared__ __align__(16) double dsm[];
+    const unsigned sm0 = (unsigned)__cvta_generic_to_shared(dsm) + threadIdx.x * 16u;
+
+    const int64_t lid = (int64_t)blockIdx.x * MARCH_BLOCK + threadIdx.x;
+    const bool active = lid < a.nlines;
+    LineDesc ln; ln.patch = 0; ln.line = 0; ln.c0 = 2; ln.nc = -4;
+    if (active) { int4 v = *reinterpret_cast<const int4 *>(a.lines + lid); ln.patch = v.x; ln.line = v.y; ln.c0 = v.z; ln.nc = v.w; }
+    const PatchDesc pd = a.pat[ln.patch];
+    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
+    const int nst = ln.nc + 4;                                   // cells read by this line
+    const int nst_warp = __reduce_max_sync(0xffffffffu, nst);
+    const int cfirst = ln.c0 - 2;                                // storage index (along the sweep) of the first cell read
+    int64_t base; int64_t str;
+    if (DIR == 0) { base = pd.off + (int64_t)ln.line * pd.pitch + cfirst; str = 1; }
+    else          { base = pd.off + (int64_t)cfirst * pd.pitch + ln.line; str = pd.pitch; }
+    const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
+    const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
+    const int jrow = pd.j0 + cfirst;                             // y-sweep: global row (+2) of the first cell read
+
+#pragma unroll
+    for (int k = 0; k < PK_RING; k++) sts2(sm0 + k * PK_SL, 0.0, 0.0);
+    RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
+    double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
+    bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
+    unsigned ro0 = PK_RING * PK_SL, ro1 = (PK_RING + 2) * PK_SL, ro2 = (PK_RING + 4) * PK_SL;   // ring slots of cells r, r-1, r-2
+
+    // staging: thread-private slots, filled by cp.async one group (x: 2 cells, y: 1 cell) ahead of their use
+    const unsigned st0 = (DIR == 0) ? sm0 + PK_XST * PK_SL : (unsigned)__cvta_generic_to_shared(dsm) + PK_STAGE * PK_SL + threadIdx.x * 8u;
+    unsigned xprev = 2 * (4 * PK_SL), xcur = 0, xnext = 4 * PK_SL;      // x: stage offsets of groups g-1, g, g+1
+    if (nst > 0) {
+        if (DIR == 0) { cpa16(st0, a.h + base); cpa16(st0 + PK_SL, a.hu + base); cpa16(st0 + 2 * PK_SL, a.hv + base); cpa16(st0 + 3 * PK_SL, a.b + base); }
+        else          { cpa8(st0, a.h + base); cpa8(st0 + PK_SL / 2, a.hv + base); cpa8(st0 + 2 * (PK_SL / 2), a.hu + base); cpa8(st0 + 3 * (PK_SL / 2), a.b + base); }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+
+    for (int r = 0; r < nst_warp; r++) {
+        const bool live = r < nst;
+        double qh, qp, qt, qb;
+        if (DIR == 0) {
+            if ((r & 1) == 0) {
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                if (r > 0) { const unsigned t = xprev; xprev = xcur; xcur = xnext; xnext = t; }
+                if (r + 2 < nst) {
+                    const unsigned sd = st0 + xnext;
+                    const int64_t o = base + r + 2;
+                    cpa16(sd, a.h + o); cpa16(sd + PK_SL, a.hu + o); cpa16(sd + 2 * PK_SL, a.hv + o); cpa16(sd + 3 * PK_SL, a.b + o);
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+            }
+            const unsigned sa = st0 + xcur + (r & 1) * 8u;
+            qh = lds1(sa); qp = lds1(sa + PK_SL); qt = lds1(sa + 2 * PK_SL); qb = lds1(sa + 3 * PK_SL);
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            if (r + 1 < nst) {
+                const unsigned sd = st0 + ((r + 1) & 1) * (4 * (PK_SL / 2));
+                const int64_t o = base + (int64_t)(r + 1) * str;
+                cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            const unsigned sa = st0 + (r & 1) * (4 * (PK_SL / 2));
+            qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
+        }
+        if (!live) { qh = 0.0; qp = 0.0; qt = 0.0; qb = 0.0; }
+        double rd0, ef;
+        if (DIR == 0) { rd0 = rdrow; ef = a.ex; }
+        else          { rd0 = live ? a.rd[jrow + r] : 0.0; ef = live ? a.ey[jrow + r] : 1.0; }
+        if (DIR == 1) { sts2(sm0 + ro0, qh, qp); sts2(sm0 + ro0 + PK_SL, qt, rd0); }
+
+        RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
+        Waves Wn;
+        bool stdn = false;
+        {   // straight-line code for an open-ocean edge first; any other kind of edge, or a fast-math operand outside its
+            // window, redoes this cell + edge with the general code and IEEE operators (same bits)
+            MathFast mf;
+            const RState R0 = R;
+            gc_prim_fast(mf, R, a.g, a.eps);
+            bool ok = !mf.failed();
+            if (r >= 1 && live) ok = gc_riemann_fast(mf, a.g, a.eps, Lst, R, Wn.Z, Wn.s) && ok;
+            else gc_waves_zero(Wn);
+            stdn = ok && (r >= 1) && live;
+            if (!ok) {
+                MathIeee mi;
+                R = R0;
+                gc_prim(mi, R, a.g, a.eps);
+                if (r >= 1 && live) gc_riemann(mi, a.g, a.eps, Lst, R, Wn.Z, Wn.s);
+            }
+            if (a.coord == 1) {                                   // scale by the edge factor
+#pragma unroll
+                for (int w = 0; w < 3; w++) { Wn.s[w] = Wn.s[w] * ef; Wn.Z[w][0] = Wn.Z[w][0] * ef; Wn.Z[w][1] = Wn.Z[w][1] * ef; Wn.Z[w][2] = Wn.Z[w][2] * ef; }
+            }
+        }
+        Lst = R;
+
+        // waves of edge r-1 and its lower dot products come back from their slots; those of edge r take their place
+        Waves Wc; double dlo[3], dhi[3];
+        lds2(sm0, Wc.Z[0][0], Wc.Z[0][1]); lds2(sm0 + PK_SL, Wc.Z[0][2], Wc.Z[1][1]); lds2(sm0 + 2 * PK_SL, Wc.Z[1][2], Wc.Z[2][0]);
+        lds2(sm0 + 3 * PK_SL, Wc.Z[2][1], Wc.Z[2][2]); lds2(sm0 + 4 * PK_SL, Wc.s[0], Wc.s[1]); lds2(sm0 + 5 * PK_SL, Wc.s[2], dlo[0]);
+        lds2(sm0 + 6 * PK_SL, dlo[1], dlo[2]);
+        Wc.Z[1][0] = 0.0;
+        gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
+        sts2(sm0, Wn.Z[0][0], Wn.Z[0][1]); sts2(sm0 + PK_SL, Wn.Z[0][2], Wn.Z[1][1]); sts2(sm0 + 2 * PK_SL, Wn.Z[1][2], Wn.Z[2][0]);
+        sts2(sm0 + 3 * PK_SL, Wn.Z[2][1], Wn.Z[2][2]); sts2(sm0 + 4 * PK_SL, Wn.s[0], Wn.s[1]); sts2(sm0 + 5 * PK_SL, Wn.s[2], dhi[0]);
+        sts2(sm0 + 6 * PK_SL, dhi[1], dhi[2]);
+
+        double q2h, q2p, q2t, rd2, rd1;
+        if (DIR == 0) {
+            const unsigned sq = st0 + xprev + (r & 1) * 8u;                             // cell r-2 is in the previous group
+            q2h = lds1(sq); q2p = lds1(sq + PK_SL); q2t = lds1(sq + 2 * PK_SL); rd2 = rdrow; rd1 = rdrow;
+        } else {
+            lds2(sm0 + ro2, q2h, q2p); lds2(sm0 + ro2 + PK_SL, q2t, rd2);
+            rd1 = lds1(sm0 + ro1 + PK_SL + 8u);
+        }
+        double fm[3], fp[3];
+        {   // edge r-1: a standard edge (s[0] < 0 < s[2], solved by the fast path) needs no sign tests for families 1 and 3
+            MathFast mf;
+            if (stdc) gc_edge_flux_std(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
+            else gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
+            if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
+        }
+        if (live && r >= 3 && count) cflm = dmax(cflm, stdc ? gc_edge_cfl_std(Wc, rd2, rd1) : gc_edge_cfl(Wc, rd2, rd1));
+        double fpp[3], unused_;
+        lds2(sm0 + 7 * PK_SL, fpp[0], fpp[1]); lds2(sm0 + 8 * PK_SL, fpp[2], unused_);
+        sts2(sm0 + 7 * PK_SL, fp[0], fp[1]); sts2(sm0 + 8 * PK_SL, fp[2], 0.0);
+        if (live && r >= 4) {                                                           // cell r-2
+            const double dtdx = dt * rd2;
+            double uh = q2h - dtdx * (fm[0] - fpp[0]);
+            double up = q2p - dtdx * (fm[1] - fpp[1]);
+            double ut = q2t - dtdx * (fm[2] - fpp[2]);
+            const int64_t o = base + (int64_t)(r - 2) * str;
+            if (DIR == 0) {
+                // cell j = r-2 of the row goes to slot (plane, (j >> 1) & 1); a full aligned group of 4 leaves as one store
+                const int j = r - 2;
+                const unsigned so = sm0 + (PK_XOUT + ((j >> 1) & 1)) * PK_SL + (j & 1) * 8u;
+                sts1(so, uh); sts1(so + 2 * PK_SL, up); sts1(so + 4 * PK_SL, ut);
+                if ((j & 3) == 3) {
+                    const unsigned sf = sm0 + PK_XOUT * PK_SL;
+                    double x0, x1, x2, x3;
+                    if (j == 3) {                                                        // cells 0, 1 of the first group are not ours
+                        lds2(sf + PK_SL, x2, x3); stg2(a.oh + o - 1, x2, x3);
+                        lds2(sf + 3 * PK_SL, x2, x3); stg2(a.ohu + o - 1, x2, x3);
+                        lds2(sf + 5 * PK_SL, x2, x3); stg2(a.ohv + o - 1, x2, x3);
+                    } else {
+                        lds2(sf, x0, x1); lds2(sf + PK_SL, x2, x3); stg4(a.oh + o - 3, x0, x1, x2, x3);
+                        lds2(sf + 2 * PK_SL, x0, x1); lds2(sf + 3 * PK_SL, x2, x3); stg4(a.ohu + o - 3, x0, x1, x2, x3);
+                        lds2(sf + 4 * PK_SL, x0, x1); lds2(sf + 5 * PK_SL, x2, x3); stg4(a.ohv + o - 3, x0, x1, x2, x3);
+                    }
+                }
+            } else {
+                if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
+                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[jrow + r - 2] * a.dxdy); }
+                    uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
+                }
+                if (uh != uh || up != up || ut != ut) nanf = 1;
+                if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
+            }
+        }
+        stdc = stdn;
+        { const unsigned t = ro2; ro2 = ro1; ro1 = ro0; ro0 = t; }
+    }
+
+    if (DIR == 0 && nst >= 5) {                                  // x-sweep: the cells of the last, incomplete group
+        const int jl = nst - 3;
+        if ((jl & 3) != 3) {
+            for (int j = (jl & ~3) < 2 ? 2 : (jl & ~3); j <= jl; j++) {
+                const unsigned so = sm0 + (PK_XOUT + ((j >> 1) & 1)) * PK_SL + (j & 1) * 8u;
+                a.oh[base + j] = lds1(so); a.ohu[base + j] = lds1(so + 2 * PK_SL); a.ohv[base + j] = lds1(so + 4 * PK_SL);
+            }
+        }
+    }
+
+    cflm = warp_max(cflm);
+    if (DIR == 1) {
+        nclip = __reduce_add_sync(0xffffffffu, nclip);
+        nanf = __any_sync(0xffffffffu, nanf);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) clipm += __shfl_xor_sync(0xffffffffu, clipm, o);
+    }
+    const int k = threadIdx.x;
+    if ((k & 31) == 0) { sred[k >> 5] = cflm; if (DIR == 1) { sclip[k >> 5] = nclip; sclipm[k >> 5] = clipm; if (nanf) a.stats->nan_seen = 1; } }
+    __syncthreads();
+    if (k == 0) {
+        double m = sred[0];
+#pragma unroll
+        for (int w = 1; w < MARCH_BLOCK / 32; w++) m = dmax(m, sred[w]);
+        if (m > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(m));
+        if (DIR == 1) {
+            unsigned long long n = 0; double cm = 0.0;
+#pragma unroll
+            for (int w = 0; w < MARCH_BLOCK / 32; w++) { n += sclip[w]; cm += sclipm[w]; }
+            if (n) { atomicAdd(&a.stats->nclip, n); atomicAdd(&a.stats->clipped, cm); }
+        }
+    }
+}
+
 __global__ void k_stats_reset(DevStats *s) { s->sdx_bits = 0ull; s->nclip = 0ull; s->clipped = 0.0; s->nan_seen = 0; }
 
 __global__ void k_next_dt(const DevStats *s, double *dt_dev, double cfl)
@@ -360,6 +619,18 @@ __global__ void k_next_dt(const DevStats *s, double *dt_dev, double cfl)
 void gc_launch_stats_reset(gc_level *L) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_stats_reset<<<1, 1, 0, L->ctx->stream>>>(L->d_stats); }
 
 void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_next_dt<<<1, 1, 0, L->ctx->stream>>>(L->d_stats, dt_dev, cfl); }
+
+// GC_MARCH=regs selects the register-resident marching kernels (k_march); default: parked state (k_marchp)
+static bool march_parked()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char *e = getenv("GC_MARCH"); v = (e && !strcmp(e, "regs")) ? 0 : 1;
+        cudaFuncSetAttribute(k_marchp<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_X);
+        cudaFuncSetAttribute(k_marchp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_Y);
+    }
+    return v != 0;
+}
 
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out)
 {
@@ -375,14 +646,24 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     a.oh = L->qs[0]; a.ohu = L->qs[1]; a.ohv = L->qs[2]; a.rd = L->d_rdx;
     if (L->use_march) {
         a.lines = L->d_xl; a.nlines = L->nxl_lines;
-        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_march<0><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, MARCH_STAGE_BYTES, L->ctx->stream>>>(a); }
+        if (a.nlines > 0) {
+            ProfScope ps(L->ctx, GC_SLOT_XSWEEP);
+            const unsigned nb = (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK);
+            if (march_parked()) k_marchp<0><<<nb, MARCH_BLOCK, PARK_BYTES_X, L->ctx->stream>>>(a);
+            else k_march<0><<<nb, MARCH_BLOCK, MARCH_STAGE_BYTES, L->ctx->stream>>>(a);
+        }
     } else if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
     // y-sweep: Q* -> Q^{n+1}
     a.tiles = L->d_yt; a.h = L->qs[0]; a.hu = L->qs[1]; a.hv = L->qs[2];
     a.oh = L->q[nxt][0]; a.ohu = L->q[nxt][1]; a.ohv = L->q[nxt][2]; a.rd = L->d_rdy;
     if (L->use_march) {
         a.lines = L->d_yl; a.nlines = L->nyl_lines;
-        if (a.nlines > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_march<1><<<(unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK), MARCH_BLOCK, 0, L->ctx->stream>>>(a); }
+        if (a.nlines > 0) {
+            ProfScope ps(L->ctx, GC_SLOT_YSWEEP);
+            const unsigned nb = (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK);
+            if (march_parked()) k_marchp<1><<<nb, MARCH_BLOCK, PARK_BYTES_Y, L->ctx->stream>>>(a);
+            else k_march<1><<<nb, MARCH_BLOCK, 0, L->ctx->stream>>>(a);
+        }
     } else if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
 }
 
