@@ -21,16 +21,17 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# Algorithmic work per cell update: the open-ocean path of the scheme executes 415 fp64 flops per cell
-# per sweep (147 DMUL + 106 DADD + 81 DFMA x 2, divides and square roots expanded into their correctly rounded
-# Newton sequences; counted from the ncu source page, profiles/r01_march_final.md), i.e. 830 per update (x + y).
-FLOP_PER_SWEEP = 415.0
-FLOP_PER_UPDATE = 2.0 * FLOP_PER_SWEEP
-FP64_SLOTS_PER_SWEEP = 394.0   # instructions issued to the fp64 pipe per cell per sweep (arithmetic + DSETP compares)
+# Algorithmic work per cell per sweep, counted per kernel from the ncu source page of the default marching
+# kernels k_marchp<0> (x-sweep) / k_marchp<1> (y-sweep), profiles/r01_marchp.md: thread instructions / cells of one launch.
+#   x-sweep: 140.7 DMUL + 103.7 DADD + 81.2 DFMA (x 2 flops) = 407 flops, + 60.5 DSETP = 386 fp64-pipe instructions
+#   y-sweep: 143.9 DMUL + 104.8 DADD + 81.2 DFMA (x 2 flops) = 411 flops, + 64.6 DSETP = 394 fp64-pipe instructions
+# (divides and square roots expanded into their correctly rounded Newton sequences; no FMA contraction elsewhere)
+FLOP_PER_SWEEP = {"xsweep": 407.0, "ysweep": 411.0}
+FP64_SLOTS_PER_SWEEP = {"xsweep": 386.0, "ysweep": 394.0}
 BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once; the two-pass design moves 112
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (k_march<0>, the x-sweep) at the bench
-# size 8192^2 / side 256, from the ncu --set full capture summarised in profiles/r01_march_final.md
-NCU_TRAFFIC_BYTES = {"xsweep": 5.935e9, "ysweep": 3.922e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of each sweep kernel at the bench size 8192^2 / side 256, from the
+# ncu --set full capture summarised in profiles/r01_marchp.md (k_marchp; not valid for GC_MARCH=regs or GC_SWEEP=edge)
+NCU_TRAFFIC_BYTES = {"xsweep": 4.376e9, "ysweep": 3.907e9}
 METRIC = "fp64 cell updates/sec per level step (device-timed)"
 UNIT = "cell updates/s"
 
@@ -251,10 +252,12 @@ def main():
     share = {k: v[0] / max(sum(x[0] for x in prof.values()), 1e-12) for k, v in prof.items() if v[1]}
     # cells one launch of the dominant kernel updates: the x-sweep also covers the 4 ghost rows of every patch (S-5)
     per_launch = {"xsweep": cells * (1.0 + 4.0 / args.side), "ysweep": float(cells)}.get(dom, float(cells))
-    alu_achieved = FLOP_PER_SWEEP * per_launch / (dom_ms * 1e-3) / 1e12
+    flop_sweep = FLOP_PER_SWEEP.get(dom, 411.0)
+    alu_achieved = flop_sweep * per_launch / (dom_ms * 1e-3) / 1e12
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
-    slot_frac = FP64_SLOTS_PER_SWEEP * per_launch / (dom_ms * 1e-3) / slot_peak
+    slot_frac = FP64_SLOTS_PER_SWEEP.get(dom, 394.0) * per_launch / (dom_ms * 1e-3) / slot_peak
+    default_kernels = os.environ.get("GC_MARCH") != "regs" and os.environ.get("GC_SWEEP") != "edge"
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -268,10 +271,10 @@ def main():
                 "steps": Ke, "note": "state copied host->device and back every step through the C ABI (P:166 pipeline)"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                     "frac": alu_achieved / (fp64_peak / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(dom),
+                     "frac": alu_achieved / (fp64_peak / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(dom) if default_kernels else None,
                      "peak_source": "DFMA micro-benchmark in this run (gc_probe_fp64_peak = 2 flop x 64 lanes x SMs x clock); "
                                     "the scheme is compiled without FMA contraction, so add/mul code tops out at 0.5",
-                     "flop_per_cell_per_sweep": FLOP_PER_SWEEP, "cells_per_launch": per_launch, "kernel_ms": dom_ms,
+                     "flop_per_cell_per_sweep": flop_sweep, "cells_per_launch": per_launch, "kernel_ms": dom_ms,
                      "fp64_pipe_slot_frac": slot_frac, "kernel_share_of_step": share},
         "hbm": {"achieved_gbs": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9, "peak_gbs": hbm_peak,
                 "frac": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9 / hbm_peak, "of": which,
