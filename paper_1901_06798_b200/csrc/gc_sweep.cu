@@ -620,16 +620,18 @@ void gc_launch_stats_reset(gc_level *L) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_
 
 void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_next_dt<<<1, 1, 0, L->ctx->stream>>>(L->d_stats, dt_dev, cfl); }
 
-// GC_MARCH=regs selects the register-resident marching kernels (k_march); default: parked state (k_marchp)
+// GC_MARCH=regs selects the register-resident marching kernels (k_march); default: parked state (k_marchp).
+// Read at every launch (a getenv, no device work), so that one process can run both.
 static bool march_parked()
 {
-    static int v = -1;
-    if (v < 0) {
-        const char *e = getenv("GC_MARCH"); v = (e && !strcmp(e, "regs")) ? 0 : 1;
+    static bool attr_done = false;
+    if (!attr_done) {
         cudaFuncSetAttribute(k_marchp<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_X);
         cudaFuncSetAttribute(k_marchp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_Y);
+        attr_done = true;
     }
-    return v != 0;
+    const char *e = getenv("GC_MARCH");
+    return !(e && !strcmp(e, "regs"));
 }
 
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out)

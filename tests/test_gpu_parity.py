@@ -13,11 +13,16 @@ pytestmark = pytest.mark.gpu
 G = 9.81
 
 
-@pytest.fixture(autouse=True, params=["edge", "march"])
+@pytest.fixture(autouse=True, params=["edge", "march", "march-regs"])
 def sweep_mode(request, monkeypatch):
-    """Both sweep kernel families (edge-parallel tiles / line-marching, DESIGN.md 5) must give the oracle's bits;
-    the library picks one by level size unless GC_SWEEP says otherwise."""
-    monkeypatch.setenv("GC_SWEEP", request.param)
+    """Every sweep kernel family (edge-parallel tiles k_sweep / line-marching with parked state k_marchp / line-marching
+    with the state in registers k_march) must give the oracle's bits; the library picks one by level size
+    unless GC_SWEEP / GC_MARCH say otherwise (both are read when a level is created / a sweep is launched)."""
+    monkeypatch.setenv("GC_SWEEP", "edge" if request.param == "edge" else "march")
+    if request.param == "march-regs":
+        monkeypatch.setenv("GC_MARCH", "regs")
+    else:
+        monkeypatch.delenv("GC_MARCH", raising=False)
     return request.param
 
 
@@ -99,6 +104,11 @@ def test_tilings_match_single_patch_oracle(gc, gco, bc):
         np.array([[0, 0, 20, 48], [20, 0, 28, 10], [20, 10, 28, 38]], dtype=np.int32),
         workloads.tile(n, n, 2),
         workloads.tile(n, n, 6),
+        # columns 2, 3, 5 and 38 cells wide (rows 5, 43 high; 2 is the narrowest patch gc_level_create accepts): the
+        # x-sweep's 4-cell output groups with only a head (2), a one-cell tail (3), a three-cell tail (5), and 38 cut into
+        # segments of 12, 16, 10 cells (two-cell tails, and no tail)
+        np.array([[0, 0, 2, 5], [2, 0, 3, 5], [5, 0, 5, 5], [10, 0, 38, 5],
+                  [0, 5, 2, 43], [2, 5, 3, 43], [5, 5, 5, 43], [10, 5, 38, 43]], dtype=np.int32),
     ]
     for pats in tilings:
         Lg, Lo = both(gc, gco, wl, patches_g=pats)
