@@ -27,20 +27,24 @@ def set_initial(L, wl, state=True):
     patch box grown by the ghost width and clipped to the domain."""
     pats = L.patches
     # if the patches cover most of a modest domain, evaluate once globally; else patch by patch
+    # (the bathymetry comes from the workload's tile cache either way; the initial state only when asked for)
     if L.nxl * L.nyl <= (1 << 27) and L.nxl * L.nyl <= 2 * L.ncells:
-        b, h, hu, hv = wl.fields(L.dx, L.dy, 0, 0, L.nxl, L.nyl)
-        L.set_global("b", b)
         if state:
-            L.set_global("h", h); L.set_global("hu", hu); L.set_global("hv", hv)
+            b, h, hu, hv = wl.fields(L.dx, L.dy, 0, 0, L.nxl, L.nyl)
+            L.set_global("b", b); L.set_global("h", h); L.set_global("hu", hu); L.set_global("hv", hv)
+        else:
+            L.set_global("b", wl.bathy_box(L.dx, L.dy, 0, 0, L.nxl, L.nyl))
     else:
         for p in range(len(pats)):
             i0, j0, nx, ny = (int(v) for v in pats[p])
             a0, a1 = max(i0 - 2, 0), min(i0 + nx + 2, L.nxl)
             c0, c1 = max(j0 - 2, 0), min(j0 + ny + 2, L.nyl)
-            b, h, hu, hv = wl.fields(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0)
-            L.set_global("b", b, a0, c0)
             if state:
+                b, h, hu, hv = wl.fields(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0)
+                L.set_global("b", b, a0, c0)
                 L.set_global("h", h, a0, c0); L.set_global("hu", hu, a0, c0); L.set_global("hv", hv, a0, c0)
+            else:
+                L.set_global("b", wl.bathy_box(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0), a0, c0)
     L.fill_ghost_b()
 
 
@@ -208,7 +212,11 @@ class Hierarchy:
         f = dict(self.wl.flag)
         # a box that refines level lv -> lv + 1 needs every coarser level underneath: it flags levels 1..lv
         boxes = [b[1:] for b in self.wl.forced_boxes if b[0] >= k + 1]
-        wave = k + 1 <= self.wl.wave_levels
+        wave = k + 1 <= self.wl.wave_levels and f.get("tol_eta", 0.0) > 0.0
+        # nothing can flag this level now (no wave criterion here, no box whose window [t0, t1] holds t -- the test the
+        # flag kernel applies): the pass would return no flags, so it is not launched and nothing is downloaded
+        if not wave and not any(b[4] <= self.t <= b[5] for b in boxes):
+            return None
         packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0) if wave else 0.0, tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
                            buffer=f.get("buffer", 0), boxes=boxes, t=self.t)
         self.flag_log.append((k, self.t, packed.copy()))

@@ -39,6 +39,7 @@ class Workload:
     patch_max: int = 64
     forced_boxes: Tuple = ()          # (level, x0, x1, y0, y1, t0, t1): refine level -> level+1 inside
     wave_levels: int = 99             # the wave criteria (tol_eta, ...) flag levels 1..wave_levels only; finer levels come from boxes
+    _tiles: dict = field(default_factory=dict, repr=False, compare=False)   # bathy_box cache
 
     def centers(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
         dx = self.dx if level_dx is None else level_dx
@@ -49,10 +50,39 @@ class Workload:
         y = self.ylo + (np.arange(j0, j0 + ny, dtype=np.float64) + 0.5) * dy
         return np.meshgrid(x, y)
 
+    TILE = 256                        # bathy_box: cells per tile side
+    TILE_CACHE_BYTES = 6 << 30        # the cache is dropped when it grows past this
+
+    def bathy_box(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
+        """b at the cell centres of the box [i0,i0+nx) x [j0,j0+ny) of a level with the given cell size.
+        The bathymetry is static, so it is evaluated once per cell and level -- in tiles of TILE x TILE cells aligned to
+        the level's global cell indices, kept for the life of the workload -- the way a topography file is read once;
+        a regrid that re-refines a region already seen costs a copy.  A cell's value does not depend on which box asks."""
+        dx = self.dx if level_dx is None else level_dx
+        dy = self.dy if level_dy is None else level_dy
+        nx = self.nx if nx is None else nx
+        ny = self.ny if ny is None else ny
+        T = self.TILE
+        out = np.empty((ny, nx), dtype=np.float64)
+        for tj in range(j0 // T, (j0 + ny - 1) // T + 1):
+            for ti in range(i0 // T, (i0 + nx - 1) // T + 1):
+                key = (id(self.bathy), dx, dy, ti, tj)
+                tile = self._tiles.get(key)
+                if tile is None:
+                    if sum(t.nbytes for t in self._tiles.values()) > self.TILE_CACHE_BYTES:
+                        self._tiles.clear()
+                    X, Y = self.centers(dx, dy, ti * T, tj * T, T, T)
+                    tile = np.ascontiguousarray(self.bathy(X, Y), dtype=np.float64)
+                    self._tiles[key] = tile
+                a0, a1 = max(i0, ti * T), min(i0 + nx, (ti + 1) * T)
+                c0, c1 = max(j0, tj * T), min(j0 + ny, (tj + 1) * T)
+                out[c0 - j0:c1 - j0, a0 - i0:a1 - i0] = tile[c0 - tj * T:c1 - tj * T, a0 - ti * T:a1 - ti * T]
+        return out
+
     def fields(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
         """b, h, hu, hv at cell centres of the box [i0,i0+nx) x [j0,j0+ny) of a level with the given cell size."""
         X, Y = self.centers(level_dx, level_dy, i0, j0, nx, ny)
-        b = np.asarray(self.bathy(X, Y), dtype=np.float64)
+        b = self.bathy_box(level_dx, level_dy, i0, j0, nx, ny)
         eta = np.asarray(self.eta0(X, Y), dtype=np.float64)
         h = np.maximum(0.0, eta - b)
         z = np.zeros_like(h)
