@@ -37,6 +37,23 @@ void gc_dev_free(gc_ctx *c, void *p)
     if (c->free_) c->free_(p, c->user); else if (!c->alloc) cudaFree(p);
 }
 
+#define GC_STAGE_KEEP_MAX ((size_t)64 << 20)
+void *gc_stage_get(gc_ctx *c, size_t bytes, bool *transient)
+{
+    *transient = bytes > GC_STAGE_KEEP_MAX;
+    if (*transient) return gc_dev_alloc(c, bytes);
+    if (bytes > c->stage_bytes) {
+        // every host-pointer call ends with a stream synchronisation, so nothing queued still uses the old buffer
+        if (c->stage) { cudaStreamSynchronize(c->stream); gc_dev_free(c, c->stage); c->stage = nullptr; c->stage_bytes = 0; }
+        size_t cap = (size_t)1 << 20;
+        while (cap < bytes) cap <<= 1;
+        c->stage = gc_dev_alloc(c, cap);
+        if (!c->stage) return nullptr;
+        c->stage_bytes = cap;
+    }
+    return c->stage;
+}
+
 extern "C" const char *gc_last_error(const gc_ctx *c) { return c ? c->err.c_str() : "null context"; }
 
 extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc, gc_free_fn free_, void *user, gc_ctx **out)
@@ -50,7 +67,12 @@ extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc
     *out = c;
     return GC_OK;
 }
-extern "C" int gc_ctx_destroy(gc_ctx *c) { delete c; return GC_OK; }
+extern "C" int gc_ctx_destroy(gc_ctx *c)
+{
+    if (c && c->stage) { cudaStreamSynchronize(c->stream); gc_dev_free(c, c->stage); }
+    delete c;
+    return GC_OK;
+}
 
 extern "C" int64_t gc_launch_count(const gc_ctx *c) { return c ? (int64_t)c->launches : 0; }
 extern "C" int gc_profile_enable(gc_ctx *c, int on) { if (!c) return GC_ERR_BADARG; c->prof = on != 0; return GC_OK; }
@@ -379,15 +401,15 @@ extern "C" int gc_level_set_global(gc_level *L, int field, const double *src, in
 {
     if (!L || field < 0 || field > 3 || !src || gnx < 1 || gny < 1 || ld < gnx) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_set_global: bad argument");
     gc_ctx *c = L->ctx;
-    const double *dsrc = src; int64_t dld = ld; double *tmp = nullptr;
+    const double *dsrc = src; int64_t dld = ld; double *tmp = nullptr; bool transient = false;
     if (!is_device) {
-        tmp = (double *)gc_dev_alloc(c, (size_t)gnx * gny * 8);
+        tmp = (double *)gc_stage_get(c, (size_t)gnx * gny * 8, &transient);
         if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_level_set_global: staging allocation failed");
         cudaMemcpy2DAsync(tmp, (size_t)gnx * 8, src, (size_t)ld * 8, (size_t)gnx * 8, gny, cudaMemcpyHostToDevice, c->stream);
         dsrc = tmp; dld = gnx;
     }
     gc_launch_set_global(L, plane_of(L, field, GC_NEW), dsrc, dld, gi0, gj0, gnx, gny);
-    if (tmp) { cudaStreamSynchronize(c->stream); gc_dev_free(c, tmp); }
+    if (tmp) { cudaStreamSynchronize(c->stream); if (transient) gc_dev_free(c, tmp); }   // the caller's array is free on return
     return gc_cuda_check(c, "gc_level_set_global");
 }
 
@@ -396,9 +418,9 @@ extern "C" int gc_level_get_global(const gc_level *L, int field, int which, doub
 {
     if (!L || field < 0 || field > 3 || !dst || gnx < 1 || gny < 1 || ld < gnx) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_get_global: bad argument");
     gc_ctx *c = L->ctx;
-    double *ddst = dst; int64_t dld = ld; double *tmp = nullptr;
+    double *ddst = dst; int64_t dld = ld; double *tmp = nullptr; bool transient = false;
     if (!is_device) {
-        tmp = (double *)gc_dev_alloc(c, (size_t)gnx * gny * 8);
+        tmp = (double *)gc_stage_get(c, (size_t)gnx * gny * 8, &transient);
         if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_level_get_global: staging allocation failed");
         // cells not covered by a patch keep the caller's values
         cudaMemcpy2DAsync(tmp, (size_t)gnx * 8, dst, (size_t)ld * 8, (size_t)gnx * 8, gny, cudaMemcpyHostToDevice, c->stream);
@@ -408,7 +430,7 @@ extern "C" int gc_level_get_global(const gc_level *L, int field, int which, doub
     if (tmp) {
         cudaMemcpy2DAsync(dst, (size_t)ld * 8, tmp, (size_t)gnx * 8, (size_t)gnx * 8, gny, cudaMemcpyDeviceToHost, c->stream);
         cudaStreamSynchronize(c->stream);
-        gc_dev_free(c, tmp);
+        if (transient) gc_dev_free(c, tmp);
     }
     return gc_cuda_check(c, "gc_level_get_global");
 }

@@ -86,6 +86,7 @@ struct gc_ctx {
     void *user;
     std::string err;
     bool prof = false;
+    void *stage = nullptr; size_t stage_bytes = 0;   // grow-only device staging buffer of the host-pointer paths (gc_stage_get)
     unsigned long long launches = 0;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];
 };
@@ -144,6 +145,9 @@ struct gc_level {
 // ---- helpers (gc_api.cu)
 void *gc_dev_alloc(gc_ctx *c, size_t bytes);
 void gc_dev_free(gc_ctx *c, void *p);
+// device staging for a host-pointer transfer: the context's retained buffer when the request is small (no allocator
+// callback per call), a transient allocation otherwise (*transient = true: release with gc_dev_free after a stream sync)
+void *gc_stage_get(gc_ctx *c, size_t bytes, bool *transient);
 int gc_fail(gc_ctx *c, int code, const char *msg);
 int gc_cuda_check(gc_ctx *c, const char *what);
 int gc_find_patch_host(const gc_level *L, int64_t gi, int64_t gj);

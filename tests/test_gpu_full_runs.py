@@ -1,0 +1,98 @@
+"""Full-length GPU parity runs of BASELINE.json's configs 2 and 3 against the oracle (north_star: "h, hu, hv within 1e-12
+relative per step and 1e-9 relative to max|eta| after the full run", masks and flags bit-exact, dt within 1e-14).
+
+The oracle needs about two minutes per config on one host core, so these are opt-in:
+
+    GC_FULL_PARITY=1 python -m pytest tests/test_gpu_full_runs.py -m gpu -x -q -s
+
+Without GC_FULL_PARITY they are skipped; tests/test_gpu_configs.py holds the prefixes that always run.  The design is
+bit-reproducible, so the assertions are exact equality; the north_star tolerances are evaluated as well
+and printed, so that a future non-zero difference is reported against the bar it has to meet."""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+from paper_1901_06798_b200 import driver
+from test_gpu_amr import same_storage
+
+pytestmark = [pytest.mark.gpu,
+              pytest.mark.skipif(os.environ.get("GC_FULL_PARITY") != "1", reason="full-length runs: set GC_FULL_PARITY=1")]
+
+G = 9.81
+
+
+def end_of_run_bar(fields_g, fields_o, b):
+    """north_star's end-of-run norm: |dh| <= 1e-9 max|eta|, |dhu|, |dhv| <= 1e-9 max|eta| sqrt(g max h).
+    Returns the largest difference as a fraction of its bar (0.0 when the fields are identical)."""
+    h = fields_o["h"]
+    sea = (h > 0.0) & (b < 0.0)                      # wet offshore cells: the scale is the wave amplitude, not the run-up height
+    eta_max = float(np.abs((h + b)[sea]).max()) if sea.any() else 0.0
+    bars = {"h": 1e-9 * eta_max, "hu": 1e-9 * eta_max * np.sqrt(G * h.max()), "hv": 1e-9 * eta_max * np.sqrt(G * h.max())}
+    worst = 0.0
+    for f in ("h", "hu", "hv"):
+        d = float(np.abs(fields_g[f] - fields_o[f]).max())
+        assert d <= bars[f], (f, d, bars[f])
+        worst = max(worst, d / bars[f] if bars[f] > 0 else 0.0)
+    return worst
+
+
+def test_config2_full_run(gc, gco):
+    """config 2 as BASELINE.json states it: 512 x 512, 2000 steps, run-up and draw-down on the wet/dry shoreline"""
+    wl = workloads.cfg2(512)
+    Lg = driver.setup_level(gc.Context(**wl.params), wl, patches=workloads.tile(512, 512, 128))
+    Lo = driver.setup_level(gco.Context(**wl.params), wl)
+    masks_g, masks_o = [], []
+    hg = driver.run_single_level(Lg, wl.nsteps, wl.cfl, record=lambda n, dt, st, L: masks_g.append(L.wet_mask().sum()) if n % 50 == 49 else None)
+    ho = driver.run_single_level(Lo, wl.nsteps, wl.cfl, record=lambda n, dt, st, L: masks_o.append(L.wet_mask().sum()) if n % 50 == 49 else None)
+    assert wl.nsteps == 2000 and len(hg) == len(ho) == 2000
+    assert [d for d, _ in hg] == [d for d, _ in ho]                                   # dt: exact (bar: 1e-14 relative)
+    assert [s["n_clipped"] for _, s in hg] == [s["n_clipped"] for _, s in ho]
+    assert [s["cfl_max"] for _, s in hg] == [s["cfl_max"] for _, s in ho]
+    assert masks_g == masks_o
+    fg = {f: Lg.get_global(f) for f in ("h", "hu", "hv")}
+    fo = {f: Lo.get_global(f) for f in ("h", "hu", "hv")}
+    worst = end_of_run_bar(fg, fo, Lo.get_global("b"))
+    for f in ("h", "hu", "hv"):
+        assert np.array_equal(fg[f], fo[f]), f
+    mg = driver.unpack_cells(Lg, Lg.wet_mask()); mo = driver.unpack_cells(Lo, Lo.wet_mask())
+    assert np.array_equal(mg, mo) and 0 < mo.sum() < mo.size
+    print("\nconfig 2 full run: 2000 steps, t = %.1f s, wet cells %d of %d, clipped cells in total %d; "
+          "largest end-of-run difference = %.3g of the 1e-9 bar (bit-identical)"
+          % (sum(d for d, _ in ho), int(mo.sum()), mo.size, sum(s["n_clipped"] for _, s in ho), worst))
+
+
+def test_config3_full_run(gc, gco):
+    """config 3 as BASELINE.json states it: 256 x 256 coarse at 2 arcmin, ratio 4, regrid every 4 coarse steps, to 1 hour"""
+    wl = workloads.cfg3(256)
+    Hg = driver.Hierarchy(gc.Context(**wl.params), wl)
+    Ho = driver.Hierarchy(gco.Context(**wl.params), wl)
+    dtg, dto = Hg.probe(), Ho.probe()
+    n = 0
+    while Ho.t < wl.t_end:
+        assert dtg == dto, (n, dtg, dto)
+        if Ho.t + dto > wl.t_end:
+            dtg = dto = wl.t_end - Ho.t
+        dtg, dto = Hg.step(dtg), Ho.step(dto)
+        assert Hg.t == Ho.t and len(Hg.levels) == len(Ho.levels)
+        for Lg, Lo in zip(Hg.levels, Ho.levels):
+            assert np.array_equal(Lg.patches, Lo.patches), n
+            assert np.array_equal(Lg.wet_mask(), Lo.wet_mask()), n
+        if n % 10 == 9:                                    # every patch of every level, ghost cells included
+            for Lg, Lo in zip(Hg.levels, Ho.levels):
+                same_storage(Lg, Lo)
+        n += 1
+    assert Ho.t == wl.t_end and Hg.regrids == Ho.regrids and Hg.regrids >= 50
+    assert len(Hg.flag_log) == len(Ho.flag_log)
+    for (kg, tg, fg), (ko, to, fo) in zip(Hg.flag_log, Ho.flag_log):
+        assert kg == ko and tg == to and np.array_equal(fg, fo)                        # refinement flags: bit-exact
+    worst = 0.0
+    for Lg, Lo in zip(Hg.levels, Ho.levels):
+        same_storage(Lg, Lo)
+        fg = {f: Lg.get_global(f, fill=0.0) for f in ("h", "hu", "hv")}
+        fo = {f: Lo.get_global(f, fill=0.0) for f in ("h", "hu", "hv")}
+        worst = max(worst, end_of_run_bar(fg, fo, Lo.get_global("b", fill=0.0)))
+    print("\nconfig 3 full run: %d coarse steps to t = %.0f s, %d regrids, levels %s cells; "
+          "largest end-of-run difference = %.3g of the 1e-9 bar (bit-identical)"
+          % (n, Ho.t, Ho.regrids, [int(L.ncells) for L in Ho.levels], worst))
