@@ -35,6 +35,8 @@ typedef struct {
     double g, dry_tol, sea_level, earth_radius;
     int limiter;          /* 0 none (first order), 1 MC */
     int bc[4];            /* xlo, xhi, ylo, yhi: 0 extrapolation, 1 wall */
+    double manning_n;     /* Manning coefficient n of P:52-57 eq. 2 (the paper uses 0.025); 0 = friction off */
+    double friction_depth;/* friction acts in cells with dry_tol < h <= friction_depth */
 } gco_params;
 
 typedef struct { int32_t i0, j0, nx, ny; } gco_patch; /* interior box, global cell indices of the level */
@@ -55,6 +57,13 @@ typedef struct {
 
 typedef struct gco_ctx gco_ctx;
 typedef struct gco_level gco_level;
+
+/* ---- Manning friction (gco_level.c), eq. 1b-1c, 2; DESIGN.md 3.9 (reading S-16) ---- */
+/* cube root of a positive normal double by the fixed sequence of DESIGN.md 3.9 (bit seed + three Halley steps) */
+double gco_cbrt(double x);
+/* semi-implicit friction step of one cell over dt: hu, hv <- hu / d, hv / d, d = 1 + dt g n^2 |hu, hv| / h^(7/3);
+ * acts only if manning_n > 0 and dry_tol < h <= friction_depth */
+void gco_friction(const gco_params *P, double dt, double h, double *hu, double *hv);
 
 /* ---- Riemann solver (gco_riemann.c), DESIGN.md 3.3 ---- */
 /* inputs: depth, normal momentum, transverse momentum, bathymetry on each side.

@@ -27,7 +27,8 @@ def build(force=False):
 
 class Params(C.Structure):
     _fields_ = [("coord", C.c_int), ("g", C.c_double), ("dry_tol", C.c_double), ("sea_level", C.c_double),
-                ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4)]
+                ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4),
+                ("manning_n", C.c_double), ("friction_depth", C.c_double)]
 
 
 class FlagParams(C.Structure):
@@ -81,12 +82,30 @@ def _chk(rc, what):
         raise RuntimeError("oracle %s failed: %d" % (what, rc))
 
 
-def make_params(coord=0, g=9.81, dry_tol=1e-3, sea_level=0.0, earth_radius=6367500.0, limiter=1, bc=(1, 1, 1, 1)):
+def make_params(coord=0, g=9.81, dry_tol=1e-3, sea_level=0.0, earth_radius=6367500.0, limiter=1, bc=(1, 1, 1, 1),
+                manning_n=0.0, friction_depth=1.0e6):
     p = Params()
     p.coord, p.g, p.dry_tol, p.sea_level, p.earth_radius, p.limiter = coord, g, dry_tol, sea_level, earth_radius, limiter
+    p.manning_n, p.friction_depth = manning_n, friction_depth
     for i in range(4):
         p.bc[i] = int(bc[i])
     return p
+
+
+def cbrt(x):
+    """the fixed cube-root sequence of DESIGN.md 3.9"""
+    f = lib().gco_cbrt; f.restype = C.c_double; f.argtypes = [C.c_double]
+    return f(float(x))
+
+
+def friction(dt, h, hu, hv, **kw):
+    """one cell's friction step -> (hu, hv)"""
+    p = make_params(**kw)
+    a, b = C.c_double(hu), C.c_double(hv)
+    f = lib().gco_friction; f.restype = None
+    f.argtypes = [C.POINTER(Params), C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    f(C.byref(p), float(dt), float(h), C.byref(a), C.byref(b))
+    return a.value, b.value
 
 
 def riemann(g, eps, hL, pL, tL, bL, hR, pR, tR, bR):
