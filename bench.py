@@ -129,6 +129,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--sweep", action="store_true", help="also report every tiling 16..256 in config.tilings")
+    ap.add_argument("--manning", type=float, default=0.0,
+                    help="Manning n of the friction step (DESIGN.md 3.9); 0 = off, as BASELINE.json's configs state no n")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -149,6 +151,8 @@ def main():
     W = max(args.warmup, 3)
     n = args.n
     wl = workloads.cfg5(n)
+    if args.manning > 0.0:
+        wl.params = dict(wl.params, manning_n=args.manning)
     ctx = binding.Context(device=dev, **wl.params)
 
     def make(side):
@@ -265,7 +269,8 @@ def main():
         "config": {"workload": "cfg5: spherical single level %dx%d at 0.5 arcmin, %dx%d patches of side %d, ghost fill + level step"
                                % (n, n, n // args.side, n // args.side, args.side),
                    "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (L.ncells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9 if L else 0),
-                   "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl, "fmad": False},
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl, "fmad": False,
+                   "manning_n": args.manning},
         "clocks": clocks,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 3 * cells * 8, "d2h_bytes_per_step": 3 * cells * 8 + 40,
                 "steps": Ke, "note": "state copied host->device and back every step through the C ABI (P:166 pipeline)"},

@@ -47,6 +47,9 @@ typedef struct {
     double earth_radius;  /* metres; used when coord == 1 */
     int limiter;          /* 0 none (first-order Godunov, eq. 4), 1 MC */
     int bc[4];            /* xlo, xhi, ylo, yhi: 0 zero-order extrapolation, 1 reflecting wall */
+    double manning_n;     /* Manning coefficient n of the drag term, eq. 1b-1c, 2 (the paper uses 0.025); 0 = friction off.
+                             Fractional step after the y-sweep of every level step with dt > 0 (reading S-16) */
+    double friction_depth;/* friction acts in cells with dry_tol < h <= friction_depth */
 } gc_params;
 
 typedef struct { int32_t i0, j0, nx, ny; } gc_patch;   /* interior box of a patch */

@@ -23,7 +23,8 @@ SYMBOLS = [
 
 class Params(C.Structure):
     _fields_ = [("coord", C.c_int), ("g", C.c_double), ("dry_tol", C.c_double), ("sea_level", C.c_double),
-                ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4)]
+                ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4),
+                ("manning_n", C.c_double), ("friction_depth", C.c_double)]
 
 
 class FlagParams(C.Structure):
@@ -202,7 +203,7 @@ class Context:
     name = "b200"
 
     def __init__(self, coord=0, g=9.81, dry_tol=1e-3, sea_level=0.0, earth_radius=6367500.0, limiter=1,
-                 bc=(1, 1, 1, 1), device="cuda:0", stream=None):
+                 bc=(1, 1, 1, 1), manning_n=0.0, friction_depth=1.0e6, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1901_06798_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -215,6 +216,7 @@ class Context:
         self._free_cb = FREE_FN(self._free)
         p = Params()
         p.coord, p.g, p.dry_tol, p.sea_level, p.earth_radius, p.limiter = coord, g, dry_tol, sea_level, earth_radius, limiter
+        p.manning_n, p.friction_depth = manning_n, friction_depth
         for k in range(4):
             p.bc[k] = int(bc[k])
         self.params = p

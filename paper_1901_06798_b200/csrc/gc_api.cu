@@ -60,6 +60,7 @@ extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc
 {
     if (!P || !out) return GC_ERR_BADARG;
     if (!(P->g > 0.0) || !(P->dry_tol >= 0.0) || (P->coord != 0 && P->coord != 1)) return GC_ERR_BADARG;
+    if (!(P->manning_n >= 0.0) || (P->manning_n > 0.0 && !(P->dry_tol > 0.0))) return GC_ERR_BADARG;   // friction divides by h^(7/3), h > dry_tol
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return GC_ERR_CUDA; }   // no CPU fallback
     gc_ctx *c = new gc_ctx();

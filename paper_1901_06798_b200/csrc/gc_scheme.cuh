@@ -198,3 +198,34 @@ __device__ __forceinline__ double gc_edge_cfl_std(const Waves &W, double rdL, do
     m = dmax(m, W.s[2] * rdR);
     return m;
 }
+
+// ---- Manning friction (eq. 1b-1c, 2, reading S-16) -----------------------------------------
+// Cube root of a positive normal double by a fixed sequence (no library call, so that every compiler produces the same
+// bits): bit pattern / 3 + K as the seed (worst relative error 3.2 %), then three Halley steps.
+__device__ __forceinline__ double gc_cbrt(double x)
+{
+    unsigned long long i = (unsigned long long)__double_as_longlong(x);
+    i = i / 3ull + 0x2A9F762500000000ull;
+    double y = __longlong_as_double((long long)i);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const double y3 = (y * y) * y;
+        y = y * ((y3 + 2.0 * x) / (2.0 * y3 + x));
+    }
+    return y;
+}
+
+// Semi-implicit fractional step of one cell over dt: hu, hv <- hu / d, hv / d with d = 1 + dt g n^2 |(hu, hv)| / h^(7/3)
+// (D of eq. 2 read over the momenta), for dry_tol < h <= friction_depth; gn2 = g * (n * n) formed by the host in that order.
+// Returns d, or exactly 1 for a cell friction does not act on (x / 1 = x bit for bit, so the caller divides either way).
+#ifndef GC_FRICTION_INLINE
+#define GC_FRICTION_INLINE __noinline__
+#endif
+static __device__ GC_FRICTION_INLINE double gc_friction_d(double gn2, double eps, double fdepth, double dt, double h, double hu, double hv)
+{
+    if (!(h > eps) || !(h <= fdepth)) return 1.0;
+    const double m = sqrt(hu * hu + hv * hv);
+    const double c = gc_cbrt(h);
+    const double gam = (gn2 * m) / ((h * h) * c);
+    return 1.0 + dt * gam;
+}

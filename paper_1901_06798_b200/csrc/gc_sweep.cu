@@ -43,6 +43,7 @@ struct SweepArgs {
     double dt; const double *dt_dev; // dt_dev != NULL: read dt from device memory
     int coord, limiter, write_out;
     DevStats *stats;
+    double gn2, fdepth; int friction; // Manning friction after the y-sweep: g n^2, friction_depth, on/off
     double dxdy;                     // dx*dy (cell area = kappa*dx*dy)
     const double *kappa;
 };
@@ -152,6 +153,10 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
             if (nh < a.eps && a.write_out) {           // dry clean-up (S-9)
                 if (nh < 0.0) { nclip = 1; clipm = (-nh) * (a.kappa[pd.j0 + ce] * a.dxdy); }
                 nh = dmax(nh, 0.0); np_ = 0.0; nt = 0.0;
+            }
+            if (a.friction && a.write_out) {                                                       // DESIGN.md 3.9; (hu, hv) = (nt, np_)
+                const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, nh, nt, np_);
+                nt = nt / d; np_ = np_ / d;
             }
             if (nh != nh || np_ != np_ || nt != nt) nanf = 1;
             if (a.write_out) { a.oh[idx] = nh; a.ohv[idx] = np_; a.ohu[idx] = nt; }
@@ -315,6 +320,10 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
                 if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
                     if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[pd.j0 + c - 2] * a.dxdy); }
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
+                }
+                if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
+                    const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
+                    ut = ut / d; up = up / d;
                 }
                 if (uh != uh || up != up || ut != ut) nanf = 1;
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
@@ -566,6 +575,10 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
                     if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[jrow + r - 2] * a.dxdy); }
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
                 }
+                if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
+                    const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
+                    ut = ut / d; up = up / d;
+                }
                 if (uh != uh || up != up || ut != ut) nanf = 1;
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
             }
@@ -641,6 +654,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     SweepArgs a;
     a.pat = L->d_pat; a.g = P.g; a.eps = P.dry_tol; a.dt = dt; a.dt_dev = dt_dev;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out; a.stats = L->d_stats;
+    a.gn2 = P.g * (P.manning_n * P.manning_n); a.fdepth = P.friction_depth; a.friction = P.manning_n > 0.0 ? 1 : 0;
     a.lines = nullptr; a.nlines = 0;
     a.ex = L->ex; a.ey = L->d_ey; a.dxdy = L->dx * L->dy; a.kappa = L->d_kappa; a.b = L->b;
     // x-sweep: Q^n -> Q*

@@ -158,6 +158,15 @@ def test_two_level_wet_dry_run_with_regrids(gc, gco, reflux):
     assert abs(Hg.composite_mass() - Ho.composite_mass()) <= 1e-13 * abs(Ho.composite_mass())
 
 
+def test_two_level_run_with_manning_friction(gc, gco):
+    """friction inside the AMR recursion: every level applies it after its own y-sweep with its own dt"""
+    base = workloads.cfg2(48)
+    wl = workloads.Workload("amr2f", dict(base.params, manning_n=0.025), 0.0, 0.0, base.dx, base.dy, 48, 48, base.bathy, base.eta0,
+                            cfl=0.9, ratios=(2,), flag=dict(tol_eta=0.1, buffer=2), regrid_interval=2, patch_max=24)
+    Hg, Ho = lockstep_hierarchies(gc, gco, wl, 12, reflux=True)
+    assert len(Hg.levels) == 2 and Hg.regrids >= 5
+
+
 def test_three_levels_middle_level_is_coarse_and_fine_side(gc, gco):
     base = workloads.cfg1(24)
     wl = workloads.Workload("amr3", base.params, 0.0, 0.0, base.dx, base.dy, 24, 24, base.bathy, base.eta0, cfl=0.9,

@@ -144,6 +144,33 @@ def test_spherical_walls(gc, gco):
     lockstep(Lg, Lo, 20, wl.cfl, 0.5)
 
 
+@pytest.mark.parametrize("fric", [dict(manning_n=0.025), dict(manning_n=0.025, friction_depth=5.0), dict(manning_n=0.1)])
+def test_manning_friction_wet_dry(gc, gco, fric):
+    """DESIGN.md 3.9 (S-16): the friction fractional step after the y-sweep and the clean-up, on the wet/dry shoreline of the
+    config-2 recipe -- everywhere, in cells no deeper than 5 m only, and with a large n; patches of 16 and one ragged tiling."""
+    n = 48
+    wl = workloads.cfg2(n)
+    wl.params = dict(wl.params, **fric)
+    ragged = np.array([[0, 0, 20, 48], [20, 0, 28, 10], [20, 10, 28, 38]], dtype=np.int32)
+    for pats in (workloads.tile(n, n, 16), ragged):
+        Lg, Lo = both(gc, gco, wl, patches_g=pats)
+        lockstep(Lg, Lo, 40, wl.cfl, 2.0)
+        assert np.abs(Lo.get_global("hu")).max() > 1e-3          # the run has flow for friction to act on
+
+
+def test_manning_friction_spherical(gc, gco):
+    n = 128
+    wl = workloads.cfg5(n)
+    wl.params = dict(wl.params, manning_n=0.025)
+    Lg, Lo = both(gc, gco, wl, patches_g=workloads.tile(n, n, 32))
+    lockstep(Lg, Lo, 10, wl.cfl, 1.0)
+    # and it is not a no-op there: the same run without friction ends with different momenta
+    wl0 = workloads.cfg5(n)
+    L0 = driver.setup_level(gco.Context(**wl0.params), wl0)
+    driver.run_single_level(L0, 10, wl0.cfl)
+    assert not np.array_equal(L0.get_global("hu"), Lo.get_global("hu"))
+
+
 def test_first_order_mode(gc, gco):
     wl = workloads.cfg2(64)
     wl.params = dict(wl.params, limiter=0)
