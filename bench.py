@@ -84,6 +84,37 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# ---- N > 1: replicas only.  One process per GPU, each advancing its own copy of the level; no data-path collective.
+# The only exchanges are a barrier on both sides of a timed region and the max over ranks of its duration.
+def init_ranks(backend="nccl", device=None):
+    """-> (rank, world, local_rank, dist or None) from torchrun's environment; joins the process group when world > 1."""
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world == 1:
+        return rank, world, local, None
+    import torch.distributed as dist
+    if device is not None:
+        dist.init_process_group(backend, device_id=device)
+    else:
+        dist.init_process_group(backend)
+    return rank, world, local, dist
+
+
+def max_over_ranks(x, dist, device="cpu"):
+    """the slowest rank's value of a duration (every rank gets it); x itself without a process group"""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.item()
+
+
+def job_rate(units_per_rank, world, seconds):
+    """whole-job throughput of `world` replicas that each processed units_per_rank in `seconds` (the max over ranks)"""
+    return world * units_per_rank / seconds
+
+
 def oracle_rate(n, steps, warmup=0):
     """The oracle as it stands, one thread: config-5 recipe at n x n, one patch.  -> (updates/s, seconds)"""
     import workloads
@@ -140,13 +171,9 @@ def main():
     import workloads
     from paper_1901_06798_b200 import binding, driver
 
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        torch.cuda.set_device(local)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    rank, world, local, dist = init_ranks("nccl", torch.device("cuda", local))
     dev = "cuda:%d" % local
     W = max(args.warmup, 3)
     n = args.n
@@ -201,12 +228,9 @@ def main():
     ms, launches, prof = timed(L, args.steps, W)
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
-    if dist:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = t.item()
+    ms = max_over_ranks(ms, dist, dev)
     cells = n * n
-    value = world * cells * args.steps / (ms * 1e-3)
+    value = job_rate(cells * args.steps, world, ms * 1e-3)
 
     # end to end through the C ABI with HOST buffers: every step copies the state host -> device and back (the paper's own
     # pipeline) around fill + step; pinned host memory
@@ -229,11 +253,8 @@ def main():
             ctx._chk(binding.lib().gc_level_get_global(L.h, k, 0, hnp[k].ctypes.data, 0, n, 0, 0, n, n), "get")
     torch.cuda.synchronize()
     e2e_s = time.time() - w0
-    if dist:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = t.item()
-    e2e = world * cells * Ke / e2e_s
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
+    e2e = job_rate(cells * Ke, world, e2e_s)
 
     tilings = None
     if args.sweep and rank == 0:
