@@ -9,6 +9,7 @@ Without GC_FULL_PARITY they are skipped; tests/test_gpu_configs.py holds the pre
 bit-reproducible, so the assertions are exact equality; the north_star tolerances are evaluated as well
 and printed, so that a future non-zero difference is reported against the bar it has to meet."""
 import os
+import time
 
 import numpy as np
 import pytest
@@ -44,8 +45,11 @@ def test_config2_full_run(gc, gco):
     Lg = driver.setup_level(gc.Context(**wl.params), wl, patches=workloads.tile(512, 512, 128))
     Lo = driver.setup_level(gco.Context(**wl.params), wl)
     masks_g, masks_o = [], []
+    t0 = time.time()
     hg = driver.run_single_level(Lg, wl.nsteps, wl.cfl, record=lambda n, dt, st, L: masks_g.append(L.wet_mask().sum()) if n % 50 == 49 else None)
+    t1 = time.time()
     ho = driver.run_single_level(Lo, wl.nsteps, wl.cfl, record=lambda n, dt, st, L: masks_o.append(L.wet_mask().sum()) if n % 50 == 49 else None)
+    t2 = time.time()
     assert wl.nsteps == 2000 and len(hg) == len(ho) == 2000
     assert [d for d, _ in hg] == [d for d, _ in ho]                                   # dt: exact (bar: 1e-14 relative)
     assert [s["n_clipped"] for _, s in hg] == [s["n_clipped"] for _, s in ho]
@@ -61,6 +65,9 @@ def test_config2_full_run(gc, gco):
     print("\nconfig 2 full run: 2000 steps, t = %.1f s, wet cells %d of %d, clipped cells in total %d; "
           "largest end-of-run difference = %.3g of the 1e-9 bar (bit-identical)"
           % (sum(d for d, _ in ho), int(mo.sum()), mo.size, sum(s["n_clipped"] for _, s in ho), worst))
+    upd = 512 * 512 * 2000
+    print("config 2 wall time of the run (host-synchronised every step, wet mask fetched every 50): CUDA path %.2f s = %.3g updates/s; "
+          "oracle on one host core %.1f s = %.3g updates/s" % (t1 - t0, upd / (t1 - t0), t2 - t1, upd / (t2 - t1)))
 
 
 def test_config3_full_run(gc, gco):
@@ -70,11 +77,13 @@ def test_config3_full_run(gc, gco):
     Ho = driver.Hierarchy(gco.Context(**wl.params), wl)
     dtg, dto = Hg.probe(), Ho.probe()
     n = 0
+    wall_g = wall_o = 0.0
     while Ho.t < wl.t_end:
         assert dtg == dto, (n, dtg, dto)
         if Ho.t + dto > wl.t_end:
             dtg = dto = wl.t_end - Ho.t
-        dtg, dto = Hg.step(dtg), Ho.step(dto)
+        w0 = time.time(); dtg = Hg.step(dtg); w1 = time.time(); dto = Ho.step(dto); w2 = time.time()
+        wall_g += w1 - w0; wall_o += w2 - w1
         assert Hg.t == Ho.t and len(Hg.levels) == len(Ho.levels)
         for Lg, Lo in zip(Hg.levels, Ho.levels):
             assert np.array_equal(Lg.patches, Lo.patches), n
@@ -96,3 +105,5 @@ def test_config3_full_run(gc, gco):
     print("\nconfig 3 full run: %d coarse steps to t = %.0f s, %d regrids, levels %s cells; "
           "largest end-of-run difference = %.3g of the 1e-9 bar (bit-identical)"
           % (n, Ho.t, Ho.regrids, [int(L.ncells) for L in Ho.levels], worst))
+    print("config 3 wall time inside Hierarchy.step (levels, regrids, average-down, fix-up): CUDA path %.2f s = %.3g updates/s; "
+          "oracle on one host core %.1f s = %.3g updates/s" % (wall_g, Ho.updates / wall_g, wall_o, Ho.updates / wall_o))
