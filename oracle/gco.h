@@ -104,6 +104,11 @@ int gco_level_get_global(const gco_level *, int field, int which, double *dst, i
 int gco_fill_ghost_b(gco_level *);
 int gco_fill_ghost(gco_level *L, const gco_level *coarser, double alpha);
 int gco_level_step(gco_level *L, double dt, gco_step_stats *out);
+/* ---- gauges (gco_amr.c); DESIGN.md 3.10 (reading S-19) ---- */
+/* Samples n points from the current state of L (ghost cells as they are): point k = (xy[2k], xy[2k+1]) must lie in the interior
+ * of patch patch[k] (else GCO_ERR_BADARG).  out: 4 per point -- h, hu, hv, eta = h + b; bilinear between the four cell centres
+ * around the point when all four are wet, else the value of the cell containing the point. */
+int gco_gauges_sample(const gco_level *L, int n, const int32_t *patch, const double *xy, double *out);
 int gco_wet_mask(const gco_level *, uint8_t *mask /* interior-packed per patch */);
 double gco_level_mass(const gco_level *);
 int64_t gco_level_ncells(const gco_level *);

@@ -186,6 +186,14 @@ class Level:
         return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
                     n_clipped=st.n_clipped, nan_seen=st.nan_seen)
 
+    def gauges_sample(self, patch, xy):
+        """(h, hu, hv, eta) at the points xy (n x 2), point k inside patch[k] -> n x 4"""
+        patch = np.ascontiguousarray(patch, dtype=np.int32); xy = np.ascontiguousarray(xy, dtype=np.float64).reshape(-1, 2)
+        out = np.empty((len(patch), 4))
+        _chk(lib().gco_gauges_sample(self.h, len(patch), patch.ctypes.data_as(C.POINTER(C.c_int32)), xy.ctypes.data_as(_dp),
+                                     out.ctypes.data_as(_dp)), "gauges_sample")
+        return out
+
     def wet_mask(self):
         m = np.zeros(self.ncells, dtype=np.uint8)
         _chk(lib().gco_wet_mask(self.h, m.ctypes.data), "wet_mask")

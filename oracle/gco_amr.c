@@ -231,3 +231,45 @@ int gco_flag_cells(const gco_level *L, const gco_flag_params *fp, double t, uint
     free(raw); free(poff);
     return GCO_OK;
 }
+
+/* P:166 "finding the best grid patch ..., interpolating from cell values": DESIGN.md 3.10 (S-19).  The best patch is found by the
+ * caller (host bookkeeping); this is the interpolation, in the order DESIGN.md states. */
+int gco_gauges_sample(const gco_level *L, int n, const int32_t *patch, const double *xy, double *out)
+{
+    int k, f;
+    if (!L || n < 0 || (n > 0 && (!patch || !xy || !out))) return GCO_ERR_BADARG;
+    for (k = 0; k < n; k++) {
+        const gco_patch *Pp;
+        const double *fld[3];
+        const double *bb;
+        double eps = L->ctx->P.dry_tol;
+        double gx, gy, xi, et, a, b, v[4][4];
+        int64_t ic, jc, i, j, pitch, c00;
+        int dry = 0, m;
+        if (patch[k] < 0 || patch[k] >= L->np) return GCO_ERR_BADARG;
+        Pp = &L->pat[patch[k]];
+        pitch = (int64_t)Pp->nx + 4;
+        gx = (xy[2 * k] - L->xlo) / L->dx;  gy = (xy[2 * k + 1] - L->ylo) / L->dy;
+        ic = (int64_t)floor(gx); jc = (int64_t)floor(gy);                 /* the cell that contains the point */
+        if (ic < Pp->i0 || ic >= (int64_t)Pp->i0 + Pp->nx || jc < Pp->j0 || jc >= (int64_t)Pp->j0 + Pp->ny) return GCO_ERR_BADARG;
+        xi = gx - 0.5; et = gy - 0.5;
+        i = (int64_t)floor(xi); j = (int64_t)floor(et);
+        a = xi - (double)i; b = et - (double)j;
+        for (f = 0; f < 3; f++) fld[f] = L->q[L->cur][f] + L->off[patch[k]];
+        bb = L->b + L->off[patch[k]];
+        c00 = (j - Pp->j0 + 2) * pitch + (i - Pp->i0 + 2);
+        for (m = 0; m < 4; m++) {                                          /* m = 0: (i, j), 1: (i+1, j), 2: (i, j+1), 3: (i+1, j+1) */
+            int64_t c = c00 + (m & 1) + (m >> 1) * pitch;
+            v[0][m] = fld[0][c]; v[1][m] = fld[1][c]; v[2][m] = fld[2][c]; v[3][m] = fld[0][c] + bb[c];
+            if (!(fld[0][c] > eps)) dry = 1;
+        }
+        if (dry) {
+            int64_t c = (jc - Pp->j0 + 2) * pitch + (ic - Pp->i0 + 2);
+            out[4 * k] = fld[0][c]; out[4 * k + 1] = fld[1][c]; out[4 * k + 2] = fld[2][c]; out[4 * k + 3] = fld[0][c] + bb[c];
+        } else {
+            for (f = 0; f < 4; f++)
+                out[4 * k + f] = (1.0 - b) * ((1.0 - a) * v[f][0] + a * v[f][1]) + b * ((1.0 - a) * v[f][2] + a * v[f][3]);
+        }
+    }
+    return GCO_OK;
+}

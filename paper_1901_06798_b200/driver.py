@@ -72,7 +72,7 @@ def run_single_level(L, nsteps, cfl, dt0=None, record=None):
 
 # ---------------------------------------------------------------------------------------------------------
 # Clustering ("Berger-Rigoutsos"): flagged cells of level l -> rectangles.  Deterministic (ties to the
-# lower index), shared by both backends AFTER their flags have been compared bit for bit (DESIGN.md 3.10 S-13).
+# lower index), shared by both backends AFTER their flags have been compared bit for bit (DESIGN.md 3.11 S-13).
 def _signature_cut(sig):
     """Cut position (1..n-1) for a 1-D signature: first a hole (zero entry) nearest the centre, else the strongest
     inflection of the discrete Laplacian; None if neither exists."""
