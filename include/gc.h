@@ -75,6 +75,18 @@ typedef struct {
 typedef void *(*gc_alloc_fn)(size_t bytes, void *user);
 typedef void (*gc_free_fn)(void *ptr, void *user);
 
+/* Gauges ("finding the best grid patch to sample quantities of interest from, interpolating from cell values"; DESIGN.md
+ * 3.10, reading S-19).  The caller finds the best patch (finest level whose interior holds the point: host bookkeeping).
+ * gc_gauges_bind: gauge k = point (xy[2k], xy[2k+1]) in the level's coordinates, inside the INTERIOR of patch patch[k] of L
+ * (else GC_ERR_BADARG, nothing changes); both arrays HOST, read before return; replaces any earlier binding; n = 0 unbinds.
+ * The binding dies with the level.
+ * gc_gauges_sample: 4 doubles per bound gauge, in binding order -- h, hu, hv, eta = h + b -- from the level's current state with
+ * its ghost cells as they are (call gc_fill_ghost first): bilinear between the four cell centres around the point when all four
+ * are wet (h > dry_tol), else the values of the cell containing the point.  out DEVICE: enqueued on the context's stream,
+ * returns without synchronising (a device-resident series costs one small kernel per record); out HOST: synchronous. */
+int gc_gauges_bind(gc_level *L, int n, const int32_t *patch /*HOST*/, const double *xy /*HOST*/);
+int gc_gauges_sample(const gc_level *L, double *out, int out_is_device);
+
 /* Context: parameters + the CUDA stream (cudaStream_t passed as void*; NULL = legacy default stream). */
 int gc_ctx_create(const gc_params *params /*HOST*/, void *cuda_stream, gc_alloc_fn alloc, gc_free_fn free_,
                   void *user, gc_ctx **out);

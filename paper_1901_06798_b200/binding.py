@@ -17,7 +17,7 @@ SYMBOLS = [
     "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
-    "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math",
+    "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample",
 ]
 
 
@@ -65,6 +65,8 @@ def lib():
     L.gc_level_get_global.argtypes = [vp, i, i, vp, i, i64, i64, i64, i64, i64]
     L.gc_fill_ghost.argtypes = [vp, vp, d]
     L.gc_fill_ghost_b.argtypes = [vp]
+    L.gc_gauges_bind.argtypes = [vp, i, vp, vp]
+    L.gc_gauges_sample.argtypes = [vp, vp, i]
     L.gc_level_step.argtypes = [vp, d, vp]
     L.gc_level_step_auto.argtypes = [vp, vp, d]
     L.gc_level_stats.argtypes = [vp, vp]
@@ -166,6 +168,27 @@ class Level:
         self.ctx._chk(lib().gc_level_stats(self.h, C.byref(st)), "gc_level_stats")
         return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
                     n_clipped=st.n_clipped, nan_seen=st.nan_seen)
+
+    # ---- gauges
+    def gauges_bind(self, patch, xy):
+        """binds gauge k = point xy[k] inside the interior of patch[k]; replaces any earlier binding (empty lists unbind)"""
+        patch = np.ascontiguousarray(patch, dtype=np.int32); xy = np.ascontiguousarray(xy, dtype=np.float64).reshape(-1, 2)
+        self.ctx._chk(lib().gc_gauges_bind(self.h, len(patch), patch.ctypes.data, xy.ctypes.data), "gc_gauges_bind")
+        self.ngauge = len(patch)
+
+    def gauges_sample(self, patch=None, xy=None):
+        """(h, hu, hv, eta) per gauge -> n x 4 on the host.  With patch, xy: binds them first (the oracle's call shape)."""
+        if patch is not None:
+            self.gauges_bind(patch, xy)
+        out = np.empty((getattr(self, "ngauge", 0), 4))
+        self.ctx._chk(lib().gc_gauges_sample(self.h, out.ctypes.data, 0), "gc_gauges_sample")
+        return out
+
+    def gauges_sample_into(self, row):
+        """the same, written into a device tensor of at least 4 * ngauge float64 (a row of a device-resident series);
+        enqueued on the context's stream, no synchronisation"""
+        assert row.is_cuda and row.dtype == self.ctx.torch.float64 and row.is_contiguous() and row.numel() >= 4 * getattr(self, "ngauge", 0)
+        self.ctx._chk(lib().gc_gauges_sample(self.h, row.data_ptr(), 1), "gc_gauges_sample")
 
     def wet_mask(self):
         m = np.zeros(self.ncells, dtype=np.uint8)

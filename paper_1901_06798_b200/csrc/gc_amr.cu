@@ -454,3 +454,40 @@ void gc_launch_flux_fixup(gc_level *C)
                                                                    C->q[C->cur][0], C->q[C->cur][1], C->q[C->cur][2],
                                                                    C->d_kappa, C->dx, C->dy, C->ctx->P.dry_tol);
 }
+
+
+// ---- gauges (reading S-19): thread per bound gauge.  Offsets and weights were fixed on the host at bind
+// time; the sample is the bilinear form in the cell centres, in DESIGN.md's order, or the containing cell if the stencil is not all wet.
+__global__ void k_gauges_sample(const GaugeLoc *g, int n, const double *h, const double *hu, const double *hv, const double *b,
+                                double eps, double *out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const GaugeLoc G = g[k];
+    double v[4][4];
+    bool dry = false;
+#pragma unroll
+    for (int m = 0; m < 4; m++) {
+        const int64_t c = G.c00 + (m & 1) + (int64_t)(m >> 1) * G.pitch;
+        const double hh = h[c];
+        v[0][m] = hh; v[1][m] = hu[c]; v[2][m] = hv[c]; v[3][m] = hh + b[c];
+        dry = dry || !(hh > eps);
+    }
+    if (dry) {
+        const double hh = h[G.cc];
+        out[4 * k] = hh; out[4 * k + 1] = hu[G.cc]; out[4 * k + 2] = hv[G.cc]; out[4 * k + 3] = hh + b[G.cc];
+    } else {
+        const double a = G.a, bw = G.b;
+#pragma unroll
+        for (int f = 0; f < 4; f++)
+            out[4 * k + f] = (1.0 - bw) * ((1.0 - a) * v[f][0] + a * v[f][1]) + bw * ((1.0 - a) * v[f][2] + a * v[f][3]);
+    }
+}
+
+void gc_launch_gauges(const gc_level *L, double *out)
+{
+    if (L->ngauge <= 0) return;
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
+    k_gauges_sample<<<(L->ngauge + 127) / 128, 128, 0, L->ctx->stream>>>(L->d_gauge, L->ngauge, L->q[L->cur][0], L->q[L->cur][1],
+                                                                         L->q[L->cur][2], L->b, L->ctx->P.dry_tol, out);
+}

@@ -1,5 +1,6 @@
 // gc_api_amr.cu -- level-transfer entry points (A3, A8-A11): host list building + launches.
 // The host only intersects boxes and builds index lists (bookkeeping); every value is computed in gc_amr.cu.
+#include <math.h>
 #include <string.h>
 #include <algorithm>
 #include <map>
@@ -344,4 +345,54 @@ extern "C" int gc_flux_fixup(gc_level *C, gc_level *F)
     if (!C || !F || C->reg_fine != F) return gc_fail(C ? C->ctx : nullptr, GC_ERR_BADARG, "gc_flux_fixup: levels are not attached");
     gc_launch_flux_fixup(C);
     return gc_cuda_check(C->ctx, "gc_flux_fixup");
+}
+
+
+// ---- gauges
+extern "C" int gc_gauges_bind(gc_level *L, int n, const int32_t *patch, const double *xy)
+{
+    if (!L || n < 0 || (n > 0 && (!patch || !xy))) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_gauges_bind: bad argument");
+    std::vector<GaugeLoc> loc((size_t)n);
+    for (int k = 0; k < n; k++) {
+        if (patch[k] < 0 || patch[k] >= L->np) return gc_fail(L->ctx, GC_ERR_BADARG, "gc_gauges_bind: no such patch");
+        const PatchDesc &D = L->hpat[patch[k]];
+        const double gx = (xy[2 * k] - L->xlo) / L->dx, gy = (xy[2 * k + 1] - L->ylo) / L->dy;
+        if (!(gx >= (double)D.i0 && gx < (double)D.i0 + D.nx && gy >= (double)D.j0 && gy < (double)D.j0 + D.ny))
+            return gc_fail(L->ctx, GC_ERR_BADARG, "gc_gauges_bind: gauge outside the interior of its patch");
+        const int64_t ic = (int64_t)floor(gx), jc = (int64_t)floor(gy);       // the cell that contains the point
+        const double xi = gx - 0.5, et = gy - 0.5;
+        const int64_t i = (int64_t)floor(xi), j = (int64_t)floor(et);
+        GaugeLoc &G = loc[(size_t)k];
+        G.a = xi - (double)i; G.b = et - (double)j;
+        G.pitch = D.pitch; G.pad = 0;
+        G.c00 = D.off + (j - D.j0 + 2) * (int64_t)D.pitch + (i - D.i0 + 2);
+        G.cc = D.off + (jc - D.j0 + 2) * (int64_t)D.pitch + (ic - D.i0 + 2);
+    }
+    if (L->d_gauge) { cudaStreamSynchronize(L->ctx->stream); drop_alloc(L, L->d_gauge); L->d_gauge = nullptr; }
+    L->ngauge = 0;
+    if (n > 0) {
+        L->d_gauge = upload_tmp(L->ctx, loc);
+        if (!L->d_gauge) return gc_fail(L->ctx, GC_ERR_NOMEM, "gc_gauges_bind: allocation failed");
+        L->allocs.push_back(L->d_gauge);
+        L->ngauge = n;
+        cudaStreamSynchronize(L->ctx->stream);                                   // loc goes out of scope
+    }
+    return gc_cuda_check(L->ctx, "gc_gauges_bind");
+}
+
+extern "C" int gc_gauges_sample(const gc_level *L, double *out, int out_is_device)
+{
+    if (!L || (L->ngauge > 0 && !out)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_gauges_sample: bad argument");
+    if (L->ngauge == 0) return GC_OK;
+    gc_ctx *c = L->ctx;
+    if (out_is_device) { gc_launch_gauges(L, out); return gc_cuda_check(c, "gc_gauges_sample"); }   // asynchronous
+    bool transient = false;
+    const size_t bytes = (size_t)L->ngauge * 4 * sizeof(double);
+    double *d = (double *)gc_stage_get(c, bytes, &transient);
+    if (!d) return gc_fail(c, GC_ERR_NOMEM, "gc_gauges_sample: staging allocation failed");
+    gc_launch_gauges(L, d);
+    cudaMemcpyAsync(out, d, bytes, cudaMemcpyDeviceToHost, c->stream);
+    cudaStreamSynchronize(c->stream);
+    if (transient) gc_dev_free(c, d);
+    return gc_cuda_check(c, "gc_gauges_sample");
 }

@@ -102,6 +102,9 @@ struct ProfScope {
     ~ProfScope() { if (e0) { cudaEventRecord(e1, c->stream); c->ev[slot].push_back({e0, e1}); } }
 };
 
+// one bound gauge: pool offsets of stencil cell (i, j) and of the containing cell, the patch's row pitch, the weights
+struct GaugeLoc { int64_t c00, cc; int32_t pitch, pad; double a, b; };
+
 struct gc_level {
     gc_ctx *ctx;
     int level, ratio, np, cur;
@@ -140,7 +143,10 @@ struct gc_level {
     // cached average-down list for a given fine level, cached neighbour lists for flag dilation
     uint64_t avg_gen; AvgRect *d_avg; int64_t *d_avgstart; int navg; int64_t navgcells;
     int nbr_buffer; int32_t *d_nbrstart, *d_nbrlist;
+    GaugeLoc *d_gauge = nullptr; int ngauge = 0;     // gauges bound to this level (gc_gauges_bind)
 };
+
+void gc_launch_gauges(const gc_level *L, double *out);
 
 // ---- helpers (gc_api.cu)
 void *gc_dev_alloc(gc_ctx *c, size_t bytes);

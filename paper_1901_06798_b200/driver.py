@@ -181,12 +181,90 @@ def nesting_mask(L, bbox=None):
     return ok
 
 
+class GaugeRecorder:
+    """Gauges (reading S-19): host bookkeeping around the backends' sampling call.  Each gauge belongs to
+    the finest level whose interior holds it (re-decided after every regrid); a level's gauges are sampled right after its ghost
+    fill and before its step, and once more at the end of the run.  records[g] = list of (t, h, hu, hv, eta).
+    device_series=True (CUDA backend only): samples go into a device tensor per level, one small kernel per record and no
+    copy; they are read back when the assignment changes and at the end."""
+
+    def __init__(self, xy, device_series=False, capacity=4096):
+        self.xy = np.ascontiguousarray(xy, dtype=np.float64).reshape(-1, 2)
+        self.records = [[] for _ in range(len(self.xy))]
+        self.device_series = device_series
+        self.capacity = capacity
+        self.assign = []            # per level: (gauge ids, patch ids)
+        self._series = []           # per level (device path): [level object, tensor capacity x n x 4, list of times]
+
+    @staticmethod
+    def patch_of(L, x, y):
+        ic = np.floor((x - L.xlo) / L.dx); jc = np.floor((y - L.ylo) / L.dy)
+        p = np.asarray(L.patches)
+        hit = np.nonzero((p[:, 0] <= ic) & (ic < p[:, 0] + p[:, 2]) & (p[:, 1] <= jc) & (jc < p[:, 1] + p[:, 3]))[0]
+        return int(hit[0]) if len(hit) else -1
+
+    def rebind(self, levels):
+        self.flush()
+        owner = [None] * len(self.xy)
+        for k in reversed(range(len(levels))):                      # finest level first
+            for g, (x, y) in enumerate(self.xy):
+                if owner[g] is None:
+                    pch = self.patch_of(levels[k], x, y)
+                    if pch >= 0:
+                        owner[g] = (k, pch)
+        self.assign = []
+        for k in range(len(levels)):
+            ids = [g for g, o in enumerate(owner) if o is not None and o[0] == k]
+            self.assign.append((ids, [owner[g][1] for g in ids]))
+        self._series = []
+        if self.device_series:
+            for k, L in enumerate(levels):
+                ids, pats = self.assign[k]
+                L.gauges_bind(pats, self.xy[ids])
+                buf = L.ctx.torch.empty((self.capacity, max(len(ids), 1), 4), dtype=L.ctx.torch.float64, device=L.ctx.device) if ids else None
+                self._series.append([L, buf, []])
+
+    def record(self, k, L, t):
+        ids, pats = self.assign[k]
+        if not ids:
+            return
+        if self.device_series:
+            lev, buf, times = self._series[k]
+            if len(times) == self.capacity:
+                self.flush(only=k)
+                lev, buf, times = self._series[k]
+            L.gauges_sample_into(buf[len(times)])
+            times.append(t)
+        else:
+            out = L.gauges_sample(pats, self.xy[ids])
+            for n, g in enumerate(ids):
+                self.records[g].append((t,) + tuple(float(v) for v in out[n]))
+
+    def flush(self, only=None):
+        """device path: read the finished part of every series back and append it to the records"""
+        for k, ser in enumerate(self._series):
+            if (only is not None and k != only) or ser[1] is None or not ser[2]:
+                continue
+            lev, buf, times = ser
+            host = buf[:len(times)].cpu().numpy()
+            for n, g in enumerate(self.assign[k][0]):
+                for r, t in enumerate(times):
+                    self.records[g].append((t,) + tuple(float(v) for v in host[r, n]))
+            ser[2] = []
+
+    def series(self, g):
+        """records of gauge g sorted by time, as an array n x 5 (t, h, hu, hv, eta)"""
+        self.flush()
+        return np.array(sorted(self.records[g]), dtype=np.float64).reshape(-1, 5)
+
+
 class Hierarchy:
     """The AMR recursion of P:140-146 (steps 1-5) with regridding every `regrid_interval` steps of a level,
     driving one backend through the C-ABI calls.  Bookkeeping only."""
 
-    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7):
+    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7, gauges=None):
         self.ctx, self.wl, self.reflux, self.eff = ctx, wl, reflux, efficiency
+        self.gauges = gauges             # GaugeRecorder or None (DESIGN.md 3.10)
         nl = 1 + len(wl.ratios) if max_levels is None else min(max_levels, 1 + len(wl.ratios))
         self.ratios = list(wl.ratios)[:nl - 1]
         self.levels = [setup_level(ctx, wl, patches=patches1)]
@@ -259,6 +337,8 @@ class Hierarchy:
                 self.levels.append(N); self.alpha_now.append(1.0); self.steps.append(0); self.sdx.append(0.0)
             if self.reflux:
                 C.flux_attach(N)
+        if self.gauges is not None:
+            self.gauges.rebind(self.levels)
 
     def probe(self):
         """dt of level 1 from dt = 0 probe steps of every level"""
@@ -269,9 +349,12 @@ class Hierarchy:
             m = max(m, L.step(0.0)["s_over_dx_max"] / R)
         return self.wl.cfl / m
 
-    def _advance(self, k, dt, alpha):
+    def _advance(self, k, dt, alpha, t):
+        """one step of level k from its time t (alpha: that time as a fraction of the coarser level's current step)"""
         L = self.levels[k]
         L.fill_ghost(self.levels[k - 1] if k > 0 else None, alpha)
+        if self.gauges is not None:
+            self.gauges.record(k, L, t)
         st = L.step(dt)
         self.sdx[k] = max(self.sdx[k], st["s_over_dx_max"])
         self.steps[k] += 1
@@ -280,7 +363,7 @@ class Hierarchy:
             r = self.ratios[k]
             for s in range(r):
                 self.alpha_now[k + 1] = (s + 1) / r
-                self._advance(k + 1, dt / r, s / r)
+                self._advance(k + 1, dt / r, s / r, t + s * (dt / r))
         if k + 1 < len(self.levels):        # the finer level may have vanished in a regrid below
             F = self.levels[k + 1]
             if self.reflux:
@@ -293,7 +376,7 @@ class Hierarchy:
         """one step of level 1 (and everything above it); returns the next dt of level 1"""
         self.sdx = [0.0] * len(self.levels)
         self.alpha_now[0] = 1.0
-        self._advance(0, dt, 1.0)
+        self._advance(0, dt, 1.0, self.t)
         self.t += dt
         if len(self.ratios) > 0 and self.steps[0] % self.wl.regrid_interval == 0:
             self._regrid(0)
@@ -314,7 +397,16 @@ class Hierarchy:
                 record(n, dt, self)
             dt = dtn
             n += 1
+        self.record_gauges_now()
         return n
+
+    def record_gauges_now(self):
+        """one record of every gauge at the hierarchy's current time (all levels are at self.t between coarse steps)"""
+        if self.gauges is None:
+            return
+        for k, L in enumerate(self.levels):
+            L.fill_ghost(self.levels[k - 1] if k > 0 else None, 1.0)
+            self.gauges.record(k, L, self.t)
 
     def composite_mass(self):
         """mass over the finest available cells: sum over levels of the mass of cells not covered by a finer level.

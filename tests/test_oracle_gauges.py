@@ -103,3 +103,58 @@ def test_point_outside_its_patch_is_refused(gco):
             L.gauges_sample([0], bad)
     with pytest.raises(RuntimeError):
         L.gauges_sample([7], [[3500.0, 3500.0]])
+
+
+def test_gauges_in_an_ocean_at_rest_record_the_sea_level(gco):
+    rng = np.random.default_rng(21)
+    n, d = 40, 200.0
+    X, Y = np.meshgrid(centres(n, d), centres(n, d))
+    bathy = lambda x, y: -300.0 + 330.0 * np.exp(-((x - 2500) ** 2 + (y - 4000) ** 2) / 900.0 ** 2) + 12.0 * np.sin(x / 310.0) * np.cos(y / 270.0)
+    wl = workloads.Workload("rest", dict(coord=0, dry_tol=1e-3, bc=(1, 1, 0, 0)), 0.0, 0.0, d, d, n, n, bathy, lambda x, y: 0.0 * x, cfl=0.9)
+    island = (2500.0, 4000.0)
+    assert bathy(*island) > 5.0
+    pts = np.vstack([rng.uniform(300.0, 7700.0, (12, 2)), [island]])
+    G = driver.GaugeRecorder(pts)
+    H = driver.Hierarchy(gco.Context(**wl.params), wl, gauges=G)
+    nsteps = H.run(nsteps=60)
+    assert nsteps == 60
+    wet_seen = 0
+    for g in range(len(pts)):
+        S = G.series(g)
+        assert len(S) == 61 and S[0, 0] == 0.0 and S[-1, 0] == H.t and (np.diff(S[:, 0]) > 0).all()
+        if bathy(*pts[g]) < -1.0:
+            wet_seen += 1
+            assert np.abs(S[:, 4]).max() < 1e-11 and np.abs(S[:, 2]).max() < 1e-10 and np.abs(S[:, 3]).max() < 1e-10
+    assert wet_seen >= 8
+    S = G.series(len(pts) - 1)                                                # on the island: dry, eta = the land elevation of its cell
+    assert (S[:, 1] == 0.0).all() and (S[:, 4] > 5.0).all() and np.ptp(S[:, 4]) == 0.0
+
+
+def test_gauge_ownership_and_times_in_an_amr_run(gco):
+    base = workloads.cfg2(48)
+    wl = workloads.Workload("amr2g", base.params, 0.0, 0.0, base.dx, base.dy, 48, 48, base.bathy, base.eta0, cfl=0.9,
+                            ratios=(2,), flag=dict(tol_eta=0.1, buffer=2), regrid_interval=2, patch_max=24)
+    Lx = 48 * base.dx
+    pts = np.array([[x, y] for x in np.linspace(0.06, 0.94, 9) * Lx for y in (0.3 * Lx, 0.71 * Lx)])
+    G = driver.GaugeRecorder(pts)
+    H = driver.Hierarchy(gco.Context(**wl.params), wl, gauges=G)
+    owners0 = [len(ids) for ids, _ in G.assign]
+    assert len(H.levels) == 2 and owners0[1] > 0 and owners0[0] > 0              # some gauges start on the fine level, some on the coarse
+    ncoarse = H.run(nsteps=12)
+    assert H.regrids >= 5
+    fine_counts = []
+    for g in range(len(pts)):
+        S = G.series(g)
+        assert S[0, 0] == 0.0 and S[-1, 0] == H.t and (np.diff(S[:, 0]) >= 0).all()
+        assert ncoarse + 1 <= len(S) <= 2 * ncoarse + 1                       # once per step of the owning level (ratio 2), once at the end
+        assert (S[:, 1] >= 0.0).all() and np.isfinite(S).all()
+        fine_counts.append(len(S))
+    assert max(fine_counts) > ncoarse + 1                                     # a gauge spent time on the fine level
+    # the last record is a direct sample of the final state from the level that owns the gauge now
+    for k, L in enumerate(H.levels):
+        ids, pats = G.assign[k]
+        if ids:
+            L.fill_ghost(H.levels[k - 1] if k > 0 else None, 1.0)
+            now = L.gauges_sample(pats, pts[ids])
+            for n, g in enumerate(ids):
+                assert np.array_equal(G.series(g)[-1, 1:], now[n])
