@@ -160,6 +160,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--sweep", action="store_true", help="also report every tiling 16..256 in config.tilings")
+    ap.add_argument("--gauges", type=int, default=0,
+                    help="bind this many seeded gauges and record them into a device-resident series every step (DESIGN.md 3.10)")
     ap.add_argument("--manning", type=float, default=0.0,
                     help="Manning n of the friction step (DESIGN.md 3.9); 0 = off, as BASELINE.json's configs state no n")
     args = ap.parse_args()
@@ -196,16 +198,29 @@ def main():
     def timed(L, K, warm):
         dt0 = driver.probe_dt(L, wl.cfl)
         dt_dev = torch.tensor([dt0], dtype=torch.float64, device=dev)
-        for _ in range(warm):
-            L.fill_ghost(None, 1.0); L.step_auto(dt_dev, wl.cfl)
+        series = None
+        if args.gauges > 0:      # seeded points, each bound to the patch that holds it; one record per step, kept on the device
+            rng = np.random.default_rng(1901067985)
+            pts = np.stack([wl.xlo + rng.uniform(0.0, 1.0, args.gauges) * n * wl.dx * (1 - 1e-12),
+                            wl.ylo + rng.uniform(0.0, 1.0, args.gauges) * n * wl.dy * (1 - 1e-12)], axis=1)
+            L.gauges_bind([driver.GaugeRecorder.patch_of(L, x, y) for x, y in pts], pts)
+            series = torch.empty((max(K, warm), args.gauges, 4), dtype=torch.float64, device=dev)
+            torch.cuda.synchronize()
+        def one_step(k):
+            L.fill_ghost(None, 1.0)
+            if series is not None:
+                L.gauges_sample_into(series[k])      # one record per step, straight into the device-resident series
+            L.step_auto(dt_dev, wl.cfl)
+        for k in range(warm):
+            one_step(k)
         torch.cuda.synchronize()
         if dist: dist.barrier()
         torch.cuda.synchronize()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         lc0 = ctx.launch_count()
         e0.record()
-        for _ in range(K):
-            L.fill_ghost(None, 1.0); L.step_auto(dt_dev, wl.cfl)
+        for k in range(K):
+            one_step(k)
         e1.record()
         torch.cuda.synchronize()
         if dist: dist.barrier()
@@ -213,8 +228,8 @@ def main():
         launches = ctx.launch_count() - lc0
         # same K steps again with the library's per-kernel event brackets (separate pass: brackets perturb a little)
         ctx.profile(True)
-        for _ in range(K):
-            L.fill_ghost(None, 1.0); L.step_auto(dt_dev, wl.cfl)
+        for k in range(K):
+            one_step(k)
         prof = ctx.profile_read()
         ctx.profile(False)
         st = L.stats()
@@ -291,7 +306,7 @@ def main():
                                % (n, n, n // args.side, n // args.side, args.side),
                    "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (L.ncells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9 if L else 0),
                    "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl, "fmad": False,
-                   "manning_n": args.manning},
+                   "manning_n": args.manning, "gauges": args.gauges},
         "clocks": clocks,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 3 * cells * 8, "d2h_bytes_per_step": 3 * cells * 8 + 40,
                 "steps": Ke, "note": "state copied host->device and back every step through the C ABI (P:166 pipeline)"},
