@@ -103,6 +103,12 @@ int gc_level_create(gc_ctx *, int level, double xlo, double ylo, double dx, doub
 int gc_level_destroy(gc_level *);
 int64_t gc_level_ncells(const gc_level *);   /* interior cells of the level */
 
+/* Sets a field on every patch of the level at once, ghost cells included: one transfer and one kernel, against one
+ * gc_level_set_global per patch when a level is initialised patch by patch (every regrid).  src: for patch p = 0 .. np-1 in
+ * order, (ny_p + 4) rows of (nx_p + 4) doubles, x fastest, back to back (HOST or DEVICE; a host array is free on return).  Cells
+ * outside the level are not read; field GC_H..GC_B, written to the "new" buffer. */
+int gc_level_set_patches(gc_level *L, int field, const double *src, int src_is_device);
+
 /* Field transfer.  Per patch: arrays shaped like the storage, (ny+4) rows of (nx+4), leading dimension
  * ld (elements).  Global: the array covers global cells [gi0, gi0+gnx) x [gj0, gj0+gny) of the level with
  * leading dimension ld; set writes every storage cell (ghosts included) that falls inside, get reads

@@ -167,6 +167,16 @@ class Level:
         a = np.ascontiguousarray(arr, dtype=np.float64)
         _chk(lib().gco_level_set_global(self.h, FIELDS[field], a.ctypes.data, a.shape[1], gi0, gj0, a.shape[1], a.shape[0]), "set_global")
 
+    def set_patches(self, field, packed):
+        """the CUDA binding's call shape: every patch's storage-shaped block (ghost cells included), back to back"""
+        a = np.ascontiguousarray(packed, dtype=np.float64).ravel()
+        o = 0
+        for p, (i0, j0, nx, ny) in enumerate(self.patches):
+            n = (nx + 4) * (ny + 4)
+            self.set_field(p, field, a[o:o + n].reshape(ny + 4, nx + 4))
+            o += n
+        assert o == a.size
+
     def get_global(self, field, which=0, gi0=0, gj0=0, gnx=None, gny=None, fill=np.nan):
         gnx = self.nxl if gnx is None else gnx
         gny = self.nyl if gny is None else gny

@@ -17,7 +17,7 @@ SYMBOLS = [
     "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
-    "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample",
+    "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
 ]
 
 
@@ -65,6 +65,7 @@ def lib():
     L.gc_level_get_global.argtypes = [vp, i, i, vp, i, i64, i64, i64, i64, i64]
     L.gc_fill_ghost.argtypes = [vp, vp, d]
     L.gc_fill_ghost_b.argtypes = [vp]
+    L.gc_level_set_patches.argtypes = [vp, i, vp, i]
     L.gc_gauges_bind.argtypes = [vp, i, vp, vp]
     L.gc_gauges_sample.argtypes = [vp, vp, i]
     L.gc_level_step.argtypes = [vp, d, vp]
@@ -131,6 +132,12 @@ class Level:
         a, ptr, dev, ld = self._src(arr)
         self.ctx._chk(lib().gc_level_set_global(self.h, FIELDS[field], ptr, dev, ld, gi0, gj0, a.shape[1], a.shape[0]),
                       "gc_level_set_global")
+
+    def set_patches(self, field, packed):
+        """every patch at once: packed = for each patch in order its (ny + 4) x (nx + 4) block, ghost cells included, back to back"""
+        a = np.ascontiguousarray(packed, dtype=np.float64).ravel()
+        assert a.size == int(((self.patches[:, 2] + 4).astype(np.int64) * (self.patches[:, 3] + 4)).sum())
+        self.ctx._chk(lib().gc_level_set_patches(self.h, FIELDS[field], a.ctypes.data, 0), "gc_level_set_patches")
 
     def get_global(self, field, which=0, gi0=0, gj0=0, gnx=None, gny=None, fill=np.nan, out=None):
         gnx = self.nxl if gnx is None else gnx

@@ -414,6 +414,33 @@ extern "C" int gc_level_set_global(gc_level *L, int field, const double *src, in
     return gc_cuda_check(c, "gc_level_set_global");
 }
 
+extern "C" int gc_level_set_patches(gc_level *L, int field, const double *src, int is_device)
+{
+    if (!L || field < 0 || field > 3 || !src) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_set_patches: bad argument");
+    gc_ctx *c = L->ctx;
+    if (!L->d_goff) {                                 // packed layout: patch p starts at the sum of (nx + 4)(ny + 4) of the patches before it
+        std::vector<int64_t> goff((size_t)std::max(L->np, 1));
+        int64_t o = 0;
+        for (int p = 0; p < L->np; p++) { goff[(size_t)p] = o; o += (int64_t)(L->pat[p].nx + 4) * (L->pat[p].ny + 4); }
+        L->gtot = o;
+        L->d_goff = (int64_t *)gc_dev_alloc(c, goff.size() * sizeof(int64_t));
+        if (!L->d_goff) return gc_fail(c, GC_ERR_NOMEM, "gc_level_set_patches: table allocation failed");
+        L->allocs.push_back(L->d_goff);
+        cudaMemcpyAsync(L->d_goff, goff.data(), goff.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream);
+        cudaStreamSynchronize(c->stream);
+    }
+    const double *dsrc = src; double *tmp = nullptr; bool transient = false;
+    if (!is_device) {
+        tmp = (double *)gc_stage_get(c, (size_t)std::max<int64_t>(L->gtot, 1) * 8, &transient);
+        if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_level_set_patches: staging allocation failed");
+        cudaMemcpyAsync(tmp, src, (size_t)L->gtot * 8, cudaMemcpyHostToDevice, c->stream);
+        dsrc = tmp;
+    }
+    gc_launch_set_patches(L, plane_of(L, field, GC_NEW), L->d_goff, dsrc);
+    if (tmp) { cudaStreamSynchronize(c->stream); if (transient) gc_dev_free(c, tmp); }   // the caller's array is free on return
+    return gc_cuda_check(c, "gc_level_set_patches");
+}
+
 extern "C" int gc_level_get_global(const gc_level *L, int field, int which, double *dst, int is_device, int64_t ld,
                                    int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {

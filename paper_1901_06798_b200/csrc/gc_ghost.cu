@@ -104,6 +104,27 @@ __global__ void k_set_global(const PatchDesc *pat, double *plane, const double *
     }
 }
 
+// every patch at once from a packed source: patch p's (ny + 4) x (nx + 4) block, ghost cells included, starts at goff[p];
+// cells outside the level are left alone (the boundary fill owns them), as k_set_global leaves them
+__global__ void k_set_patches(const PatchDesc *pat, const int64_t *goff, double *plane, const double *src, int64_t nxl, int64_t nyl)
+{
+    const PatchDesc pd = pat[blockIdx.x];
+    const double *sp = src + goff[blockIdx.x];
+    const int W = pd.nx + 4;
+    const int n = W * (pd.ny + 4);
+    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+        const int j = t / W, i = t - j * W;
+        const int64_t gi = (int64_t)pd.i0 + i - 2, gj = (int64_t)pd.j0 + j - 2;
+        if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
+        plane[pd.off + (int64_t)j * pd.pitch + i] = sp[t];
+    }
+}
+void gc_launch_set_patches(gc_level *L, double *plane, const int64_t *goff, const double *src)
+{
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
+    if (L->np) k_set_patches<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, goff, plane, src, L->nxl, L->nyl);
+}
+
 __global__ void k_get_global(const PatchDesc *pat, const double *plane, double *dst, int64_t ld,
                              int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {

@@ -143,6 +143,7 @@ struct gc_level {
     // cached average-down list for a given fine level, cached neighbour lists for flag dilation
     uint64_t avg_gen; AvgRect *d_avg; int64_t *d_avgstart; int navg; int64_t navgcells;
     int nbr_buffer; int32_t *d_nbrstart, *d_nbrlist;
+    int64_t *d_goff = nullptr; int64_t gtot = 0;      // packed offsets of gc_level_set_patches (built at first use)
     GaugeLoc *d_gauge = nullptr; int ngauge = 0;     // gauges bound to this level (gc_gauges_bind)
 };
 
@@ -168,6 +169,7 @@ void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, in
 // gc_ghost.cu
 void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);
 void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int is_state);
+void gc_launch_set_patches(gc_level *L, double *plane, const int64_t *goff, const double *src);
 void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
 void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
 void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *src, int64_t sld, int w, int h);

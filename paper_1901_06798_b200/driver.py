@@ -35,16 +35,23 @@ def set_initial(L, wl, state=True):
         else:
             L.set_global("b", wl.bathy_box(L.dx, L.dy, 0, 0, L.nxl, L.nyl))
     else:
+        # every patch's storage-shaped block (its box grown by the ghost width; the part inside the level is filled) packed back to
+        # back and handed over in one call; cells outside the level stay 0 here and belong to the boundary fill
+        names = ("b", "h", "hu", "hv") if state else ("b",)
+        sizes = [(int(p[2]) + 4) * (int(p[3]) + 4) for p in pats]
+        packed = {f: np.zeros(int(np.sum(sizes, dtype=np.int64))) for f in names}
+        o = 0
         for p in range(len(pats)):
             i0, j0, nx, ny = (int(v) for v in pats[p])
             a0, a1 = max(i0 - 2, 0), min(i0 + nx + 2, L.nxl)
             c0, c1 = max(j0 - 2, 0), min(j0 + ny + 2, L.nyl)
-            if state:
-                b, h, hu, hv = wl.fields(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0)
-                L.set_global("b", b, a0, c0)
-                L.set_global("h", h, a0, c0); L.set_global("hu", hu, a0, c0); L.set_global("hv", hv, a0, c0)
-            else:
-                L.set_global("b", wl.bathy_box(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0), a0, c0)
+            vals = wl.fields(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0) if state else (wl.bathy_box(L.dx, L.dy, a0, c0, a1 - a0, c1 - c0),)
+            for f, v in zip(names, vals):
+                blk = packed[f][o:o + sizes[p]].reshape(ny + 4, nx + 4)
+                blk[c0 - (j0 - 2):c1 - (j0 - 2), a0 - (i0 - 2):a1 - (i0 - 2)] = v
+            o += sizes[p]
+        for f in names:
+            L.set_patches(f, packed[f])
     L.fill_ghost_b()
 
 

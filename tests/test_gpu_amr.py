@@ -158,6 +158,45 @@ def test_two_level_wet_dry_run_with_regrids(gc, gco, reflux):
     assert abs(Hg.composite_mass() - Ho.composite_mass()) <= 1e-13 * abs(Ho.composite_mass())
 
 
+def test_set_patches_and_patchwise_initialisation(gc, gco):
+    """gc_level_set_patches: every patch's storage-shaped block in one call.  Random data on a fine level whose patches touch the
+    domain edge and each other: every in-level cell of every patch, ghost cells included, takes its block's value, cells outside
+    the level are the boundary fill's.  Then driver.set_initial's patch-by-patch path (used at every regrid) on both backends."""
+    n, r = 32, 4
+    fine = np.array([[0, 0, 40, 32], [40, 0, 24, 56], [0, 32, 40, 24], [112, 116, 16, 12]], dtype=np.int32)   # two touch x = 0, y = 0; one the far corner
+    rng = np.random.default_rng(17)
+    levels = []
+    for b in (gc, gco):
+        ctx = b.Context(**PARAMS)
+        levels.append(ctx.level_create(2, 0.0, 0.0, 25.0, 25.0, n * r, n * r, r, fine))
+    Lg, Lo = levels
+    sizes = [(nx + 4) * (ny + 4) for _, _, nx, ny in fine]
+    for f in ("h", "hu", "hv", "b"):
+        packed = rng.uniform(0.5, 2.0, sum(sizes))
+        Lg.set_patches(f, packed); Lo.set_patches(f, packed)
+        o = 0
+        for p, (i0, j0, nx, ny) in enumerate(fine):
+            blk = packed[o:o + sizes[p]].reshape(ny + 4, nx + 4); o += sizes[p]
+            gi = i0 - 2 + np.arange(nx + 4); gj = j0 - 2 + np.arange(ny + 4)
+            inside = np.outer((gj >= 0) & (gj < n * r), (gi >= 0) & (gi < n * r))
+            got = Lg.get_field(p, f)
+            assert np.array_equal(got[inside], blk[inside]), (f, p)
+            assert np.array_equal(Lo.get_field(p, f)[inside], blk[inside]), (f, p)
+    # the initialisation path of every regrid: analytic bathymetry and state patch by patch, then the ghost fill of b
+    base = workloads.cfg2(n * r)
+    wl = workloads.Workload("fine", base.params, 0.0, 0.0, 25.0, 25.0, n * r, n * r, base.bathy, base.eta0)
+    assert Lg.nxl * Lg.nyl > 2 * Lg.ncells                                # the patch-by-patch branch
+    for L in (Lg, Lo):
+        driver.set_initial(L, wl, state=True)
+    same_storage(Lg, Lo, fields=("b", "h", "hu", "hv"))
+    x = (np.arange(n * r) + 0.5) * 25.0
+    X, Y = np.meshgrid(x, x)
+    want = np.asarray(base.bathy(X, Y))
+    got = Lg.get_global("b", fill=np.nan)
+    cov = ~np.isnan(got)
+    assert cov.sum() == Lg.ncells and np.array_equal(got[cov], want[cov])
+
+
 def test_two_level_run_with_manning_friction(gc, gco):
     """friction inside the AMR recursion: every level applies it after its own y-sweep with its own dt"""
     base = workloads.cfg2(48)

@@ -107,3 +107,52 @@ def test_config3_full_run(gc, gco):
           % (n, Ho.t, Ho.regrids, [int(L.ncells) for L in Ho.levels], worst))
     print("config 3 wall time inside Hierarchy.step (levels, regrids, average-down, fix-up): CUDA path %.2f s = %.3g updates/s; "
           "oracle on one host core %.1f s = %.3g updates/s" % (wall_g, Ho.updates / wall_g, wall_o, Ho.updates / wall_o))
+
+
+def lockstep_full(gc, gco, wl, ncoarse, every=1):
+    """both hierarchies step by step: dt, patch lists and wet masks every step, every patch's storage every `every` steps and at
+    the end, every flagging pass at the end; returns them with the wall time spent inside each side's step()"""
+    Hg = driver.Hierarchy(gc.Context(**wl.params), wl)
+    Ho = driver.Hierarchy(gco.Context(**wl.params), wl)
+    dtg, dto = Hg.probe(), Ho.probe()
+    wall_g = wall_o = 0.0
+    for n in range(ncoarse):
+        assert dtg == dto, (n, dtg, dto)
+        w0 = time.time(); dtg = Hg.step(dtg); w1 = time.time(); dto = Ho.step(dto); w2 = time.time()
+        wall_g += w1 - w0; wall_o += w2 - w1
+        assert len(Hg.levels) == len(Ho.levels)
+        for Lg, Lo in zip(Hg.levels, Ho.levels):
+            assert np.array_equal(Lg.patches, Lo.patches), n
+            assert np.array_equal(Lg.wet_mask(), Lo.wet_mask()), n
+        if n % every == every - 1 or n == ncoarse - 1:
+            for Lg, Lo in zip(Hg.levels, Ho.levels):
+                same_storage(Lg, Lo)
+    assert Hg.regrids == Ho.regrids and len(Hg.flag_log) == len(Ho.flag_log)
+    for (kg, tg, fg), (ko, to, fo) in zip(Hg.flag_log, Ho.flag_log):
+        assert kg == ko and tg == to and np.array_equal(fg, fo)
+    return Hg, Ho, wall_g, wall_o
+
+
+def test_config4_full_size_prefix(gc, gco):
+    """config 4 as BASELINE.json states it (1800 x 900 coarse at 4 arcmin, ratios 5, 6, 4): the first 6 coarse steps of the run --
+    the wave-following level 2 is regridded by level 1 twice and regrids itself after every 3 of its own steps"""
+    wl = workloads.cfg4()
+    assert (wl.nx, wl.ny) == (1800, 900) and tuple(wl.ratios) == (5, 6, 4)
+    Hg, Ho, wg, wo = lockstep_full(gc, gco, wl, 6, every=2)
+    assert len(Ho.levels) == 2 and Ho.regrids >= 10 and Ho.levels[1].ncells > 200000     # observed: 12 regrids, 474 450 fine cells
+    print("\nconfig 4 full size, 6 coarse steps to t = %.1f s: levels %s cells, %d regrids, %d flagging passes, %d updates; all identical. "
+          "Wall inside step(): CUDA path %.2f s = %.3g updates/s; oracle on one host core %.1f s = %.3g updates/s"
+          % (Ho.t, [int(L.ncells) for L in Ho.levels], Ho.regrids, len(Ho.flag_log), Ho.updates, wg, Ho.updates / wg, wo, Ho.updates / wo))
+
+
+def test_config4_full_size_four_levels(gc, gco):
+    """the same full-size hierarchy with the nested coastal boxes switched on from t = 0 instead of 6 h / 6.5 h, so that levels 3
+    and 4 (8 and 2 arcsec, straddling the shoreline) exist: one coarse step = 5 / 30 / 120 substeps of levels 2 / 3 / 4"""
+    wl = workloads.cfg4()
+    wl.forced_boxes = tuple((lv, x0, x1, y0, y1, 0.0, t1) for lv, x0, x1, y0, y1, t0, t1 in wl.forced_boxes)
+    Hg, Ho, wg, wo = lockstep_full(gc, gco, wl, 1)
+    assert len(Ho.levels) == 4
+    assert any(int(L.wet_mask().sum()) < L.ncells for L in Ho.levels[2:])          # the fine levels straddle the shoreline
+    print("\nconfig 4 full size with the coastal boxes on, 1 coarse step to t = %.1f s: levels %s cells, %d regrids, %d updates; all identical. "
+          "Wall inside step(): CUDA path %.2f s = %.3g updates/s; oracle on one host core %.1f s = %.3g updates/s"
+          % (Ho.t, [int(L.ncells) for L in Ho.levels], Ho.regrids, Ho.updates, wg, Ho.updates / wg, wo, Ho.updates / wo))
