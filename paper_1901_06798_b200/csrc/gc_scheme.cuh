@@ -201,8 +201,16 @@ __device__ __forceinline__ double gc_edge_cfl_std(const Waves &W, double rdL, do
 
 // ---- Manning friction (eq. 1b-1c, 2, reading S-16) -----------------------------------------
 // Cube root of a positive normal double by a fixed sequence (no library call, so that every compiler produces the same
-// bits): bit pattern / 3 + K as the seed (worst relative error 3.2 %), then three Halley steps.
-__device__ __forceinline__ double gc_cbrt(double x)
+// bits): bit pattern / 3 + K as the seed (worst relative error 3.2 %), then three Halley steps -- gc_cbrt_m below.
+
+// Semi-implicit fractional step of one cell over dt: hu, hv <- hu / d, hv / d with d = 1 + dt g n^2 |(hu, hv)| / h^(7/3)
+// (D of eq. 2 read over the momenta), for dry_tol < h <= friction_depth; gn2 = g * (n * n) formed by the host in that order.
+// Returns the new (hu, hv) by value (references would give the calling kernel a stack frame); out of line, so that the default
+// (friction off) path of the marching kernels keeps its registers.  M = MathFast: the six divides and the square root as the
+// branch-free correctly rounded sequences of gc_math.cuh (the two final divides share their reciprocal); operands outside
+// its window fall back to M = MathIeee.  Both give the oracle's bits.
+template <class M>
+__device__ __forceinline__ double gc_cbrt_m(M &m, double x)
 {
     unsigned long long i = (unsigned long long)__double_as_longlong(x);
     i = i / 3ull + 0x2A9F762500000000ull;
@@ -210,22 +218,25 @@ __device__ __forceinline__ double gc_cbrt(double x)
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         const double y3 = (y * y) * y;
-        y = y * ((y3 + 2.0 * x) / (2.0 * y3 + x));
+        y = y * m.div(y3 + 2.0 * x, 2.0 * y3 + x);
     }
     return y;
 }
-
-// Semi-implicit fractional step of one cell over dt: hu, hv <- hu / d, hv / d with d = 1 + dt g n^2 |(hu, hv)| / h^(7/3)
-// (D of eq. 2 read over the momenta), for dry_tol < h <= friction_depth; gn2 = g * (n * n) formed by the host in that order.
-// Returns d, or exactly 1 for a cell friction does not act on (x / 1 = x bit for bit, so the caller divides either way).
-#ifndef GC_FRICTION_INLINE
-#define GC_FRICTION_INLINE __noinline__
-#endif
-static __device__ GC_FRICTION_INLINE double gc_friction_d(double gn2, double eps, double fdepth, double dt, double h, double hu, double hv)
+template <class M>
+__device__ __forceinline__ double2 gc_friction_m(M &m, double gn2, double dt, double h, double hu, double hv)
 {
-    if (!(h > eps) || !(h <= fdepth)) return 1.0;
-    const double m = sqrt(hu * hu + hv * hv);
-    const double c = gc_cbrt(h);
-    const double gam = (gn2 * m) / ((h * h) * c);
-    return 1.0 + dt * gam;
+    const double mag = m.sqrt_(hu * hu + hv * hv);
+    const double c = gc_cbrt_m(m, h);
+    const double gam = m.div(gn2 * mag, (h * h) * c);
+    const double d = 1.0 + dt * gam;
+    return make_double2(m.div(hu, d), m.div(hv, d));
+}
+static __device__ __noinline__ double2 gc_friction_apply(double gn2, double eps, double fdepth, double dt, double h, double hu, double hv)
+{
+    if (!(h > eps) || !(h <= fdepth)) return make_double2(hu, hv);
+    MathFast mf;
+    const double2 q = gc_friction_m(mf, gn2, dt, h, hu, hv);
+    if (!mf.failed()) return q;
+    MathIeee mi;
+    return gc_friction_m(mi, gn2, dt, h, hu, hv);
 }

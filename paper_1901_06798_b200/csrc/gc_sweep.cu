@@ -155,8 +155,8 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
                 nh = dmax(nh, 0.0); np_ = 0.0; nt = 0.0;
             }
             if (a.friction && a.write_out) {                                                       // DESIGN.md 3.9; (hu, hv) = (nt, np_)
-                const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, nh, nt, np_);
-                nt = nt / d; np_ = np_ / d;
+                const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, dt, nh, nt, np_);
+                nt = q.x; np_ = q.y;
             }
             if (nh != nh || np_ != np_ || nt != nt) nanf = 1;
             if (a.write_out) { a.oh[idx] = nh; a.ohv[idx] = np_; a.ohu[idx] = nt; }
@@ -322,8 +322,8 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
                 }
                 if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
-                    const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
-                    ut = ut / d; up = up / d;
+                    const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
+                    ut = q.x; up = q.y;
                 }
                 if (uh != uh || up != up || ut != ut) nanf = 1;
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
@@ -576,8 +576,8 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
                 }
                 if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
-                    const double d = gc_friction_d(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
-                    ut = ut / d; up = up / d;
+                    const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
+                    ut = q.x; up = q.y;
                 }
                 if (uh != uh || up != up || ut != ut) nanf = 1;
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
