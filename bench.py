@@ -31,7 +31,7 @@ FP64_SLOTS_PER_SWEEP = {"xsweep": 386.0, "ysweep": 394.0}
 BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once; the two-pass design moves 112
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of each sweep kernel at the bench size 8192^2 / side 256, from the
 # ncu --set full capture summarised in profiles/r01_marchp.md (k_marchp; not valid for GC_MARCH=regs or GC_SWEEP=edge)
-NCU_TRAFFIC_BYTES = {"xsweep": 4.376e9, "ysweep": 3.907e9}
+NCU_TRAFFIC_BYTES = {"xsweep": 4.385e9, "ysweep": 3.906e9}
 METRIC = "fp64 cell updates/sec per level step (device-timed)"
 UNIT = "cell updates/s"
 
