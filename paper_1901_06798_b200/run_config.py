@@ -107,6 +107,8 @@ def main():
     ap.add_argument("--max-steps", type=int, default=None)
     ap.add_argument("--max-wall", type=float, default=None)
     ap.add_argument("--max-levels", type=int, default=None)
+    ap.add_argument("--boxes-from-start", action="store_true",
+                    help="config 4: switch the forced coastal boxes on at t = 0 instead of 6 h / 6.5 h, so that all four levels exist at once")
     ap.add_argument("--graph", type=int, default=0, help="single-level configs: replay the step as a CUDA graph of this many steps")
     ap.add_argument("--device", default="cuda:0")
     a = ap.parse_args()
@@ -122,7 +124,10 @@ def main():
         wl = workloads.cfg3(a.scale or 256); res = run_amr(3, wl, a.max_steps, a.max_wall, a.device, a.max_levels)
     else:
         nx = a.scale or 1800
-        wl = workloads.cfg4(nx, nx // 2); res = run_amr(4, wl, a.max_steps, a.max_wall, a.device, a.max_levels)
+        wl = workloads.cfg4(nx, nx // 2)
+        if a.boxes_from_start:
+            wl.forced_boxes = tuple((lv, x0, x1, y0, y1, 0.0, t1) for lv, x0, x1, y0, y1, t0, t1 in wl.forced_boxes)
+        res = run_amr(4, wl, a.max_steps, a.max_wall, a.device, a.max_levels)
     res.update(config=a.config, workload=wl.name, e2e_updates_per_s=res["updates"] / res["wall_s"], unit="cell updates/s")
     if "device_ms" in res:
         res["device_updates_per_s"] = res["updates"] / (res["device_ms"] * 1e-3)
