@@ -204,3 +204,47 @@ def test_cluster_covers_flags_with_disjoint_valid_boxes():
     assert cover.max() == 1 and (cover[fl] == 1).all()
     assert fl.sum() / (cover > 0).sum() > 0.5
     assert boxes == sorted(boxes, key=lambda b: (b[1], b[0]))
+
+
+def _run_hierarchy(gco, wl, n, **kw):
+    H = driver.Hierarchy(gco.Context(**wl.params), wl, **kw)
+    dts = []; dt = H.probe()
+    for _ in range(n):
+        dts.append(dt); dt = H.step(dt)
+    return H, dts
+
+
+@pytest.mark.parametrize("case", ["four_levels_fixed_boxes", "two_levels_wave_following", "three_levels", "four_levels_no_reflux"])
+def test_keeping_a_level_whose_regrid_reproduces_it_changes_no_bit(gco, monkeypatch, case):
+    """every ghost cell is rewritten before it is read (a level's ghost ring is refilled right after its own step, at
+    the new state's time), and the regrid transfer copies every interior cell of an unchanged level -- so a level whose regrid
+    reproduces its patch list may simply stay.  With the switch on and off: same dt sequence, same patch lists, same flagging passes,
+    every interior cell of every level identical."""
+    kw = {}
+    if case.startswith("four_levels"):
+        wl = workloads.cfg4(120, 60); wl.patch_max = 60
+        wl.forced_boxes = tuple((lv, x0, x1, y0, y1, 0.0, t1) for lv, x0, x1, y0, y1, t0, t1 in wl.forced_boxes)
+        n = 3
+        kw = dict(reflux=not case.endswith("no_reflux"))
+    elif case == "two_levels_wave_following":
+        base = workloads.cfg2(48)
+        wl = workloads.Workload("amr2", base.params, 0.0, 0.0, base.dx, base.dy, 48, 48, base.bathy, base.eta0, cfl=0.9,
+                                ratios=(2,), flag=dict(tol_eta=0.1, buffer=2), regrid_interval=2, patch_max=24)
+        n = 12
+    else:
+        base = workloads.cfg1(24)
+        wl = workloads.Workload("amr3", base.params, 0.0, 0.0, base.dx, base.dy, 24, 24, base.bathy, base.eta0, cfl=0.9,
+                                ratios=(2, 3), flag=dict(tol_eta=0.25, buffer=1), regrid_interval=2, patch_max=18)
+        n = 8
+    monkeypatch.setenv("GC_REGRID_KEEP", "1"); Ha, da = _run_hierarchy(gco, wl, n, **kw)
+    monkeypatch.setenv("GC_REGRID_KEEP", "0"); Hb, db = _run_hierarchy(gco, wl, n, **kw)
+    assert Hb.kept == 0 and da == db and Ha.regrids == Hb.regrids and len(Ha.levels) == len(Hb.levels)
+    if case.startswith("four_levels"):
+        assert Ha.kept >= 30 and len(Ha.levels) == 4                         # the fixed-box levels came back unchanged every time
+    for La, Lb in zip(Ha.levels, Hb.levels):
+        assert np.array_equal(La.patches, Lb.patches)
+        for f in ("h", "hu", "hv", "b"):
+            assert np.array_equal(La.get_global(f, fill=0.0), Lb.get_global(f, fill=0.0)), (case, La.level, f)
+    assert len(Ha.flag_log) == len(Hb.flag_log)
+    for (ka, ta, fa), (kb, tb, fb) in zip(Ha.flag_log, Hb.flag_log):
+        assert ka == kb and ta == tb and np.array_equal(fa, fb)
