@@ -4,6 +4,7 @@
 //
 // The paper keeps all of these on the CPU; here each is ONE launch over host-built work lists covering
 // every patch of the level, so the parallelism is O(perimeter) or O(cells), not O(patch side).
+#include <algorithm>
 #include "gc_internal.h"
 #include "gc_scheme.cuh"
 
@@ -179,13 +180,16 @@ void gc_launch_average_down(gc_level *C, const gc_level *F, const AvgRect *rects
 // ---- A10: flags.  Pass 1 (k_flag_raw): the criteria per interior cell.  Pass 2 (k_flag_dilate): a cell is flagged
 // if any raw-flagged cell of the level lies within `buffer` cells (Chebyshev distance): gather over the patch's
 // own cells and those of the neighbour patches listed by the host.  One block per patch.
+// grid = (patches, chunks of FLAG_CHUNK cells of a patch): a level that is one large patch spreads over the chip, not over one SM
+#define FLAG_CHUNK 4096
 __global__ void k_flag_raw(const PatchDesc *pat, const double *h, const double *b, double eps, double sea, double tol_eta,
                            double tol_slope, int offshore_only, int nboxes, const double *boxes, double t,
                            double xlo, double ylo, double dx, double dy, uint8_t *raw)
 {
     const PatchDesc pd = pat[blockIdx.x];
     const int n = pd.nx * pd.ny;
-    for (int q = threadIdx.x; q < n; q += blockDim.x) {
+    const int q1 = min(n, (int)(blockIdx.y + 1) * FLAG_CHUNK);
+    for (int q = (int)blockIdx.y * FLAG_CHUNK + threadIdx.x; q < q1; q += blockDim.x) {
         const int j = q / pd.nx, i = q - j * pd.nx;
         const int64_t c = pd.off + (int64_t)(j + 2) * pd.pitch + i + 2;
         const double hc = h[c], bc = b[c];
@@ -233,8 +237,9 @@ __global__ void k_flag_dilate(const PatchDesc *pat, const uint8_t *raw, uint8_t 
     const int p = blockIdx.x;
     const PatchDesc pd = pat[p];
     const int n = pd.nx * pd.ny;
+    const int q1 = min(n, (int)(blockIdx.y + 1) * FLAG_CHUNK);
     unsigned mine = 0;
-    for (int q = threadIdx.x; q < n; q += blockDim.x) {
+    for (int q = (int)blockIdx.y * FLAG_CHUNK + threadIdx.x; q < q1; q += blockDim.x) {
         const int j = q / pd.nx, i = q - j * pd.nx;
         const int64_t gi = (int64_t)pd.i0 + i, gj = (int64_t)pd.j0 + j;
         bool fl = raw[pd.ioff + q] != 0;
@@ -259,9 +264,12 @@ void gc_launch_flags(const gc_level *L, const gc_flag_params *fp, const double *
     if (L->np == 0) return;
     const gc_params &P = L->ctx->P;
     ProfScope ps(L->ctx, GC_SLOT_FLAG, 2);
-    k_flag_raw<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->b, P.dry_tol, P.sea_level, fp->tol_eta, fp->tol_slope,
+    int64_t maxn = 1;
+    for (const gc_patch &pp : L->pat) maxn = std::max<int64_t>(maxn, (int64_t)pp.nx * pp.ny);
+    const dim3 grid((unsigned)L->np, (unsigned)((maxn + FLAG_CHUNK - 1) / FLAG_CHUNK));
+    k_flag_raw<<<grid, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->b, P.dry_tol, P.sea_level, fp->tol_eta, fp->tol_slope,
                                                   fp->offshore_only, fp->nboxes, d_boxes, t, L->xlo, L->ylo, L->dx, L->dy, raw);
-    k_flag_dilate<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, raw, flags, fp->buffer > 0 ? fp->buffer : 0, nbr_start, nbr_list, d_count);
+    k_flag_dilate<<<grid, 256, 0, L->ctx->stream>>>(L->d_pat, raw, flags, fp->buffer > 0 ? fp->buffer : 0, nbr_start, nbr_list, d_count);
 }
 
 // ---- A8: flux registers.  The sweeps keep nothing per edge; a register re-derives the flux-like
