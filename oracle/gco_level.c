@@ -321,10 +321,10 @@ void gco_friction(const gco_params *P, double dt, double h, double *hu, double *
 {
     double m, c, gam, d;
     if (!(P->manning_n > 0.0) || !(h > P->dry_tol) || !(h <= P->friction_depth)) return;
-    m = sqrt((*hu) * (*hu) + (*hv) * (*hv));
+    m = sqrt(fma(*hu, *hu, (*hv) * (*hv)));
     c = gco_cbrt(h);
     gam = ((P->g * (P->manning_n * P->manning_n)) * m) / ((h * h) * c);
-    d = 1.0 + dt * gam;
+    d = fma(dt, gam, 1.0);
     *hu = *hu / d;
     *hv = *hv / d;
 }

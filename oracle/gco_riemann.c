@@ -14,6 +14,9 @@
 
 static double max2(double a, double b) { return a > b ? a : b; }
 static double min2(double a, double b) { return a < b ? a : b; }
+/* fma(a, b, c) = a*b + c with ONE rounding (C99 fma, correctly rounded by libm with or without hardware
+ * support), used at exactly the places DESIGN.md 3.3-3.4 write it; every other operation rounds on its own
+ * (-ffp-contract=off).  north_star: "both sides fp64, FMA contraction stated". */
 
 #define TAU 1.0e-6      /* critical-flow tolerance */
 #define SQRT_TAU 1.0e-3
@@ -36,25 +39,25 @@ void gco_middle_state(double g, double eps, double hL, double hR, double uL, dou
     double cmax = (hL > hR) ? cL : cR; /* = sqrt(g hmax) */
     if (hL == hR) { cmin = cL; cmax = cL; }
     double Fmin = du + 2.0 * (cmin - cmax);
-    double Fmax = du + (hmax - hmin) * sqrt(0.5 * g * (hmax + hmin) / (hmax * hmin));
+    double Fmax = fma(hmax - hmin, sqrt(0.5 * g * (hmax + hmin) / (hmax * hmin)), du);
     if (Fmin > 0.0) { /* two rarefactions: closed form */
         double cm = 0.25 * max2(0.0, 2.0 * (cL + cR) - du);
         *hm = cm * cm / g;
-        *s1m = (uL + 2.0 * cL) - 3.0 * cm;
-        *s2m = (uR - 2.0 * cR) + 3.0 * cm;
+        *s1m = fma(-3.0, cm, uL + 2.0 * cL);
+        *s2m = fma(3.0, cm, uR - 2.0 * cR);
     } else if (Fmax <= 0.0) { /* two shocks: one Newton step in sqrt(h) from hmax */
         double h0 = hmax;
         double gL = sqrt(0.5 * g * (1.0 / h0 + 1.0 / hL));
         double gR = sqrt(0.5 * g * (1.0 / h0 + 1.0 / hR));
-        double F0 = du + (h0 - hL) * gL + (h0 - hR) * gR;
+        double F0 = fma(h0 - hR, gR, fma(h0 - hL, gL, du));
         double dfdh = (gL - g * (h0 - hL) / (4.0 * (h0 * h0) * gL))
                     + (gR - g * (h0 - hR) / (4.0 * (h0 * h0) * gR));
         double sq0 = sqrt(h0);
         double slope = 2.0 * sq0 * dfdh;
         double sq = sq0 - F0 / slope;
         double h1 = sq * sq;
-        double u1m = uL - (h1 - hL) * sqrt(0.5 * g * (1.0 / h1 + 1.0 / hL));
-        double u2m = uR + (h1 - hR) * sqrt(0.5 * g * (1.0 / h1 + 1.0 / hR));
+        double u1m = fma(-(h1 - hL), sqrt(0.5 * g * (1.0 / h1 + 1.0 / hL)), uL);
+        double u2m = fma(h1 - hR, sqrt(0.5 * g * (1.0 / h1 + 1.0 / hR)), uR);
         double cm = sqrt(g * h1);
         *hm = h1;
         *s1m = u1m - cm;
@@ -64,10 +67,10 @@ void gco_middle_state(double g, double eps, double hL, double hR, double uL, dou
         double cm = sqrt(g * h1);
         *hm = h1;
         if (hL > hR) { /* 1-rarefaction on the deeper (left) side */
-            *s1m = (uL + 2.0 * cL) - 3.0 * cm;
+            *s1m = fma(-3.0, cm, uL + 2.0 * cL);
             *s2m = (uL + 2.0 * cL) - cm;
         } else {
-            *s2m = (uR - 2.0 * cR) + 3.0 * cm;
+            *s2m = fma(3.0, cm, uR - 2.0 * cR);
             *s1m = (uR - 2.0 * cR) + cm;
         }
     }
@@ -88,9 +91,9 @@ void gco_riemann(double g, double eps, double hL, double pL, double tL, double b
     /* R2 primitive variables per side */
     double uL, vL, phiL, cL, uR, vR, phiR, cR;
     if (hL <= eps) { hL = 0.0; pL = 0.0; tL = 0.0; uL = 0.0; vL = 0.0; phiL = 0.0; }
-    else { double rh = 1.0 / hL; uL = pL * rh; vL = tL * rh; phiL = pL * uL + 0.5 * g * (hL * hL); }
+    else { double rh = 1.0 / hL; uL = pL * rh; vL = tL * rh; phiL = fma(pL, uL, 0.5 * g * (hL * hL)); }
     if (hR <= eps) { hR = 0.0; pR = 0.0; tR = 0.0; uR = 0.0; vR = 0.0; phiR = 0.0; }
-    else { double rh = 1.0 / hR; uR = pR * rh; vR = tR * rh; phiR = pR * uR + 0.5 * g * (hR * hR); }
+    else { double rh = 1.0 / hR; uR = pR * rh; vR = tR * rh; phiR = fma(pR, uR, 0.5 * g * (hR * hR)); }
     cL = sqrt(g * hL);
     cR = sqrt(g * hR);
 
@@ -140,9 +143,9 @@ void gco_riemann(double g, double eps, double hL, double pL, double tL, double b
     double hbar = max2(0.5 * (hL + hR), 0.0);
     double ghbar = g * hbar;
     double su = uL + uR;
-    double pbar = 0.25 * (su * su) - ghbar;           /* \bar P */
+    double pbar = fma(0.25 * su, su, -ghbar);          /* \bar P */
     double ptil = max2(0.0, uL * uR) - ghbar;         /* \tilde P */
-    double hsd = max2(0.0, ((pL - pR) + l3 * hR) - l1 * hL); /* h*_HLL (l3 - l1) */
+    double hsd = max2(0.0, fma(-l1, hL, fma(l3, hR, pL - pR))); /* h*_HLL (l3 - l1) */
     int sonic = 0;
     if (fabs(pbar) <= TAU) sonic = 1;
     if (pbar * ptil <= TAU) sonic = 1;
@@ -184,9 +187,9 @@ void gco_riemann(double g, double eps, double hL, double pL, double tL, double b
     double d3 = (phiR - phiL) - dphi;
     double rdl = 1.0 / (l3 - l1);
     double l1sq = l1 * l1, l3sq = l3 * l3;
-    double b1 = (l3 * d1 - d2) * rdl;
-    double b3 = (d2 - l1 * d1) * rdl;
-    double b2 = (d3 - l1sq * b1) - l3sq * b3;
+    double b1 = fma(l3, d1, -d2) * rdl;
+    double b3 = fma(-l1, d1, d2) * rdl;
+    double b2 = fma(-l3sq, b3, fma(-l1sq, b1, d3));
 
     Z[0][0] = b1 * l1;  Z[0][1] = b1 * l1sq;  Z[0][2] = vL * Z[0][0];
     Z[2][0] = b3 * l3;  Z[2][1] = b3 * l3sq;  Z[2][2] = vR * Z[2][0];

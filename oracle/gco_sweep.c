@@ -5,7 +5,8 @@
  * Order of operations: (1) solve every edge 1..n+3; (2) scale by the edge factor; (3) fluctuations;
  * (4) limiter (eq. 10-11 with the reading S-1 theta = (Z_I . Z_e)/(Z_e . Z_e), MC limiter P:292);
  * (5) correction flux (eq. 9); (6) fm = F~ + A-dQ, fp = F~ - A+dQ; (7) update (eq. 8 / 13 / 14)
- *     Q_c <- Q_c - dt*rdx_c*(fm_{c+1} - fp_c); (8) CFL (eq. 15).
+ *     Q_c <- fma(-dt*rdx_c, fm_{c+1} - fp_c, Q_c); (8) CFL (eq. 15).
+ * fma(a, b, c) = a*b + c rounded once, at exactly the places DESIGN.md 3.4 writes it (C99 fma; -ffp-contract=off elsewhere).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -51,23 +52,26 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
     /* (4)-(6): limited second-order correction at edges 2..n+2 */
     for (e = 2; e <= n + 2; e++) {
         double F[3] = {0.0, 0.0, 0.0};
+        double T[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         if (P->limiter != 0) {
-            double dtdx_ave = 0.5 * (dt * rdx[e - 1] + dt * rdx[e]);
+            double dtdx_ave = 0.5 * fma(dt, rdx[e - 1], dt * rdx[e]);
             for (w = 0; w < 3; w++) {
                 double sw = s[e][w];
                 if (sw == 0.0) continue; /* sgn(0) = 0, S-4 */
-                double zz = (Z[e][w][0] * Z[e][w][0] + Z[e][w][1] * Z[e][w][1]) + Z[e][w][2] * Z[e][w][2];
+                double zz = fma(Z[e][w][2], Z[e][w][2], fma(Z[e][w][1], Z[e][w][1], Z[e][w][0] * Z[e][w][0]));
                 double phi = 1.0;
                 if (zz != 0.0) {
                     int I = (sw > 0.0) ? e - 1 : e + 1; /* eq. 11 */
-                    double zi = (Z[I][w][0] * Z[e][w][0] + Z[I][w][1] * Z[e][w][1]) + Z[I][w][2] * Z[e][w][2];
+                    double zi = fma(Z[I][w][2], Z[e][w][2], fma(Z[I][w][1], Z[e][w][1], Z[I][w][0] * Z[e][w][0]));
                     double theta = zi / zz; /* eq. 10, reading S-1 */
                     /* MC: max(0, min((1+theta)/2, 2, 2 theta)) */
                     phi = max2(0.0, min2(min2(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
                 }
-                double coef = ((sw > 0.0) ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
-                for (k = 0; k < 3; k++) F[k] = F[k] + coef * (phi * Z[e][w][k]);
+                double coef = ((sw > 0.0) ? 0.5 : -0.5) * fma(-fabs(sw), dtdx_ave, 1.0);
+                double cphi = coef * phi;
+                for (k = 0; k < 3; k++) T[w][k] = cphi * Z[e][w][k];
             }
+            for (k = 0; k < 3; k++) F[k] = (T[0][k] + T[2][k]) + T[1][k];
         }
         for (k = 0; k < 3; k++) {
             fm[e][k] = F[k] + am[e][k];
@@ -78,9 +82,9 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
     /* (7) update of cells 2..n+1 */
     for (c = 2; c <= n + 1; c++) {
         double dtdx = dt * rdx[c];
-        ho[c] = h[c] - dtdx * (fm[c + 1][0] - fp[c][0]);
-        po[c] = p[c] - dtdx * (fm[c + 1][1] - fp[c][1]);
-        to[c] = t[c] - dtdx * (fm[c + 1][2] - fp[c][2]);
+        ho[c] = fma(-dtdx, fm[c + 1][0] - fp[c][0], h[c]);
+        po[c] = fma(-dtdx, fm[c + 1][1] - fp[c][1], p[c]);
+        to[c] = fma(-dtdx, fm[c + 1][2] - fp[c][2], t[c]);
     }
 
     /* (8) CFL: right-going waves enter cell e, left-going waves enter cell e-1 */

@@ -2,8 +2,9 @@
 //
 // P:122 names the solver (George 2008, augmented system with topography and momentum flux) and its
 // properties; the steps R0-R8 implemented here are DESIGN.md section 3.3.  Every expression is
-// evaluated in the order DESIGN.md states (no FMA contraction: the library is built with -fmad=false;
-// '/' and sqrt are IEEE), so the result is bit-identical to a plain C evaluation.  Divides, reciprocals and
+// evaluated in the order DESIGN.md states: fused multiply-adds exactly where it writes fma(a, b, c) (__fma_rn here, C99
+// fma in the oracle), no contraction anywhere else (the library is built with -fmad=false), '/' and sqrt IEEE, so the
+// result is bit-identical to a plain C evaluation.  Divides, reciprocals and
 // square roots go through a math policy M (gc_math.cuh): MathIeee = the operators, MathFast = the same
 // correctly rounded results without a branch per operation (valid inside an exponent window, else M.failed()).
 #pragma once
@@ -28,7 +29,7 @@ __device__ __forceinline__ void gc_prim(M &m, RState &S, double g, double eps)
     } else {
         double rh = m.rcp(S.h);
         S.u = S.p * rh; S.v = S.t * rh;
-        S.phi = S.p * S.u + 0.5 * g * (S.h * S.h);
+        S.phi = __fma_rn(S.p, S.u, 0.5 * g * (S.h * S.h));
     }
     S.c = m.sqrt_(g * S.h);
 }
@@ -48,33 +49,33 @@ __device__ __forceinline__ void gc_middle(M &m, double g, double eps, double hL,
     double cmin = (hL < hR) ? cL : cR;
     double cmax = (hL < hR) ? cR : cL;
     double Fmin = du + 2.0 * (cmin - cmax);
-    double Fmax = du + (hmax - hmin) * m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin));
+    double Fmax = __fma_rn(hmax - hmin, m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin)), du);
     if (Fmin > 0.0) {                       // two rarefactions
         double cm = 0.25 * dmax(0.0, 2.0 * (cL + cR) - du);
         hm = m.div(cm * cm, g);
-        s1m = (uL + 2.0 * cL) - 3.0 * cm;
-        s2m = (uR - 2.0 * cR) + 3.0 * cm;
+        s1m = __fma_rn(-3.0, cm, uL + 2.0 * cL);
+        s2m = __fma_rn(3.0, cm, uR - 2.0 * cR);
     } else if (Fmax <= 0.0) {               // two shocks: one Newton step in sqrt(h) from hmax
         double h0 = hmax;
         double gL = m.sqrt_(0.5 * g * (m.rcp(h0) + m.rcp(hL)));
         double gR = m.sqrt_(0.5 * g * (m.rcp(h0) + m.rcp(hR)));
-        double F0 = du + (h0 - hL) * gL + (h0 - hR) * gR;
+        double F0 = __fma_rn(h0 - hR, gR, __fma_rn(h0 - hL, gL, du));
         double dfdh = (gL - m.div(g * (h0 - hL), 4.0 * (h0 * h0) * gL))
                     + (gR - m.div(g * (h0 - hR), 4.0 * (h0 * h0) * gR));
         double sq0 = m.sqrt_(h0);
         double slope = 2.0 * sq0 * dfdh;
         double sq = sq0 - m.div(F0, slope);
         double h1 = sq * sq;
-        double u1m = uL - (h1 - hL) * m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hL)));
-        double u2m = uR + (h1 - hR) * m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hR)));
+        double u1m = __fma_rn(-(h1 - hL), m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hL))), uL);
+        double u2m = __fma_rn(h1 - hR, m.sqrt_(0.5 * g * (m.rcp(h1) + m.rcp(hR))), uR);
         double cm = m.sqrt_(g * h1);
         hm = h1; s1m = u1m - cm; s2m = u2m + cm;
     } else {                                // shock + rarefaction: one secant step from hmin
         double h1 = hmin - m.div(Fmin * (hmax - hmin), Fmax - Fmin);
         double cm = m.sqrt_(g * h1);
         hm = h1;
-        if (hL > hR) { s1m = (uL + 2.0 * cL) - 3.0 * cm; s2m = (uL + 2.0 * cL) - cm; }
-        else         { s2m = (uR - 2.0 * cR) + 3.0 * cm; s1m = (uR - 2.0 * cR) + cm; }
+        if (hL > hR) { s1m = __fma_rn(-3.0, cm, uL + 2.0 * cL); s2m = (uL + 2.0 * cL) - cm; }
+        else         { s2m = __fma_rn(3.0, cm, uR - 2.0 * cR); s1m = (uR - 2.0 * cR) + cm; }
     }
 }
 
@@ -129,9 +130,9 @@ __device__ __forceinline__ void gc_riemann(M &m, double g, double eps, RState L,
     double hbar = dmax(0.5 * (L.h + R.h), 0.0);
     double ghbar = g * hbar;
     double su = L.u + R.u;
-    double pbar = 0.25 * (su * su) - ghbar;
+    double pbar = __fma_rn(0.25 * su, su, -ghbar);
     double ptil = dmax(0.0, L.u * R.u) - ghbar;
-    double hsd = dmax(0.0, ((L.p - R.p) + l3 * R.h) - l1 * L.h);
+    double hsd = dmax(0.0, __fma_rn(-l1, L.h, __fma_rn(l3, R.h, L.p - R.p)));
     bool sonic = false;
     if (fabs(pbar) <= GC_TAU) sonic = true;
     if (pbar * ptil <= GC_TAU) sonic = true;
@@ -173,9 +174,9 @@ __device__ __forceinline__ void gc_riemann(M &m, double g, double eps, RState L,
     double d3 = (R.phi - L.phi) - dphi;
     double rdl = m.rcp(l3 - l1);
     double l1sq = l1 * l1, l3sq = l3 * l3;
-    double b1 = (l3 * d1 - d2) * rdl;
-    double b3 = (d2 - l1 * d1) * rdl;
-    double b2 = (d3 - l1sq * b1) - l3sq * b3;
+    double b1 = __fma_rn(l3, d1, -d2) * rdl;
+    double b3 = __fma_rn(-l1, d1, d2) * rdl;
+    double b2 = __fma_rn(-l3sq, b3, __fma_rn(-l1sq, b1, d3));
 
     Z[0][0] = b1 * l1; Z[0][1] = b1 * l1sq; Z[0][2] = L.v * Z[0][0];
     Z[2][0] = b3 * l3; Z[2][1] = b3 * l3sq; Z[2][2] = R.v * Z[2][0];
@@ -200,7 +201,7 @@ __device__ __forceinline__ void gc_prim_fast(MathFast &m, RState &S, double g, d
     const double hs = wet ? S.h : 1.0;
     const double rh = m.rcp(hs);
     const double u = S.p * rh, v = S.t * rh;
-    const double phi = S.p * u + 0.5 * g * (S.h * S.h);
+    const double phi = __fma_rn(S.p, u, 0.5 * g * (S.h * S.h));
     S.h = wet ? S.h : 0.0; S.p = wet ? S.p : 0.0; S.t = wet ? S.t : 0.0;
     S.u = wet ? u : 0.0; S.v = wet ? v : 0.0; S.phi = wet ? phi : 0.0;
     S.c = m.sqrt_(g * S.h);
@@ -225,14 +226,14 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double du = R.u - L.u;
     const double cmin = shalL ? cL : cR;
     const double cmax = shalL ? cR : cL;
-    const double Fmin = du + 2.0 * (cmin - cmax);
-    const double Fmax = du + (hmax - hmin) * m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin));
+    const double Fmin = __fma_rn(2.0, cmin - cmax, du);                 // = du + 2 (cmin - cmax) bit for bit (x 2 is exact)
+    const double Fmax = __fma_rn(hmax - hmin, m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin)), du);
     ok = ok && !(Fmin > 0.0) && !(Fmax <= 0.0);
     const double h1 = hmin - m.div(Fmin * (hmax - hmin), Fmax - Fmin);
     const double cm = m.sqrt_(g * h1);
-    const double aL = L.u + 2.0 * cL, aR = R.u - 2.0 * cR;
-    const double s1m = deepL ? (aL - 3.0 * cm) : (aR + cm);
-    const double s2m = deepL ? (aL - cm) : (aR + 3.0 * cm);
+    const double aL = __fma_rn(2.0, cL, L.u), aR = __fma_rn(-2.0, cR, R.u);   // = u + 2c, u - 2c bit for bit
+    const double s1m = deepL ? __fma_rn(-3.0, cm, aL) : (aR + cm);
+    const double s2m = deepL ? (aL - cm) : __fma_rn(3.0, cm, aR);
     // R6
     const double l1 = dmin(sE1, s2m);
     const double l3 = dmax(sE2, s1m);
@@ -242,9 +243,9 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double hbar = dmax(0.5 * (hL + hR), 0.0);
     const double ghbar = g * hbar;
     const double su = L.u + R.u;
-    const double pbar = 0.25 * (su * su) - ghbar;
+    const double pbar = __fma_rn(0.25 * su, su, -ghbar);
     const double ptil = dmax(0.0, L.u * R.u) - ghbar;
-    const double hsd = dmax(0.0, ((L.p - R.p) + l3 * hR) - l1 * hL);
+    const double hsd = dmax(0.0, __fma_rn(-l1, hL, __fma_rn(l3, hR, L.p - R.p)));
     bool sonic = fabs(pbar) <= GC_TAU;
     sonic = sonic || (pbar * ptil <= GC_TAU);
     sonic = sonic || (pbar * l1 * l3 <= GC_TAU);
@@ -276,9 +277,9 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double d3 = (R.phi - L.phi) - dphi;
     const double rdl = m.rcp(l3 - l1);
     const double l1sq = l1 * l1, l3sq = l3 * l3;
-    const double b1 = (l3 * d1 - d2) * rdl;
-    const double b3 = (d2 - l1 * d1) * rdl;
-    const double b2 = (d3 - l1sq * b1) - l3sq * b3;
+    const double b1 = __fma_rn(l3, d1, -d2) * rdl;
+    const double b3 = __fma_rn(-l1, d1, d2) * rdl;
+    const double b2 = __fma_rn(-l3sq, b3, __fma_rn(-l1sq, b1, d3));
     Z[0][0] = b1 * l1; Z[0][1] = b1 * l1sq; Z[0][2] = L.v * Z[0][0];
     Z[2][0] = b3 * l3; Z[2][1] = b3 * l3sq; Z[2][2] = R.v * Z[2][0];
     Z[1][0] = 0.0;     Z[1][1] = b2;        Z[1][2] = ((R.p * R.v - L.p * L.v) - Z[0][2]) - Z[2][2];

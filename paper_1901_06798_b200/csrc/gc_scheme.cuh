@@ -4,7 +4,8 @@
 // P:65-105 (eqs. 4-11) in f-wave form; (1) Riemann solve (gc_riemann.cuh), (2) edge scaling
 // on the sphere, (3) fluctuations A-dQ / A+dQ (eq. 5-6, tie S-4), (4) MC-limited waves
 // (eq. 10-11, S-1), (5) correction flux (eq. 9), (6) fm = F~ + A-dQ, fp = F~ - A+dQ.
-// Every expression is written in the order of DESIGN.md so that, with -fmad=false, all users get the same bits.
+// Every expression is written in the order of DESIGN.md -- fused multiply-adds exactly where it writes fma (__fma_rn), no
+// contraction elsewhere (-fmad=false) -- so that all users get the same bits.
 #pragma once
 #include "gc_riemann.cuh"
 
@@ -41,7 +42,7 @@ __device__ __forceinline__ void gc_solve_edge(M &m, double g, double eps, RState
 __device__ __forceinline__ void gc_wave_dots(const Waves &A, const Waves &B, double (&d)[3])
 {
 #pragma unroll
-    for (int w = 0; w < 3; w++) d[w] = (A.Z[w][0] * B.Z[w][0] + A.Z[w][1] * B.Z[w][1]) + A.Z[w][2] * B.Z[w][2];
+    for (int w = 0; w < 3; w++) d[w] = __fma_rn(A.Z[w][2], B.Z[w][2], __fma_rn(A.Z[w][1], B.Z[w][1], A.Z[w][0] * B.Z[w][0]));
 }
 
 // MC limiter value for one family: zi = Z_I . Z_e, zz = Z_e . Z_e (zz != 0)
@@ -49,7 +50,7 @@ template <class M>
 __device__ __forceinline__ double gc_mc(M &m, double zi, double zz)
 {
     double theta = m.div(zi, zz);                                                    // eq. 10 (S-1)
-    return dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));        // MC
+    return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));  // MC; fma(.5, t, .5) = .5 (1 + t) bit for bit
 }
 
 // (3)-(6) for edge e.  dlo[w] = Z_{e-1}^w . Z_e^w, dhi[w] = Z_{e+1}^w . Z_e^w (eq. 11: I = e-1 if s > 0, e+1 if s < 0).
@@ -59,6 +60,7 @@ __device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double 
                                              double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
 {
     double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
+    double T[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
 #pragma unroll
     for (int w = 0; w < 3; w++) {
 #pragma unroll
@@ -69,19 +71,21 @@ __device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double 
         }
     }
     if (limiter != 0) {
-        double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+        double dtdx_ave = 0.5 * __fma_rn(dt, rdL, dt * rdR);
 #pragma unroll
         for (int w = 0; w < 3; w++) {
             double sw = W.s[w];
             if (sw != 0.0) {
-                double zz = (W.Z[w][0] * W.Z[w][0] + W.Z[w][1] * W.Z[w][1]) + W.Z[w][2] * W.Z[w][2];
+                double zz = __fma_rn(W.Z[w][2], W.Z[w][2], __fma_rn(W.Z[w][1], W.Z[w][1], W.Z[w][0] * W.Z[w][0]));
                 double phi = 1.0;
                 if (zz != 0.0) phi = gc_mc(m, (sw > 0.0) ? dlo[w] : dhi[w], zz);
-                double coef = ((sw > 0.0) ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
+                double cphi = (((sw > 0.0) ? 0.5 : -0.5) * __fma_rn(-fabs(sw), dtdx_ave, 1.0)) * phi;
 #pragma unroll
-                for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[w][c]);   // eq. 9
+                for (int c = 0; c < 3; c++) T[w][c] = cphi * W.Z[w][c];               // eq. 9, one family
             }
         }
+#pragma unroll
+        for (int c = 0; c < 3; c++) F[c] = (T[0][c] + T[2][c]) + T[1][c];             // outer families first: mirror-symmetric
     }
 #pragma unroll
     for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
@@ -99,13 +103,19 @@ __device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double
     return m;
 }
 
-// (3)-(6) without control flow (same values as gc_edge_flux: a skipped term is added as +0.0, which changes no bit
-// because the sums start at +0.0 and can therefore never be -0.0).  m.failed() afterwards: redo with gc_edge_flux.
+// (3)-(6) without control flow (same values as gc_edge_flux: a skipped family contributes +0.0 to the fluctuations, whose sums
+// start at +0.0 and can therefore never be -0.0, and T = +0.0 to the correction, exactly what gc_edge_flux leaves there).
+// m.failed() afterwards: redo with gc_edge_flux.
+__device__ __forceinline__ double gc_mc_fast(double theta)
+{
+    return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));                      // MC
+}
 __device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
                                                   double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
 {
     double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
-    const double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+    double T[3][3];
+    const double dtdx_ave = 0.5 * __fma_rn(dt, rdL, dt * rdR);
 #pragma unroll
     for (int w = 0; w < 3; w++) {
         const double sw = W.s[w];
@@ -117,16 +127,19 @@ __device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, c
             ap[c] = ap[c] + (pos ? z : (neg ? 0.0 : hz));
         }
         if (limiter != 0) {
-            const double zz = (W.Z[w][0] * W.Z[w][0] + W.Z[w][1] * W.Z[w][1]) + W.Z[w][2] * W.Z[w][2];
+            const double zz = __fma_rn(W.Z[w][2], W.Z[w][2], __fma_rn(W.Z[w][1], W.Z[w][1], W.Z[w][0] * W.Z[w][0]));
             const bool nz = zz != 0.0;
             const double theta = m.div(pos ? dlo[w] : dhi[w], nz ? zz : 1.0);                       // eq. 10 (S-1), eq. 11
-            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));          // MC
-            const double phi = nz ? mc : 1.0;
-            const double coef = (pos ? 0.5 : -0.5) * (1.0 - fabs(sw) * dtdx_ave);
+            const double phi = nz ? gc_mc_fast(theta) : 1.0;
+            const double cphi = ((pos ? 0.5 : -0.5) * __fma_rn(-fabs(sw), dtdx_ave, 1.0)) * phi;
             const bool on = neg || pos;                                                              // sgn(0) = 0 (S-4)
 #pragma unroll
-            for (int c = 0; c < 3; c++) { const double t = coef * (phi * W.Z[w][c]); F[c] = F[c] + (on ? t : 0.0); }   // eq. 9
+            for (int c = 0; c < 3; c++) T[w][c] = on ? cphi * W.Z[w][c] : 0.0;                       // eq. 9, one family
         }
+    }
+    if (limiter != 0) {
+#pragma unroll
+        for (int c = 0; c < 3; c++) F[c] = (T[0][c] + T[2][c]) + T[1][c];
     }
 #pragma unroll
     for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
@@ -135,8 +148,8 @@ __device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, c
 // (3)-(6) for a "standard" edge: s[0] < 0 < s[2] is known (every edge solved by gc_riemann_fast: l1 < -tau, l3 > tau, and
 // the edge factor is positive), so families 1 and 3 need no sign tests; only the corrector family 2 keeps them.
 // Same values as gc_edge_flux: the sums are formed in the same order, a skipped term is added as +0.0 (no bit changes:
-// the partial sums start at +0.0 and are therefore never -0.0), |s0| = -s0 exactly, Z[1][0] is +0.0 by construction.
-// m.failed() afterwards: redo with gc_edge_flux.
+// the partial sums start at +0.0 and are therefore never -0.0), -|s0| = s0 exactly, Z[1][0] is +0.0 by construction (so its
+// square drops out of zz: fma(x, x, +0) = fl(x x) for every x).  m.failed() afterwards: redo with gc_edge_flux.
 __device__ __forceinline__ void gc_edge_flux_std(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
                                                  double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
 {
@@ -152,37 +165,34 @@ __device__ __forceinline__ void gc_edge_flux_std(MathFast &m, const Waves &W, co
         ap[c] = (0.0 + (pos1 ? z : (neg1 ? 0.0 : hz))) + W.Z[2][c];
     }
     if (limiter != 0) {
-        const double dtdx_ave = 0.5 * (dt * rdL + dt * rdR);
+        const double dtdx_ave = 0.5 * __fma_rn(dt, rdL, dt * rdR);
+        double c0, c1, c2;
         {   // family 1: s < 0, upwind neighbour e+1
-            const double zz = (W.Z[0][0] * W.Z[0][0] + W.Z[0][1] * W.Z[0][1]) + W.Z[0][2] * W.Z[0][2];
+            const double zz = __fma_rn(W.Z[0][2], W.Z[0][2], __fma_rn(W.Z[0][1], W.Z[0][1], W.Z[0][0] * W.Z[0][0]));
             const bool nz = zz != 0.0;
             const double theta = m.div(dhi[0], nz ? zz : 1.0);
-            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
-            const double phi = nz ? mc : 1.0;
-            const double coef = -0.5 * (1.0 - (-s0) * dtdx_ave);
-#pragma unroll
-            for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[0][c]);
+            const double phi = nz ? gc_mc_fast(theta) : 1.0;
+            c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * phi;
         }
         {   // family 2: either sign, sgn(0) = 0
-            const double zz = (W.Z[1][0] * W.Z[1][0] + W.Z[1][1] * W.Z[1][1]) + W.Z[1][2] * W.Z[1][2];
+            const double zz = __fma_rn(W.Z[1][2], W.Z[1][2], W.Z[1][1] * W.Z[1][1]);
             const bool nz = zz != 0.0;
             const double theta = m.div(pos1 ? dlo[1] : dhi[1], nz ? zz : 1.0);
-            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
-            const double phi = nz ? mc : 1.0;
-            const double coef = (pos1 ? 0.5 : -0.5) * (1.0 - fabs(s1) * dtdx_ave);
-            const bool on = neg1 || pos1;
-#pragma unroll
-            for (int c = 0; c < 3; c++) { const double t = coef * (phi * W.Z[1][c]); F[c] = F[c] + (on ? t : 0.0); }
+            const double phi = nz ? gc_mc_fast(theta) : 1.0;
+            c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * phi;
         }
         {   // family 3: s > 0, upwind neighbour e-1
-            const double zz = (W.Z[2][0] * W.Z[2][0] + W.Z[2][1] * W.Z[2][1]) + W.Z[2][2] * W.Z[2][2];
+            const double zz = __fma_rn(W.Z[2][2], W.Z[2][2], __fma_rn(W.Z[2][1], W.Z[2][1], W.Z[2][0] * W.Z[2][0]));
             const bool nz = zz != 0.0;
             const double theta = m.div(dlo[2], nz ? zz : 1.0);
-            const double mc = dmax(0.0, dmin(dmin(0.5 * (1.0 + theta), 2.0), 2.0 * theta));
-            const double phi = nz ? mc : 1.0;
-            const double coef = 0.5 * (1.0 - s2 * dtdx_ave);
+            const double phi = nz ? gc_mc_fast(theta) : 1.0;
+            c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * phi;
+        }
+        const bool on = neg1 || pos1;
 #pragma unroll
-            for (int c = 0; c < 3; c++) F[c] = F[c] + coef * (phi * W.Z[2][c]);
+        for (int c = 0; c < 3; c++) {
+            const double t1 = c1 * W.Z[1][c];
+            F[c] = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + (on ? t1 : 0.0);                              // eq. 9
         }
     }
 #pragma unroll
@@ -225,10 +235,10 @@ __device__ __forceinline__ double gc_cbrt_m(M &m, double x)
 template <class M>
 __device__ __forceinline__ double2 gc_friction_m(M &m, double gn2, double dt, double h, double hu, double hv)
 {
-    const double mag = m.sqrt_(hu * hu + hv * hv);
+    const double mag = m.sqrt_(__fma_rn(hu, hu, hv * hv));
     const double c = gc_cbrt_m(m, h);
     const double gam = m.div(gn2 * mag, (h * h) * c);
-    const double d = 1.0 + dt * gam;
+    const double d = __fma_rn(dt, gam, 1.0);
     return make_double2(m.div(hu, d), m.div(hv, d));
 }
 static __device__ __noinline__ double2 gc_friction_apply(double gn2, double eps, double fdepth, double dt, double h, double hu, double hv)

@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
 #pragma unroll
         for (int w = 0; w < 3; w++) {
             const int kn = (s[w] > 0.0) ? k - dk : k + dk;
-            zi[w] = (sZ[3 * w + 0][kn] * Z[w][0] + sZ[3 * w + 1][kn] * Z[w][1]) + sZ[3 * w + 2][kn] * Z[w][2];
+            zi[w] = __fma_rn(sZ[3 * w + 2][kn], Z[w][2], __fma_rn(sZ[3 * w + 1][kn], Z[w][1], sZ[3 * w + 0][kn] * Z[w][0]));
         }
         bool done = false;
         if (stdE) { MathFast mf; gc_edge_flux_std(mf, W, zi, zi, a.limiter, dt, rdL, rdR, fm, fp); done = !mf.failed(); }
@@ -144,9 +144,9 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
     if (limited && e <= ne - 3) {             // thread <-> cell ce: Q_c <- Q_c - dt rdx_c (fm_{c+1} - fp_c)
         double dtdx = dt * rdR;
         int kr = k + dk;
-        double nh = qh - dtdx * (sF[0][kr] - fp[0]);
-        double np_ = qp - dtdx * (sF[1][kr] - fp[1]);
-        double nt = qt - dtdx * (sF[2][kr] - fp[2]);
+        double nh = __fma_rn(-dtdx, sF[0][kr] - fp[0], qh);
+        double np_ = __fma_rn(-dtdx, sF[1][kr] - fp[1], qp);
+        double nt = __fma_rn(-dtdx, sF[2][kr] - fp[2], qt);
         if (DIR == 0) {
             a.oh[idx] = nh; a.ohu[idx] = np_; a.ohv[idx] = nt;
         } else {
@@ -310,9 +310,9 @@ __global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
         if (live && r >= 3 && count) cflm = dmax(cflm, stdc ? gc_edge_cfl_std(Wc, rd2, rd1) : gc_edge_cfl(Wc, rd2, rd1));
         if (live && r >= 4) {                                                           // cell r-2
             const double dtdx = dt * rd2;
-            double uh = q2h - dtdx * (fm[0] - fpp[0]);
-            double up = q2p - dtdx * (fm[1] - fpp[1]);
-            double ut = q2t - dtdx * (fm[2] - fpp[2]);
+            double uh = __fma_rn(-dtdx, fm[0] - fpp[0], q2h);
+            double up = __fma_rn(-dtdx, fm[1] - fpp[1], q2p);
+            double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q2t);
             const int64_t o = base + (int64_t)(r - 2) * str;
             if (DIR == 0) {
                 a.oh[o] = uh; a.ohu[o] = up; a.ohv[o] = ut;
@@ -548,9 +548,9 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         sts2(sm0 + 7 * PK_SL, fp[0], fp[1]); sts2(sm0 + 8 * PK_SL, fp[2], 0.0);
         if (live && r >= 4) {                                                           // cell r-2
             const double dtdx = dt * rd2;
-            double uh = q2h - dtdx * (fm[0] - fpp[0]);
-            double up = q2p - dtdx * (fm[1] - fpp[1]);
-            double ut = q2t - dtdx * (fm[2] - fpp[2]);
+            double uh = __fma_rn(-dtdx, fm[0] - fpp[0], q2h);
+            double up = __fma_rn(-dtdx, fm[1] - fpp[1], q2p);
+            double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q2t);
             const int64_t o = base + (int64_t)(r - 2) * str;
             if (DIR == 0) {
                 // cell j = r-2 of the row goes to slot (plane, (j >> 1) & 1); a full aligned group of 4 leaves as one store
