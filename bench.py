@@ -297,7 +297,7 @@ def main():
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
     slot_frac = FP64_SLOTS_PER_SWEEP.get(dom, 394.0) * per_launch / (dom_ms * 1e-3) / slot_peak
-    default_kernels = os.environ.get("GC_MARCH") != "regs" and os.environ.get("GC_SWEEP") != "edge"
+    default_kernels = True
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

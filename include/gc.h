@@ -19,8 +19,9 @@
  *    SoA planes h, hu, hv (two buffers each: "new" = current, "old" = previous step) and b.
  *  - Indices are 0-based global cell indices of the level; patches must not overlap; for level > 1
  *    patch boxes are aligned to coarse cells (i0, j0, nx, ny multiples of ratio_to_coarser).
- *  - fp64 throughout; device code is compiled with -fmad=false and uses IEEE divide / sqrt, so results
- *    are bit-identical to a plain C evaluation of DESIGN.md section 3 in the stated order.
+ *  - fp64 throughout; fused multiply-adds exactly where DESIGN.md section 3 writes fma(a, b, c), no contraction anywhere
+ *    else (-fmad=false), correctly rounded divide / sqrt: results are bit-identical to a plain C evaluation of
+ *    DESIGN.md section 3 in the stated order.
  */
 #ifndef GC_H
 #define GC_H
@@ -92,6 +93,12 @@ int gc_ctx_create(const gc_params *params /*HOST*/, void *cuda_stream, gc_alloc_
                   void *user, gc_ctx **out);
 int gc_ctx_destroy(gc_ctx *);
 const char *gc_last_error(const gc_ctx *);
+/* Tuning knobs; none changes a result bit (all sweep kernel families compute the same bits).  Read when a level
+ * is created.  GC_OPT_SWEEP_FAMILY: 0 = by level size (default), 1 = edge-parallel tiles, 2 = line marching.
+ * GC_OPT_MARCH_SEG: cells per marching segment, 4..4096 (rounded down to a multiple of 4); 0 = by level size (default).
+ * Unknown key or value out of range: GC_ERR_BADARG, nothing changes. */
+enum { GC_OPT_SWEEP_FAMILY = 0, GC_OPT_MARCH_SEG = 1 };
+int gc_ctx_set_option(gc_ctx *, int key, int64_t value);
 
 /* A1: one level = one device pool with all its patches, a patch-descriptor table,
  * per-row metric tables and the host-built work lists for ghost filling.  level is 1-based; level 1

@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("GC_LIB", os.path.join(_HERE, "libgeoclaw_b200.so"))   # GC_LIB: an alternative build of the same library
+LIB_PATH = os.path.join(_HERE, "libgeoclaw_b200.so")
 
 SYMBOLS = [
     "gc_ctx_create", "gc_ctx_destroy", "gc_last_error", "gc_level_create", "gc_level_destroy", "gc_level_ncells",
@@ -18,6 +18,7 @@ SYMBOLS = [
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
+    "gc_ctx_set_option",
 ]
 
 
@@ -55,6 +56,7 @@ def lib():
     vp, i, d, i64 = C.c_void_p, C.c_int, C.c_double, C.c_int64
     L.gc_ctx_create.argtypes = [vp, vp, ALLOC_FN, FREE_FN, vp, vp]
     L.gc_ctx_destroy.argtypes = [vp]
+    L.gc_ctx_set_option.argtypes = [vp, i, i64]
     L.gc_last_error.argtypes = [vp]; L.gc_last_error.restype = C.c_char_p
     L.gc_level_create.argtypes = [vp, i, d, d, d, d, i64, i64, i, i, vp, vp]
     L.gc_level_destroy.argtypes = [vp]
@@ -228,6 +230,11 @@ class Level:
         self.ctx._chk(lib().gc_flux_fixup(self.h, fine.h), "gc_flux_fixup")
 
 
+OPT_SWEEP_FAMILY, OPT_MARCH_SEG = 0, 1          # gc_ctx_set_option keys (include/gc.h)
+SWEEP_AUTO, SWEEP_EDGE, SWEEP_MARCH = 0, 1, 2
+DEFAULT_OPTIONS = {}                            # applied to every new Context (tests select a sweep kernel family here)
+
+
 class Context:
     """The CUDA backend: Context(**params).level_create(...) -> Level.  Device memory comes from torch."""
     name = "b200"
@@ -255,6 +262,12 @@ class Context:
         if rc != 0:
             raise RuntimeError("gc_ctx_create failed: %d" % rc)
         self.h = h
+        for key, value in DEFAULT_OPTIONS.items():
+            self.set_option(key, value)
+
+    def set_option(self, key, value):
+        """gc_ctx_set_option: tuning knobs that change no result bit (OPT_SWEEP_FAMILY, OPT_MARCH_SEG); read at level creation."""
+        self._chk(lib().gc_ctx_set_option(self.h, int(key), C.c_int64(int(value))), "gc_ctx_set_option")
 
     def _alloc(self, nbytes, user):
         try:

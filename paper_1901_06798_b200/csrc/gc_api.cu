@@ -75,6 +75,14 @@ extern "C" int gc_ctx_destroy(gc_ctx *c)
     return GC_OK;
 }
 
+extern "C" int gc_ctx_set_option(gc_ctx *c, int key, int64_t value)
+{
+    if (!c) return GC_ERR_BADARG;
+    if (key == GC_OPT_SWEEP_FAMILY && value >= 0 && value <= 2) { c->opt_family = (int)value; return GC_OK; }
+    if (key == GC_OPT_MARCH_SEG && (value == 0 || (value >= 4 && value <= 4096))) { c->opt_seg = (int)value; return GC_OK; }
+    return gc_fail(c, GC_ERR_BADARG, "gc_ctx_set_option: unknown key or value out of range");
+}
+
 extern "C" int64_t gc_launch_count(const gc_ctx *c) { return c ? (int64_t)c->launches : 0; }
 extern "C" int gc_profile_enable(gc_ctx *c, int on) { if (!c) return GC_ERR_BADARG; c->prof = on != 0; return GC_OK; }
 extern "C" int gc_profile_read(gc_ctx *c, double *ms, int64_t *count)
@@ -270,14 +278,12 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     build_tiles(L, xt, yt);
     L->nxt = (int)xt.size(); L->nyt = (int)yt.size();
     L->d_xt = upload(L, xt); L->d_yt = upload(L, yt);
-    {   // sweep kernel family: marching lines for large levels, edge-parallel tiles for small ones (GC_SWEEP=edge|march overrides)
-        const char *mode = getenv("GC_SWEEP");
+    {   // sweep kernel family: marching lines for large levels, edge-parallel tiles for small ones (gc_ctx_set_option overrides)
         L->use_march = L->ncells >= (int64_t)GC_MARCH_MIN_CELLS;
-        if (mode && !strcmp(mode, "edge")) L->use_march = 0;
-        if (mode && !strcmp(mode, "march")) L->use_march = 1;
+        if (ctx->opt_family == 1) L->use_march = 0;
+        if (ctx->opt_family == 2) L->use_march = 1;
         int seg = (int)std::min<int64_t>(128, std::max<int64_t>(16, (L->ncells / 400000 + 3) / 4 * 4));
-        const char *sg = getenv("GC_MARCH_SEG");
-        if (sg && atoi(sg) >= 4) seg = atoi(sg) / 4 * 4;
+        if (ctx->opt_seg >= 4) seg = ctx->opt_seg / 4 * 4;
         std::vector<LineDesc> xl, yl;
         if (L->use_march) build_lines(L, seg, xl, yl);
         L->nxl_lines = (int64_t)xl.size(); L->nyl_lines = (int64_t)yl.size();

@@ -86,6 +86,7 @@ struct gc_ctx {
     void *user;
     std::string err;
     bool prof = false;
+    int opt_family = 0, opt_seg = 0;                 // gc_ctx_set_option: sweep kernel family (0 auto, 1 edge, 2 march), marching segment length
     void *stage = nullptr; size_t stage_bytes = 0;   // grow-only device staging buffer of the host-pointer paths (gc_stage_get)
     unsigned long long launches = 0;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];

@@ -187,81 +187,61 @@ __device__ __forceinline__ void gc_riemann(M &m, double g, double eps, RState L,
     if (!m2) { s[2] = 0.0; Z[2][0] = 0.0; Z[2][1] = 0.0; Z[2][2] = 0.0; }
 }
 
-// ---- straight-line variants for the common case --------------------------------------------------------------
-// The same expressions in the same order as gc_prim / gc_riemann, specialised to the branch an open-ocean edge takes
-// (both sides wet, one shock + one rarefaction in R5, not near-critical in R7, subcritical clamp l1 < -tau < tau < l3)
-// and written without control flow, so that the independent divide / square-root chains can overlap.  They return
-// false when the edge is not of that kind (or a fast-math operand left its window); the caller then runs the
-// general code above.  Where both apply they produce identical bits.
+// ---- guarded open-ocean path -------------------------------------------------------------------------------------
+// The same R0-R8 result, for the edges a tsunami model meets almost everywhere (both cells wet, small Froude number,
+// similar depths), written without control flow and WITHOUT step R5.  DESIGN.md 5 ("guard") gives the argument; in short:
+// with c- = min(cL, cR) and the guard
+//     G:  |cL - cR| <= c-/4,   |uL| <= c-/4,   |uR| <= c-/4,   c- >= 0.1,
+// every branch of R5 (two rarefactions, two shocks after its one Newton step, shock + rarefaction after its one secant step)
+// returns sigma1 <= -c-/4 and sigma2 >= c-/4, while sE1 <= uL - cL < 0 < uR + cR <= sE2.  Hence R6 gives lambda1 = sE1 and
+// lambda3 = sE2 whatever R5 returned, none of the eight near-critical tests of R7 can fire (each quantity they compare with
+// tau = 1e-6 or sqrt(tau) is bounded away from it by more than a factor 50), and the clamp case is lambda1 < -tau < tau <
+// lambda3.  R5 only ever decides these comparisons, so it is not evaluated at all.  The slack in every inequality is >= 0.02
+// absolute against rounding errors of 1e-16 c.  tests/test_oracle_guard.py checks the claim on the oracle's own R5.
+// Both functions return false when the cell / edge is not of that kind; the caller then runs the general code above.
+// Where they return true they produce its bits.  Division and roots use the unchecked sequences of gc_math.cuh; their
+// operands are inside the window by the same bounds: h in (hlo, 2^100], c in [0.1, 2^54], |p-bar| >= (15/16) c-^2,
+// lambda3 - lambda1 >= 1.5 c-; the numerator of u-hat may be zero or tiny, and is then absorbed by -+ c-hat.
 
-// R0 + R2 without branches (the reciprocal of a dry cell's depth is taken of 1 and discarded)
-__device__ __forceinline__ void gc_prim_fast(MathFast &m, RState &S, double g, double eps)
+// R0 + R2 of a cell.  hlo = max(dry tolerance, 2^-100); hg = 0.5 * g.  false: dry, or h outside (hlo, 2^100].
+__device__ __forceinline__ bool gc_prim_fast(RState &S, double g, double hg, double hlo)
 {
-    const bool wet = S.h > eps;                       // h < 0 and h <= eps both end as the zero state
-    const double hs = wet ? S.h : 1.0;
-    const double rh = m.rcp(hs);
-    const double u = S.p * rh, v = S.t * rh;
-    const double phi = __fma_rn(S.p, u, 0.5 * g * (S.h * S.h));
-    S.h = wet ? S.h : 0.0; S.p = wet ? S.p : 0.0; S.t = wet ? S.t : 0.0;
-    S.u = wet ? u : 0.0; S.v = wet ? v : 0.0; S.phi = wet ? phi : 0.0;
-    S.c = m.sqrt_(g * S.h);
+    const double rh = gc_frcp(S.h);
+    S.u = S.p * rh; S.v = S.t * rh;
+    S.phi = __fma_rn(S.p, S.u, hg * (S.h * S.h));
+    S.c = gc_fsqrt(g * S.h);
+    return (S.h > hlo) && (S.h <= 0x1p100);
 }
 
-// Lanes whose edge is not of that kind compute garbage (possibly Inf / NaN: harmless, nothing traps) that the caller
-// discards; only the returned flag decides.
-__device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double eps, const RState &L, const RState &R,
-                                                double (&Z)[3][3], double (&s)[3])
+// R3-R8 of an edge whose two cells passed gc_prim_fast.  Writes all of Z and s (garbage when it returns false).
+__device__ __forceinline__ bool gc_riemann_fast(double g, const RState &L, const RState &R, double (&Z)[3][3], double (&s)[3])
 {
-    bool ok = (L.h > eps) && (R.h > eps);
     const double hL = L.h, hR = R.h, cL = L.c, cR = R.c;
-    // R4
-    const double sL = L.u - cL, sR = R.u + cR;
-    const double uhat = m.div(cL * L.u + cR * R.u, cL + cR);
-    const double chat = m.sqrt_(g * (0.5 * (hL + hR)));
-    const double sE1 = dmin(sL, uhat - chat);
-    const double sE2 = dmax(sR, uhat + chat);
-    // R5, shock + rarefaction branch
-    const bool deepL = hL > hR, shalL = hL < hR;
-    const double hmin = shalL ? hL : hR, hmax = hL > hR ? hL : hR;
-    const double du = R.u - L.u;
-    const double cmin = shalL ? cL : cR;
-    const double cmax = shalL ? cR : cL;
-    const double Fmin = __fma_rn(2.0, cmin - cmax, du);                 // = du + 2 (cmin - cmax) bit for bit (x 2 is exact)
-    const double Fmax = __fma_rn(hmax - hmin, m.sqrt_(m.div(0.5 * g * (hmax + hmin), hmax * hmin)), du);
-    ok = ok && !(Fmin > 0.0) && !(Fmax <= 0.0);
-    const double h1 = hmin - m.div(Fmin * (hmax - hmin), Fmax - Fmin);
-    const double cm = m.sqrt_(g * h1);
-    const double aL = __fma_rn(2.0, cL, L.u), aR = __fma_rn(-2.0, cR, R.u);   // = u + 2c, u - 2c bit for bit
-    const double s1m = deepL ? __fma_rn(-3.0, cm, aL) : (aR + cm);
-    const double s2m = deepL ? (aL - cm) : __fma_rn(3.0, cm, aR);
-    // R6
-    const double l1 = dmin(sE1, s2m);
-    const double l3 = dmax(sE2, s1m);
+    // guard G
+    const double cmn = dmin(cL, cR);
+    const double c4 = 0.25 * cmn;
+    bool ok = (fabs(cL - cR) <= c4) && (fabs(L.u) <= c4) && (fabs(R.u) <= c4) && (cmn >= 0.1);
+    // R4 (= R6 under G)
+    const double hsum = hL + hR;
+    const double ghbar = g * (0.5 * hsum);                               // max(0.5 (hL + hR), 0) = 0.5 (hL + hR): both wet
+    const double uhat = gc_fdiv(cL * L.u + cR * R.u, cL + cR);
+    const double chat = gc_fsqrt(ghbar);
+    const double l1 = dmin(L.u - cL, uhat - chat);
+    const double l3 = dmax(R.u + cR, uhat + chat);
     const double l2 = 0.5 * (l1 + l3);
     // R7, not near-critical, subcritical clamp
     const double delb = R.b - L.b;
-    const double hbar = dmax(0.5 * (hL + hR), 0.0);
-    const double ghbar = g * hbar;
     const double su = L.u + R.u;
     const double pbar = __fma_rn(0.25 * su, su, -ghbar);
     const double ptil = dmax(0.0, L.u * R.u) - ghbar;
     const double hsd = dmax(0.0, __fma_rn(-l1, hL, __fma_rn(l3, hR, L.p - R.p)));
-    bool sonic = fabs(pbar) <= GC_TAU;
-    sonic = sonic || (pbar * ptil <= GC_TAU);
-    sonic = sonic || (pbar * l1 * l3 <= GC_TAU);
-    sonic = sonic || (dmin(fabs(l1), fabs(l3)) < GC_SQRT_TAU);
-    sonic = sonic || (l1 < GC_SQRT_TAU && s1m > -GC_SQRT_TAU);
-    sonic = sonic || (l3 > -GC_SQRT_TAU && s2m < GC_SQRT_TAU);
-    sonic = sonic || ((L.u + cL) * (R.u + cR) < 0.0);
-    sonic = sonic || ((L.u - cL) * (R.u - cR) < 0.0);
-    ok = ok && !sonic && (l1 < -GC_TAU) && (l3 > GC_TAU);
-    const double q = m.div(ghbar, pbar);
+    const double q = gc_fdiv(ghbar, pbar);
     const double dh = delb * q;
     double dphi = -delb * (q * ptil);
     // The clamp dh <- max(min(dh, hsd / l3), hsd / l1) is the identity when dh lies inside the bounds.  That is decided
     // without the two divides, with a margin far above the rounding of the products and of the quotients:
     //   dh * l3 < hsd (1 - 1e-7)  =>  dh < fl(hsd / l3);   dh * l1 < hsd (1 - 1e-7)  =>  dh > fl(hsd / l1)   (l1 < 0 < l3).
-    // hsd > 1e-100 and |dh| < 1e100 keep every product away from underflow / overflow (|l| >= tau).  Otherwise: general code.
+    // hsd > 1e-100 and |dh| < 1e100 keep every product away from underflow / overflow.  Otherwise: general code.
     {
         const double hs = hsd * 0.9999999;
         ok = ok && (hsd > 1.0e-100) && (fabs(dh) < 1.0e100) && (dh * l3 < hs) && (dh * l1 < hs);
@@ -275,7 +255,7 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     const double d1 = (hR - hL) - dh;
     const double d2 = R.p - L.p;
     const double d3 = (R.phi - L.phi) - dphi;
-    const double rdl = m.rcp(l3 - l1);
+    const double rdl = gc_frcp(l3 - l1);
     const double l1sq = l1 * l1, l3sq = l3 * l3;
     const double b1 = __fma_rn(l3, d1, -d2) * rdl;
     const double b3 = __fma_rn(-l1, d1, d2) * rdl;
@@ -284,5 +264,5 @@ __device__ __forceinline__ bool gc_riemann_fast(MathFast &m, double g, double ep
     Z[2][0] = b3 * l3; Z[2][1] = b3 * l3sq; Z[2][2] = R.v * Z[2][0];
     Z[1][0] = 0.0;     Z[1][1] = b2;        Z[1][2] = ((R.p * R.v - L.p * L.v) - Z[0][2]) - Z[2][2];
     s[0] = l1; s[1] = l2; s[2] = l3;
-    return ok && !m.failed();
+    return ok;
 }

@@ -103,110 +103,55 @@ __device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double
     return m;
 }
 
-// (3)-(6) without control flow (same values as gc_edge_flux: a skipped family contributes +0.0 to the fluctuations, whose sums
-// start at +0.0 and can therefore never be -0.0, and T = +0.0 to the correction, exactly what gc_edge_flux leaves there).
-// m.failed() afterwards: redo with gc_edge_flux.
+// (3)-(6) for a "standard" edge, without control flow: the edge was solved by gc_riemann_fast, so s[0] < 0 < s[2] (the edge
+// factor is positive) and families 1 and 3 need no sign tests; only the corrector family 2 keeps them.  Requires limiter = MC.
+// Same values as gc_edge_flux: the fluctuation sums are formed in the same order, a skipped term is added as +0.0 (no bit
+// changes: the partial sums start at +0.0 and are therefore never -0.0), -|s0| = s0 exactly, Z[1][0] is +0.0 by construction
+// (so its square drops out of zz: fma(x, x, +0) = fl(x x) for every x).  The three limiter divides use the unchecked
+// sequence: the function returns false -- and the caller redoes the edge with gc_edge_flux -- unless all six operands are
+// inside its window (a zero wave or a zero upwind product is outside) and s[1] != 0.  dtdx_ave = 0.5 fma(dt, rdL, dt rdR).
 __device__ __forceinline__ double gc_mc_fast(double theta)
 {
     return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));                      // MC
 }
-__device__ __forceinline__ void gc_edge_flux_fast(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
-                                                  double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
-{
-    double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
-    double T[3][3];
-    const double dtdx_ave = 0.5 * __fma_rn(dt, rdL, dt * rdR);
-#pragma unroll
-    for (int w = 0; w < 3; w++) {
-        const double sw = W.s[w];
-        const bool neg = sw < 0.0, pos = sw > 0.0;
-#pragma unroll
-        for (int c = 0; c < 3; c++) {
-            const double z = W.Z[w][c], hz = 0.5 * z;
-            am[c] = am[c] + (neg ? z : (pos ? 0.0 : hz));
-            ap[c] = ap[c] + (pos ? z : (neg ? 0.0 : hz));
-        }
-        if (limiter != 0) {
-            const double zz = __fma_rn(W.Z[w][2], W.Z[w][2], __fma_rn(W.Z[w][1], W.Z[w][1], W.Z[w][0] * W.Z[w][0]));
-            const bool nz = zz != 0.0;
-            const double theta = m.div(pos ? dlo[w] : dhi[w], nz ? zz : 1.0);                       // eq. 10 (S-1), eq. 11
-            const double phi = nz ? gc_mc_fast(theta) : 1.0;
-            const double cphi = ((pos ? 0.5 : -0.5) * __fma_rn(-fabs(sw), dtdx_ave, 1.0)) * phi;
-            const bool on = neg || pos;                                                              // sgn(0) = 0 (S-4)
-#pragma unroll
-            for (int c = 0; c < 3; c++) T[w][c] = on ? cphi * W.Z[w][c] : 0.0;                       // eq. 9, one family
-        }
-    }
-    if (limiter != 0) {
-#pragma unroll
-        for (int c = 0; c < 3; c++) F[c] = (T[0][c] + T[2][c]) + T[1][c];
-    }
-#pragma unroll
-    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
-}
-
-// (3)-(6) for a "standard" edge: s[0] < 0 < s[2] is known (every edge solved by gc_riemann_fast: l1 < -tau, l3 > tau, and
-// the edge factor is positive), so families 1 and 3 need no sign tests; only the corrector family 2 keeps them.
-// Same values as gc_edge_flux: the sums are formed in the same order, a skipped term is added as +0.0 (no bit changes:
-// the partial sums start at +0.0 and are therefore never -0.0), -|s0| = s0 exactly, Z[1][0] is +0.0 by construction (so its
-// square drops out of zz: fma(x, x, +0) = fl(x x) for every x).  m.failed() afterwards: redo with gc_edge_flux.
-__device__ __forceinline__ void gc_edge_flux_std(MathFast &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
-                                                 double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
+__device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&dlo)[3], const double (&dhi)[3],
+                                                 double dtdx_ave, double (&fm)[3], double (&fp)[3])
 {
     const double s0 = W.s[0], s1 = W.s[1], s2 = W.s[2];
     const bool neg1 = s1 < 0.0, pos1 = s1 > 0.0;
-    double am[3], ap[3], F[3] = {0.0, 0.0, 0.0};
+    double am[3], ap[3];
     am[0] = 0.0 + W.Z[0][0];
     ap[0] = 0.0 + W.Z[2][0];
 #pragma unroll
     for (int c = 1; c < 3; c++) {
-        const double z = W.Z[1][c], hz = 0.5 * z;
-        am[c] = (0.0 + W.Z[0][c]) + (neg1 ? z : (pos1 ? 0.0 : hz));
-        ap[c] = (0.0 + (pos1 ? z : (neg1 ? 0.0 : hz))) + W.Z[2][c];
+        const double z = W.Z[1][c];
+        am[c] = (0.0 + W.Z[0][c]) + (neg1 ? z : 0.0);
+        ap[c] = (0.0 + (pos1 ? z : 0.0)) + W.Z[2][c];
     }
-    if (limiter != 0) {
-        const double dtdx_ave = 0.5 * __fma_rn(dt, rdL, dt * rdR);
-        double c0, c1, c2;
-        {   // family 1: s < 0, upwind neighbour e+1
-            const double zz = __fma_rn(W.Z[0][2], W.Z[0][2], __fma_rn(W.Z[0][1], W.Z[0][1], W.Z[0][0] * W.Z[0][0]));
-            const bool nz = zz != 0.0;
-            const double theta = m.div(dhi[0], nz ? zz : 1.0);
-            const double phi = nz ? gc_mc_fast(theta) : 1.0;
-            c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * phi;
-        }
-        {   // family 2: either sign, sgn(0) = 0
-            const double zz = __fma_rn(W.Z[1][2], W.Z[1][2], W.Z[1][1] * W.Z[1][1]);
-            const bool nz = zz != 0.0;
-            const double theta = m.div(pos1 ? dlo[1] : dhi[1], nz ? zz : 1.0);
-            const double phi = nz ? gc_mc_fast(theta) : 1.0;
-            c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * phi;
-        }
-        {   // family 3: s > 0, upwind neighbour e-1
-            const double zz = __fma_rn(W.Z[2][2], W.Z[2][2], __fma_rn(W.Z[2][1], W.Z[2][1], W.Z[2][0] * W.Z[2][0]));
-            const bool nz = zz != 0.0;
-            const double theta = m.div(dlo[2], nz ? zz : 1.0);
-            const double phi = nz ? gc_mc_fast(theta) : 1.0;
-            c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * phi;
-        }
-        const bool on = neg1 || pos1;
+    // eq. 10 (S-1), eq. 11: upwind neighbour e+1 for family 1 (s < 0), e-1 for family 3 (s > 0), by sign for family 2
+    const double zz0 = __fma_rn(W.Z[0][2], W.Z[0][2], __fma_rn(W.Z[0][1], W.Z[0][1], W.Z[0][0] * W.Z[0][0]));
+    const double zz1 = __fma_rn(W.Z[1][2], W.Z[1][2], W.Z[1][1] * W.Z[1][1]);
+    const double zz2 = __fma_rn(W.Z[2][2], W.Z[2][2], __fma_rn(W.Z[2][1], W.Z[2][1], W.Z[2][0] * W.Z[2][0]));
+    const double zi0 = dhi[0], zi1 = pos1 ? dlo[1] : dhi[1], zi2 = dlo[2];
+    const bool ok = (neg1 || pos1) && gc_in_window(zz0) && gc_in_window(zz1) && gc_in_window(zz2)
+                    && gc_in_window(zi0) && gc_in_window(zi1) && gc_in_window(zi2);
+    const double c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi0, zz0));
+    const double c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi1, zz1));
+    const double c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi2, zz2));
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
-            const double t1 = c1 * W.Z[1][c];
-            F[c] = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + (on ? t1 : 0.0);                              // eq. 9
-        }
+    for (int c = 0; c < 3; c++) {
+        const double F = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + c1 * W.Z[1][c];                         // eq. 9, outer families first
+        fm[c] = F + am[c]; fp[c] = F - ap[c];
     }
-#pragma unroll
-    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
+    return ok;
 }
 
-// eq. 15 for a standard edge (s[0] < 0 < s[2]): the terms max(s0, 0) rdR and max(-s2, 0) rdL are +0
+// eq. 15 for a standard edge (s[0] < 0 < s[2]): max(s0, 0) and max(-s2, 0) are +0, and the corrector speed
+// s1 = 0.5 (s0 + s2) lies between the outer two, so its terms are never the largest (rounding is monotone):
+// the edge's value is max(-s0 rdL, s2 rdR), the same number gc_edge_cfl returns.
 __device__ __forceinline__ double gc_edge_cfl_std(const Waves &W, double rdL, double rdR)
 {
-    double m = (-W.s[0]) * rdL;
-    m = dmax(m, dmax(W.s[1], 0.0) * rdR);
-    m = dmax(m, dmax(-W.s[1], 0.0) * rdL);
-    m = dmax(m, W.s[2] * rdR);
-    return m;
+    return dmax((-W.s[0]) * rdL, W.s[2] * rdR);
 }
 
 // ---- Manning friction (eq. 1b-1c, 2, reading S-16) -----------------------------------------

@@ -8,11 +8,9 @@
 // Two kernel families compute the same bits:
 //  * k_sweep  (edge-parallel): thread <-> edge, neighbour waves through shared memory.  Much parallelism per
 //    cell, used for small levels where the GPU would otherwise be empty.
-//  * k_march  (line-marching): thread <-> line segment, walking along the sweep with the waves of the previous
-//    edge, the primitive variables of the previous cell and the pending fluxes in registers.  No shared
-//    memory, no barriers, each cell's primitive variables computed once, 3 redundant edges per segment only.
-//    The x-sweep reads 4 cells of its row per 256-bit load (rows are 32-byte aligned); the y-sweep reads
-//    one row of 32 adjacent columns per warp (coalesced).  Used for large levels (fp64-pipe bound).
+//  * k_marchp (line-marching): thread <-> line segment, walking along the sweep.  Each cell's primitive variables are
+//    computed once, 3 redundant edges per segment only, no barriers; what a line carries from cell to cell is parked in
+//    the thread's own shared-memory slots.  Used for large levels (fp64-pipe bound).
 #include <cstdlib>
 #include <cstring>
 #include "gc_internal.h"
@@ -21,12 +19,6 @@
 #define SW_BLOCK 256
 #ifndef MARCH_BLOCK
 #define MARCH_BLOCK 128
-#endif
-#ifndef MARCH_MINB
-#define MARCH_MINB 3     // resident blocks per SM the register allocation is bounded for
-#endif
-#ifndef MARCH_UNROLL
-#define MARCH_UNROLL 1
 #endif
 #define SW_YW 8       // columns per y-sweep block (8 doubles = 2 full 32-byte sectors per row access)
 
@@ -40,6 +32,7 @@ struct SweepArgs {
     const double *ey;                // y edge factors per global edge (+2)
     double ex;
     double g, eps;
+    double hlo;                      // max(eps, 2^-100): lower depth bound of the guarded open-ocean path
     double dt; const double *dt_dev; // dt_dev != NULL: read dt from device memory
     int coord, limiter, write_out;
     DevStats *stats;
@@ -93,12 +86,10 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
         if (DIR == 0) { L.p = a.hu[idx - str]; L.t = a.hv[idx - str]; R.p = a.hu[idx]; R.t = a.hv[idx]; }
         else          { L.p = a.hv[idx - str]; L.t = a.hu[idx - str]; R.p = a.hv[idx]; R.t = a.hu[idx]; }
         qh = R.h; qp = R.p; qt = R.t;
-        {   // straight-line code for an open-ocean edge first; any other edge is redone with the general code (same bits)
-            MathFast mf;
+        {   // guarded open-ocean code first; any other edge is redone with the general code (same bits where both apply)
             RState Lf = L, Rf = R;
-            gc_prim_fast(mf, Lf, a.g, a.eps);
-            gc_prim_fast(mf, Rf, a.g, a.eps);
-            stdE = gc_riemann_fast(mf, a.g, a.eps, Lf, Rf, Z, s);
+            const bool okL = gc_prim_fast(Lf, a.g, 0.5 * a.g, a.hlo), okR = gc_prim_fast(Rf, a.g, 0.5 * a.g, a.hlo);
+            stdE = gc_riemann_fast(a.g, Lf, Rf, Z, s) && okL && okR;
         }
         if (!stdE) {
             MathIeee mi;
@@ -131,7 +122,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
             zi[w] = __fma_rn(sZ[3 * w + 2][kn], Z[w][2], __fma_rn(sZ[3 * w + 1][kn], Z[w][1], sZ[3 * w + 0][kn] * Z[w][0]));
         }
         bool done = false;
-        if (stdE) { MathFast mf; gc_edge_flux_std(mf, W, zi, zi, a.limiter, dt, rdL, rdR, fm, fp); done = !mf.failed(); }
+        if (stdE && a.limiter != 0) done = gc_edge_flux_std(W, zi, zi, 0.5 * __fma_rn(dt, rdL, dt * rdR), fm, fp);
         if (!done) { MathIeee mi; gc_edge_flux(mi, W, zi, zi, a.limiter, dt, rdL, rdR, fm, fp); }
         // eq. 15: right-going waves enter the right cell, left-going the left cell; interior lines only
         const bool count = (DIR == 1) || (line >= 2 && line < pd.ny + 2);
@@ -187,202 +178,34 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
     }
 }
 
-// ---- line-marching sweep ------------------------------------------------------------------------------------
-__device__ __forceinline__ void ld4(const double *p, double &x, double &y, double &z, double &w)
-{
-    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
-}
-
-// x-sweep staging: each thread copies the next 4 cells (32 bytes) of its row, per plane, into its own slots of a
-// two-stage shared-memory buffer with cp.async, one group ahead of their use
-__device__ __forceinline__ void cp16(const double *sdst, const double *gsrc)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void stage_group(const SweepArgs &a, const double *sb, int64_t o)
-{
-    cp16(sb, a.h + o);                        cp16(sb + 2, a.h + o + 2);
-    cp16(sb + MARCH_BLOCK * 4, a.hu + o);     cp16(sb + MARCH_BLOCK * 4 + 2, a.hu + o + 2);
-    cp16(sb + 2 * MARCH_BLOCK * 4, a.hv + o); cp16(sb + 2 * MARCH_BLOCK * 4 + 2, a.hv + o + 2);
-    cp16(sb + 3 * MARCH_BLOCK * 4, a.b + o);  cp16(sb + 3 * MARCH_BLOCK * 4 + 2, a.b + o + 2);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-}
-#define MARCH_STAGE_BYTES (2 * 4 * MARCH_BLOCK * 4 * 8)   // [stage][plane][thread][4 cells] doubles
-
-template <int DIR>
-__global__ void __launch_bounds__(MARCH_BLOCK, MARCH_MINB) k_march(SweepArgs a)
-{
-    __shared__ double sred[MARCH_BLOCK / 32];
-    __shared__ unsigned long long sclip[MARCH_BLOCK / 32];
-    __shared__ double sclipm[MARCH_BLOCK / 32];
-
-    const int64_t lid = (int64_t)blockIdx.x * MARCH_BLOCK + threadIdx.x;
-    const bool active = lid < a.nlines;
-    LineDesc ln; ln.patch = 0; ln.line = 0; ln.c0 = 2; ln.nc = -4;
-    if (active) { int4 v = *reinterpret_cast<const int4 *>(a.lines + lid); ln.patch = v.x; ln.line = v.y; ln.c0 = v.z; ln.nc = v.w; }
-    const PatchDesc pd = a.pat[ln.patch];
-    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
-    const int nst = ln.nc + 4;                                   // cells read by this line
-    const int nst_warp = __reduce_max_sync(0xffffffffu, nst);
-    const int cfirst = ln.c0 - 2;                                // storage index (along the sweep) of the first cell read
-    int64_t base; int64_t str;
-    if (DIR == 0) { base = pd.off + (int64_t)ln.line * pd.pitch + cfirst; str = 1; }
-    else          { base = pd.off + (int64_t)cfirst * pd.pitch + ln.line; str = pd.pitch; }
-    const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
-    const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
-
-    Waves Wc; gc_waves_zero(Wc);                                 // waves of the previous edge (r-1)
-    double dlo[3] = {0.0, 0.0, 0.0};                             // Z_{r-2} . Z_{r-1}
-    double fpp[3] = {0.0, 0.0, 0.0};                             // fp of edge r-2
-    RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
-    double q1h = 0.0, q1p = 0.0, q1t = 0.0, q2h = 0.0, q2p = 0.0, q2t = 0.0;   // raw state of cells r-1, r-2
-    double rd1 = 0.0, rd2 = 0.0;                                 // 1/(kappa dx) of cells r-1, r-2
-    double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
-    bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
-
-    extern __shared__ __align__(16) double stage[];              // x-sweep: MARCH_STAGE_BYTES of staging slots
-    if (DIR == 0 && nst > 0) stage_group(a, stage + threadIdx.x * 4, base);
-    double nh_ = 0.0, np_ = 0.0, nt_ = 0.0, nb_ = 0.0;           // y-sweep: next row, loaded one step ahead
-    if (DIR == 1 && nst > 0) {
-        nh_ = a.h[base]; nb_ = a.b[base]; np_ = a.hv[base]; nt_ = a.hu[base];
-    }
-
-    constexpr int kMarchUnroll = MARCH_UNROLL;
-#pragma unroll kMarchUnroll
-    for (int r = 0; r < nst_warp; r++) {
-        const bool live = r < nst;
-        double qh, qp, qt, qb;
-        if (DIR == 0) {
-            // the 4 cells of a group were requested one group ago (cp.async.cg into this thread's own staging slots: no
-            // register is tied up while the request is in flight and nothing is allocated in L1, which the spilled
-            // loop invariants need); each cell is read from its slot when its turn comes
-            if ((r & 3) == 0) {
-                asm volatile("cp.async.wait_group 0;" ::: "memory");
-                if (r + 4 < nst) stage_group(a, stage + (size_t)(((r >> 2) + 1) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4, base + r + 4);
-            }
-            const double *sb = stage + (size_t)((r >> 2) & 1) * (4 * MARCH_BLOCK * 4) + threadIdx.x * 4 + (r & 3);
-            qh = live ? sb[0] : 0.0; qp = live ? sb[MARCH_BLOCK * 4] : 0.0;
-            qt = live ? sb[2 * MARCH_BLOCK * 4] : 0.0; qb = live ? sb[3 * MARCH_BLOCK * 4] : 0.0;
-        } else {
-            qh = nh_; qp = np_; qt = nt_; qb = nb_;
-            if (r + 1 < nst) {
-                const int64_t o = base + (int64_t)(r + 1) * str;
-                nh_ = a.h[o]; nb_ = a.b[o]; np_ = a.hv[o]; nt_ = a.hu[o];
-            }
-        }
-        const int c = cfirst + r;                                // storage index of this cell = index of the edge on its low side
-        double rd0, ef;
-        if (DIR == 0) { rd0 = rdrow; ef = a.ex; }
-        else          { rd0 = live ? a.rd[pd.j0 + c] : 0.0; ef = live ? a.ey[pd.j0 + c] : 1.0; }
-
-        RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
-        Waves Wn;
-        bool stdn = false;
-        {   // straight-line code for an open-ocean edge first (gc_riemann_fast); any other kind of edge, or a fast-math
-            // operand outside its window (gc_math.cuh), redoes this cell + edge with the general code and IEEE operators
-            MathFast mf;
-            const RState R0 = R;
-            gc_prim_fast(mf, R, a.g, a.eps);
-            bool ok = !mf.failed();
-            if (r >= 1 && live) ok = gc_riemann_fast(mf, a.g, a.eps, Lst, R, Wn.Z, Wn.s) && ok;
-            else gc_waves_zero(Wn);
-            stdn = ok && (r >= 1) && live;
-            if (!ok) {
-                MathIeee mi;
-                R = R0;
-                gc_prim(mi, R, a.g, a.eps);
-                if (r >= 1 && live) gc_riemann(mi, a.g, a.eps, Lst, R, Wn.Z, Wn.s);
-            }
-            if (a.coord == 1) {                                   // scale by the edge factor
-#pragma unroll
-                for (int w = 0; w < 3; w++) { Wn.s[w] = Wn.s[w] * ef; Wn.Z[w][0] = Wn.Z[w][0] * ef; Wn.Z[w][1] = Wn.Z[w][1] * ef; Wn.Z[w][2] = Wn.Z[w][2] * ef; }
-            }
-        }
-        double dhi[3];
-        gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
-        double fm[3], fp[3];
-        {   // edge r-1: a standard edge (s[0] < 0 < s[2], solved by the fast path) needs no sign tests for families 1 and 3
-            MathFast mf;
-            if (stdc) gc_edge_flux_std(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
-            else gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
-            if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
-        }
-        if (live && r >= 3 && count) cflm = dmax(cflm, stdc ? gc_edge_cfl_std(Wc, rd2, rd1) : gc_edge_cfl(Wc, rd2, rd1));
-        if (live && r >= 4) {                                                           // cell r-2
-            const double dtdx = dt * rd2;
-            double uh = __fma_rn(-dtdx, fm[0] - fpp[0], q2h);
-            double up = __fma_rn(-dtdx, fm[1] - fpp[1], q2p);
-            double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q2t);
-            const int64_t o = base + (int64_t)(r - 2) * str;
-            if (DIR == 0) {
-                a.oh[o] = uh; a.ohu[o] = up; a.ohv[o] = ut;
-            } else {
-                if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
-                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[pd.j0 + c - 2] * a.dxdy); }
-                    uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
-                }
-                if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
-                    const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
-                    ut = q.x; up = q.y;
-                }
-                if (uh != uh || up != up || ut != ut) nanf = 1;
-                if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 3; k++) { fpp[k] = fp[k]; dlo[k] = dhi[k]; }
-        Wc = Wn; Lst = R; stdc = stdn;
-        q2h = q1h; q2p = q1p; q2t = q1t; q1h = qh; q1p = qp; q1t = qt;
-        rd2 = rd1; rd1 = rd0;
-    }
-
-    cflm = warp_max(cflm);
-    if (DIR == 1) {
-        nclip = __reduce_add_sync(0xffffffffu, nclip);
-        nanf = __any_sync(0xffffffffu, nanf);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) clipm += __shfl_xor_sync(0xffffffffu, clipm, o);
-    }
-    const int k = threadIdx.x;
-    if ((k & 31) == 0) { sred[k >> 5] = cflm; if (DIR == 1) { sclip[k >> 5] = nclip; sclipm[k >> 5] = clipm; if (nanf) a.stats->nan_seen = 1; } }
-    __syncthreads();
-    if (k == 0) {
-        double m = sred[0];
-#pragma unroll
-        for (int w = 1; w < MARCH_BLOCK / 32; w++) m = dmax(m, sred[w]);
-        if (m > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(m));
-        if (DIR == 1) {
-            unsigned long long n = 0; double cm = 0.0;
-#pragma unroll
-            for (int w = 0; w < MARCH_BLOCK / 32; w++) { n += sclip[w]; cm += sclipm[w]; }
-            if (n) { atomicAdd(&a.stats->nclip, n); atomicAdd(&a.stats->clipped, cm); }
-        }
-    }
-}
-
-// ---- line-marching sweep, parked state (k_marchp) ---------------------------------------------------------------
-// Same walk and the same arithmetic as k_march, but every value a line carries from one cell to the next and does not
-// need while the Riemann problem of the new edge is being solved -- the waves of the previous edge, the limiter dot
-// products, the pending flux, the raw state of the last two cells -- lives in this thread's own shared-memory slots
-// instead of registers (stored when produced, loaded when used; no rotation moves).  That bounds the kernel at 128
-// registers, so that 4 blocks (16 warps) are resident per SM, without the compiler's local-memory spills.
-// Slots are 16 bytes per thread, slot s of thread t at s * MARCH_BLOCK * 16 + t * 16: conflict-free 128-bit accesses.
-//   0-3 Z00 Z01 | Z02 Z11 | Z12 Z20 | Z21 Z22 (Z10 is +0 by construction)   4 s0 s1   5 s2 dlo0   6 dlo1 dlo2
-//   7 fpp0 fpp1   8 fpp2 -
-// y-sweep: 9-14 ring of the last 3 cells, (h, p) (t, rd) each; 15-18 the next row, 8 bytes per plane and stage (cp.async.ca).
-// x-sweep: 9-20 three stages of 2 cells x 4 planes (one 16-byte cp.async.cg each): the group in flight, the current one and
-//   the previous one, which still holds cell r-2; 21-26 the new values of 4 cells x 3 planes, written to the row with one
-//   256-bit store per plane (a thread's row accesses touch one sector per lane whatever their width, so wide ones are cheap).
+// ---- line-marching sweep (k_marchp) ------------------------------------------------------------------------------
+// Thread <-> line segment (a row for x, an interior column for y).  Iteration r takes in cell r of the segment and does two
+// INDEPENDENT pieces of work, written without control flow so that the compiler can interleave them (the kernel is bound by
+// dependent fp64 latency, not by a pipe: 8.9 cycles per dependent DFMA, 3 warps per scheduler):
+//   A  primitive variables of cell r and the Riemann problem of edge r (cells r-1 | r)          -> waves W(r)
+//   B  limiter, correction flux and fluctuations of edge r-2 from W(r-3), W(r-2), W(r-1)        -> fm, fp; update of cell r-3
+// Both use the guarded open-ocean code (gc_prim_fast / gc_riemann_fast / gc_edge_flux_std); a warp in which any lane's cell
+// or edge is of another kind (dry, near-critical, zero wave, ...) redoes exactly those lanes with the general branchy code and
+// IEEE operators afterwards -- the same bits wherever both apply, which is what every parity test asserts.
+// Everything a line carries from one iteration to the next, except the primitive variables of cell r-1, is parked in the
+// thread's own 16-byte shared-memory slots (slot s of thread t at s * PK_SL + t * 16: conflict-free 128-bit accesses):
+//   0-5, 6-11  two wave sets, used alternately: Z00 Z01 | Z02 Z11 | Z12 Z20 | Z21 Z22 | s0 s1 | s2 std  (Z10 is +0 by construction)
+//   12-14      dlo0 dlo1 | dlo2 fpp0 | fpp1 fpp2     (Z(r-3) . Z(r-2) per family; fp of edge r-3)
+//   y-sweep: 15-22 ring of the last 4 cells, (h, p) (t, rd) each; 23-26 the next row, 8 bytes per plane and stage (cp.async.ca)
+//   x-sweep: 15-30 four stages of 2 cells x 4 planes (one 16-byte cp.async.cg each): in flight, current, and the two before it
+//            (cell r-3 is read back from them); 31-36 the new values of 4 cells x 3 planes, written to the row with one 256-bit
+//            store per plane (a thread's row accesses touch one sector per lane whatever their width, so wide ones are cheap).
 #ifndef PARK_MINB
-#define PARK_MINB 4
+#define PARK_MINB 3
 #endif
 #define PK_SL (MARCH_BLOCK * 16u)
-#define PK_RING 9
-#define PK_STAGE 15
-#define PK_XST 9
-#define PK_XOUT 21
+#define PK_DOT 12
+#define PK_RING 15
+#define PK_YSTAGE 23
+#define PK_XST 15
+#define PK_XOUT 31
 #define PARK_BYTES_X ((PK_XOUT + 6) * PK_SL)
-#define PARK_BYTES_Y ((PK_STAGE + 4) * PK_SL)
+#define PARK_BYTES_Y ((PK_YSTAGE + 4) * PK_SL)
 
 __device__ __forceinline__ void sts2(unsigned addr, double x, double y)
 {
@@ -417,7 +240,7 @@ __device__ __forceinline__ void cpa8(unsigned sdst, const double *gsrc)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
 }
 
-template <int DIR>
+template <int DIR, int SPH>
 __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 {
     __shared__ double sred[MARCH_BLOCK / 32];
@@ -441,38 +264,38 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
     const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
     const int jrow = pd.j0 + cfirst;                             // y-sweep: global row (+2) of the first cell read
+    const double hg = 0.5 * a.g;
+    const bool mc = a.limiter != 0;
 
 #pragma unroll
     for (int k = 0; k < PK_RING; k++) sts2(sm0 + k * PK_SL, 0.0, 0.0);
     RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
+    bool Lok = false;                                            // cell r-1 passed gc_prim_fast
     double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
-    bool stdc = false;                                           // the previous edge is "standard" (gc_edge_flux_std)
-    unsigned ro0 = PK_RING * PK_SL, ro1 = (PK_RING + 2) * PK_SL, ro2 = (PK_RING + 4) * PK_SL;   // ring slots of cells r, r-1, r-2
 
     // staging: thread-private slots, filled by cp.async one group (x: 2 cells, y: 1 cell) ahead of their use
-    const unsigned st0 = (DIR == 0) ? sm0 + PK_XST * PK_SL : (unsigned)__cvta_generic_to_shared(dsm) + PK_STAGE * PK_SL + threadIdx.x * 8u;
-    unsigned xprev = 2 * (4 * PK_SL), xcur = 0, xnext = 4 * PK_SL;      // x: stage offsets of groups g-1, g, g+1
+    const unsigned st0 = (DIR == 0) ? sm0 + PK_XST * PK_SL : (unsigned)__cvta_generic_to_shared(dsm) + PK_YSTAGE * PK_SL + threadIdx.x * 8u;
     if (nst > 0) {
         if (DIR == 0) { cpa16(st0, a.h + base); cpa16(st0 + PK_SL, a.hu + base); cpa16(st0 + 2 * PK_SL, a.hv + base); cpa16(st0 + 3 * PK_SL, a.b + base); }
         else          { cpa8(st0, a.h + base); cpa8(st0 + PK_SL / 2, a.hv + base); cpa8(st0 + 2 * (PK_SL / 2), a.hu + base); cpa8(st0 + 3 * (PK_SL / 2), a.b + base); }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
 
-    for (int r = 0; r < nst_warp; r++) {
+    for (int r = 0; r <= nst_warp; r++) {
         const bool live = r < nst;
+        // ---- cell r arrives; the next group is requested
         double qh, qp, qt, qb;
         if (DIR == 0) {
             if ((r & 1) == 0) {
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
-                if (r > 0) { const unsigned t = xprev; xprev = xcur; xcur = xnext; xnext = t; }
                 if (r + 2 < nst) {
-                    const unsigned sd = st0 + xnext;
+                    const unsigned sd = st0 + (((r >> 1) + 1) & 3) * (4 * PK_SL);
                     const int64_t o = base + r + 2;
                     cpa16(sd, a.h + o); cpa16(sd + PK_SL, a.hu + o); cpa16(sd + 2 * PK_SL, a.hv + o); cpa16(sd + 3 * PK_SL, a.b + o);
                 }
                 asm volatile("cp.async.commit_group;" ::: "memory");
             }
-            const unsigned sa = st0 + xcur + (r & 1) * 8u;
+            const unsigned sa = st0 + ((r >> 1) & 3) * (4 * PK_SL) + (r & 1) * 8u;
             qh = lds1(sa); qp = lds1(sa + PK_SL); qt = lds1(sa + 2 * PK_SL); qb = lds1(sa + 3 * PK_SL);
         } else {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -485,76 +308,85 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             const unsigned sa = st0 + (r & 1) * (4 * (PK_SL / 2));
             qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
         }
-        if (!live) { qh = 0.0; qp = 0.0; qt = 0.0; qb = 0.0; }
-        double rd0, ef;
-        if (DIR == 0) { rd0 = rdrow; ef = a.ex; }
-        else          { rd0 = live ? a.rd[jrow + r] : 0.0; ef = live ? a.ey[jrow + r] : 1.0; }
-        if (DIR == 1) { sts2(sm0 + ro0, qh, qp); sts2(sm0 + ro0 + PK_SL, qt, rd0); }
+        double rd0 = rdrow, ef = a.ex;
+        if (DIR == 1) { rd0 = live ? a.rd[jrow + r] : 0.0; ef = live ? a.ey[jrow + r] : 1.0; }
 
+        // ---- parked state: edge r-2 (its set is overwritten by edge r below), the waves of edge r-1, Z(r-3).Z(r-2), fp(r-3)
+        const unsigned wa = sm0 + (unsigned)(r & 1) * (6 * PK_SL), wb = sm0 + (unsigned)((r & 1) ^ 1) * (6 * PK_SL);
+        Waves W2; double Z1[8], dlo[3], fpp[3], std2d;
+        lds2(wa, W2.Z[0][0], W2.Z[0][1]); lds2(wa + PK_SL, W2.Z[0][2], W2.Z[1][1]); lds2(wa + 2 * PK_SL, W2.Z[1][2], W2.Z[2][0]);
+        lds2(wa + 3 * PK_SL, W2.Z[2][1], W2.Z[2][2]); lds2(wa + 4 * PK_SL, W2.s[0], W2.s[1]); lds2(wa + 5 * PK_SL, W2.s[2], std2d);
+        W2.Z[1][0] = 0.0;
+        lds2(wb, Z1[0], Z1[1]); lds2(wb + PK_SL, Z1[2], Z1[3]); lds2(wb + 2 * PK_SL, Z1[4], Z1[5]); lds2(wb + 3 * PK_SL, Z1[6], Z1[7]);
+        lds2(sm0 + PK_DOT * PK_SL, dlo[0], dlo[1]); lds2(sm0 + (PK_DOT + 1) * PK_SL, dlo[2], fpp[0]); lds2(sm0 + (PK_DOT + 2) * PK_SL, fpp[1], fpp[2]);
+        const bool std2 = __double2loint(std2d) != 0;
+        double q3h, q3p, q3t, rd3, rd2;                                                 // raw cell r-3; 1/(kappa dx) of cells r-3, r-2
+        if (DIR == 0) {
+            const unsigned sq = st0 + (((r - 3) >> 1) & 3) * (4 * PK_SL) + ((r + 1) & 1) * 8u;
+            q3h = lds1(sq); q3p = lds1(sq + PK_SL); q3t = lds1(sq + 2 * PK_SL); rd3 = rdrow; rd2 = rdrow;
+        } else {
+            const unsigned k3 = sm0 + (PK_RING + 2 * ((r + 1) & 3)) * PK_SL, k2 = sm0 + (PK_RING + 2 * ((r + 2) & 3)) * PK_SL;
+            lds2(k3, q3h, q3p); lds2(k3 + PK_SL, q3t, rd3);
+            rd2 = lds1(k2 + PK_SL + 8u);
+            const unsigned k0 = sm0 + (PK_RING + 2 * (r & 3)) * PK_SL;
+            sts2(k0, qh, qp); sts2(k0 + PK_SL, qt, rd0);
+        }
+
+        // ---- A: cell r and edge r, guarded open-ocean code
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
         Waves Wn;
-        bool stdn = false;
-        {   // straight-line code for an open-ocean edge first; any other kind of edge, or a fast-math operand outside its
-            // window, redoes this cell + edge with the general code and IEEE operators (same bits)
-            MathFast mf;
-            const RState R0 = R;
-            gc_prim_fast(mf, R, a.g, a.eps);
-            bool ok = !mf.failed();
-            if (r >= 1 && live) ok = gc_riemann_fast(mf, a.g, a.eps, Lst, R, Wn.Z, Wn.s) && ok;
-            else gc_waves_zero(Wn);
-            stdn = ok && (r >= 1) && live;
-            if (!ok) {
-                MathIeee mi;
-                R = R0;
-                gc_prim(mi, R, a.g, a.eps);
-                if (r >= 1 && live) gc_riemann(mi, a.g, a.eps, Lst, R, Wn.Z, Wn.s);
-            }
-            if (a.coord == 1) {                                   // scale by the edge factor
-#pragma unroll
-                for (int w = 0; w < 3; w++) { Wn.s[w] = Wn.s[w] * ef; Wn.Z[w][0] = Wn.Z[w][0] * ef; Wn.Z[w][1] = Wn.Z[w][1] * ef; Wn.Z[w][2] = Wn.Z[w][2] * ef; }
-            }
-        }
-        Lst = R;
+        const bool okP = gc_prim_fast(R, a.g, hg, a.hlo);
+        const bool okR = gc_riemann_fast(a.g, Lst, R, Wn.Z, Wn.s) && okP && Lok;
 
-        // waves of edge r-1 and its lower dot products come back from their slots; those of edge r take their place
-        Waves Wc; double dlo[3], dhi[3];
-        lds2(sm0, Wc.Z[0][0], Wc.Z[0][1]); lds2(sm0 + PK_SL, Wc.Z[0][2], Wc.Z[1][1]); lds2(sm0 + 2 * PK_SL, Wc.Z[1][2], Wc.Z[2][0]);
-        lds2(sm0 + 3 * PK_SL, Wc.Z[2][1], Wc.Z[2][2]); lds2(sm0 + 4 * PK_SL, Wc.s[0], Wc.s[1]); lds2(sm0 + 5 * PK_SL, Wc.s[2], dlo[0]);
-        lds2(sm0 + 6 * PK_SL, dlo[1], dlo[2]);
-        Wc.Z[1][0] = 0.0;
-        gc_wave_dots(Wn, Wc, dhi);                                                      // Z_r . Z_{r-1}
-        sts2(sm0, Wn.Z[0][0], Wn.Z[0][1]); sts2(sm0 + PK_SL, Wn.Z[0][2], Wn.Z[1][1]); sts2(sm0 + 2 * PK_SL, Wn.Z[1][2], Wn.Z[2][0]);
-        sts2(sm0 + 3 * PK_SL, Wn.Z[2][1], Wn.Z[2][2]); sts2(sm0 + 4 * PK_SL, Wn.s[0], Wn.s[1]); sts2(sm0 + 5 * PK_SL, Wn.s[2], dhi[0]);
-        sts2(sm0 + 6 * PK_SL, dhi[1], dhi[2]);
-
-        double q2h, q2p, q2t, rd2, rd1;
-        if (DIR == 0) {
-            const unsigned sq = st0 + xprev + (r & 1) * 8u;                             // cell r-2 is in the previous group
-            q2h = lds1(sq); q2p = lds1(sq + PK_SL); q2t = lds1(sq + 2 * PK_SL); rd2 = rdrow; rd1 = rdrow;
-        } else {
-            lds2(sm0 + ro2, q2h, q2p); lds2(sm0 + ro2 + PK_SL, q2t, rd2);
-            rd1 = lds1(sm0 + ro1 + PK_SL + 8u);
-        }
+        // ---- B: edge r-2, standard-edge code
+        double dhi[3];                                                                  // Z(r-2) . Z(r-1) per family
+        dhi[0] = __fma_rn(W2.Z[0][2], Z1[2], __fma_rn(W2.Z[0][1], Z1[1], W2.Z[0][0] * Z1[0]));
+        dhi[1] = __fma_rn(W2.Z[1][2], Z1[4], __fma_rn(W2.Z[1][1], Z1[3], 0.0));
+        dhi[2] = __fma_rn(W2.Z[2][2], Z1[7], __fma_rn(W2.Z[2][1], Z1[6], W2.Z[2][0] * Z1[5]));
+        const double dtdx_ave = 0.5 * __fma_rn(dt, rd3, dt * rd2);
         double fm[3], fp[3];
-        {   // edge r-1: a standard edge (s[0] < 0 < s[2], solved by the fast path) needs no sign tests for families 1 and 3
-            MathFast mf;
-            if (stdc) gc_edge_flux_std(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
-            else gc_edge_flux_fast(mf, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp);
-            if (mf.failed()) { MathIeee mi; gc_edge_flux(mi, Wc, dlo, dhi, a.limiter, dt, rd2, rd1, fm, fp); }
+        const bool okB = gc_edge_flux_std(W2, dlo, dhi, dtdx_ave, fm, fp) && std2 && mc;
+        double cfle = gc_edge_cfl_std(W2, rd3, rd2);
+
+        // ---- lanes whose cell / edge is of another kind: general code, IEEE operators (same bits where both apply)
+        const bool needB = r >= 4 && r <= nst;
+        const bool badA = live && !(r >= 1 ? okR : okP);
+        const bool badB = needB && !okB;
+        if (__any_sync(0xffffffffu, badA || badB)) {
+            if (badA) {
+                MathIeee mi;
+                R.h = qh; R.p = qp; R.t = qt; R.b = qb;
+                gc_prim(mi, R, a.g, a.eps);
+                if (r >= 1) gc_riemann(mi, a.g, a.eps, Lst, R, Wn.Z, Wn.s);
+            }
+            if (badB) {
+                MathIeee mi;
+                gc_edge_flux(mi, W2, dlo, dhi, a.limiter, dt, rd3, rd2, fm, fp);
+                cfle = gc_edge_cfl(W2, rd3, rd2);
+            }
         }
-        if (live && r >= 3 && count) cflm = dmax(cflm, stdc ? gc_edge_cfl_std(Wc, rd2, rd1) : gc_edge_cfl(Wc, rd2, rd1));
-        double fpp[3], unused_;
-        lds2(sm0 + 7 * PK_SL, fpp[0], fpp[1]); lds2(sm0 + 8 * PK_SL, fpp[2], unused_);
-        sts2(sm0 + 7 * PK_SL, fp[0], fp[1]); sts2(sm0 + 8 * PK_SL, fp[2], 0.0);
-        if (live && r >= 4) {                                                           // cell r-2
-            const double dtdx = dt * rd2;
-            double uh = __fma_rn(-dtdx, fm[0] - fpp[0], q2h);
-            double up = __fma_rn(-dtdx, fm[1] - fpp[1], q2p);
-            double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q2t);
-            const int64_t o = base + (int64_t)(r - 2) * str;
+        if (SPH) {                                                                      // scale by the edge factor
+#pragma unroll
+            for (int w = 0; w < 3; w++) { Wn.s[w] = Wn.s[w] * ef; Wn.Z[w][0] = Wn.Z[w][0] * ef; Wn.Z[w][1] = Wn.Z[w][1] * ef; Wn.Z[w][2] = Wn.Z[w][2] * ef; }
+        }
+        Lst = R; Lok = okP;
+
+        // ---- edge r takes the place of edge r-2; Z(r-2).Z(r-1) and fp(r-2) for the next iteration
+        const double stdn = __longlong_as_double((long long)((okR && live && r >= 1) ? 1 : 0));
+        sts2(wa, Wn.Z[0][0], Wn.Z[0][1]); sts2(wa + PK_SL, Wn.Z[0][2], Wn.Z[1][1]); sts2(wa + 2 * PK_SL, Wn.Z[1][2], Wn.Z[2][0]);
+        sts2(wa + 3 * PK_SL, Wn.Z[2][1], Wn.Z[2][2]); sts2(wa + 4 * PK_SL, Wn.s[0], Wn.s[1]); sts2(wa + 5 * PK_SL, Wn.s[2], stdn);
+        sts2(sm0 + PK_DOT * PK_SL, dhi[0], dhi[1]); sts2(sm0 + (PK_DOT + 1) * PK_SL, dhi[2], fp[0]); sts2(sm0 + (PK_DOT + 2) * PK_SL, fp[1], fp[2]);
+
+        if (needB && count) cflm = dmax(cflm, cfle);
+        if (r >= 5 && r <= nst) {                                                       // cell r-3
+            const double dtdx = dt * rd3;
+            double uh = __fma_rn(-dtdx, fm[0] - fpp[0], q3h);
+            double up = __fma_rn(-dtdx, fm[1] - fpp[1], q3p);
+            double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q3t);
+            const int j = r - 3;
+            const int64_t o = base + (int64_t)j * str;
             if (DIR == 0) {
-                // cell j = r-2 of the row goes to slot (plane, (j >> 1) & 1); a full aligned group of 4 leaves as one store
-                const int j = r - 2;
+                // cell j of the row goes to slot (plane, (j >> 1) & 1); a full aligned group of 4 leaves as one store
                 const unsigned so = sm0 + (PK_XOUT + ((j >> 1) & 1)) * PK_SL + (j & 1) * 8u;
                 sts1(so, uh); sts1(so + 2 * PK_SL, up); sts1(so + 4 * PK_SL, ut);
                 if ((j & 3) == 3) {
@@ -572,7 +404,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
                 }
             } else {
                 if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
-                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[jrow + r - 2] * a.dxdy); }
+                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[jrow + j] * a.dxdy); }
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
                 }
                 if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
@@ -583,8 +415,6 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
             }
         }
-        stdc = stdn;
-        { const unsigned t = ro2; ro2 = ro1; ro1 = ro0; ro0 = t; }
     }
 
     if (DIR == 0 && nst >= 5) {                                  // x-sweep: the cells of the last, incomplete group
@@ -633,18 +463,19 @@ void gc_launch_stats_reset(gc_level *L) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_
 
 void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl) { ProfScope ps(L->ctx, GC_SLOT_MISC); k_next_dt<<<1, 1, 0, L->ctx->stream>>>(L->d_stats, dt_dev, cfl); }
 
-// GC_MARCH=regs selects the register-resident marching kernels (k_march); default: parked state (k_marchp).
-// Read at every launch (a getenv, no device work), so that one process can run both.
-static bool march_parked()
+template <int DIR>
+static void launch_march(gc_level *L, const SweepArgs &a, unsigned nb)
 {
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(k_marchp<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_X);
-        cudaFuncSetAttribute(k_marchp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PARK_BYTES_Y);
+        const int bytes = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_Y;
+        cudaFuncSetAttribute(k_marchp<DIR, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        cudaFuncSetAttribute(k_marchp<DIR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         attr_done = true;
     }
-    const char *e = getenv("GC_MARCH");
-    return !(e && !strcmp(e, "regs"));
+    const size_t bytes = DIR == 0 ? PARK_BYTES_X : PARK_BYTES_Y;
+    if (a.coord == 1) k_marchp<DIR, 1><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
+    else k_marchp<DIR, 0><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
 }
 
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out)
@@ -653,6 +484,8 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     int cur = L->cur, nxt = 1 - cur;
     SweepArgs a;
     a.pat = L->d_pat; a.g = P.g; a.eps = P.dry_tol; a.dt = dt; a.dt_dev = dt_dev;
+    // guarded open-ocean path (gc_riemann.cuh): its window argument assumes g within 2^+-20; otherwise it never applies
+    a.hlo = (P.g >= 0x1p-20 && P.g <= 0x1p20) ? (P.dry_tol > 0x1p-100 ? P.dry_tol : 0x1p-100) : INFINITY;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out; a.stats = L->d_stats;
     a.gn2 = P.g * (P.manning_n * P.manning_n); a.fdepth = P.friction_depth; a.friction = P.manning_n > 0.0 ? 1 : 0;
     a.lines = nullptr; a.nlines = 0;
@@ -664,9 +497,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
         a.lines = L->d_xl; a.nlines = L->nxl_lines;
         if (a.nlines > 0) {
             ProfScope ps(L->ctx, GC_SLOT_XSWEEP);
-            const unsigned nb = (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK);
-            if (march_parked()) k_marchp<0><<<nb, MARCH_BLOCK, PARK_BYTES_X, L->ctx->stream>>>(a);
-            else k_march<0><<<nb, MARCH_BLOCK, MARCH_STAGE_BYTES, L->ctx->stream>>>(a);
+            launch_march<0>(L, a, (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK));
         }
     } else if (L->nxt > 0) { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_sweep<0><<<L->nxt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
     // y-sweep: Q* -> Q^{n+1}
@@ -676,9 +507,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
         a.lines = L->d_yl; a.nlines = L->nyl_lines;
         if (a.nlines > 0) {
             ProfScope ps(L->ctx, GC_SLOT_YSWEEP);
-            const unsigned nb = (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK);
-            if (march_parked()) k_marchp<1><<<nb, MARCH_BLOCK, PARK_BYTES_Y, L->ctx->stream>>>(a);
-            else k_march<1><<<nb, MARCH_BLOCK, 0, L->ctx->stream>>>(a);
+            launch_march<1>(L, a, (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK));
         }
     } else if (L->nyt > 0) { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_sweep<1><<<L->nyt, SW_BLOCK, 0, L->ctx->stream>>>(a); }
 }

@@ -1,7 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the oracle, element by element on the same
 seeded inputs.  Bars (BASELINE.json north_star): wet masks bit-exact; dt within 1e-14 relative per step;
 h, hu, hv within 1e-12 relative per step and 1e-9 max|eta| at the end.  The design is bit-reproducible
-(-fmad=false on the device, -ffp-contract=off on the host), so the expected difference is exactly 0 and
+(fused multiply-adds only where DESIGN.md 3 writes them, on both sides), so the expected difference is exactly 0 and
 the tests assert that where noted."""
 import numpy as np
 import pytest
@@ -13,16 +13,13 @@ pytestmark = pytest.mark.gpu
 G = 9.81
 
 
-@pytest.fixture(autouse=True, params=["edge", "march", "march-regs"])
+@pytest.fixture(autouse=True, params=["edge", "march"])
 def sweep_mode(request, monkeypatch):
-    """Every sweep kernel family (edge-parallel tiles k_sweep / line-marching with parked state k_marchp / line-marching
-    with the state in registers k_march) must give the oracle's bits; the library picks one by level size
-    unless GC_SWEEP / GC_MARCH say otherwise (both are read when a level is created / a sweep is launched)."""
-    monkeypatch.setenv("GC_SWEEP", "edge" if request.param == "edge" else "march")
-    if request.param == "march-regs":
-        monkeypatch.setenv("GC_MARCH", "regs")
-    else:
-        monkeypatch.delenv("GC_MARCH", raising=False)
+    """Both sweep kernel families (edge-parallel tiles k_sweep / line marching k_marchp) must give the oracle's
+    bits; the library picks one by level size unless gc_ctx_set_option says otherwise (read when a level is created)."""
+    from paper_1901_06798_b200 import binding
+    fam = binding.SWEEP_EDGE if request.param == "edge" else binding.SWEEP_MARCH
+    monkeypatch.setitem(binding.DEFAULT_OPTIONS, binding.OPT_SWEEP_FAMILY, fam)
     return request.param
 
 
