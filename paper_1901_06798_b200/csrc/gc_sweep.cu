@@ -32,6 +32,7 @@ struct SweepArgs {
     const double *ey;                // y edge factors per global edge (+2)
     double ex;
     double g, eps;
+    double hg;                       // 0.5 * g
     double hlo;                      // max(eps, 2^-100): lower depth bound of the guarded open-ocean path
     double dt; const double *dt_dev; // dt_dev != NULL: read dt from device memory
     int coord, limiter, write_out;
@@ -88,7 +89,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
         qh = R.h; qp = R.p; qt = R.t;
         {   // guarded open-ocean code first; any other edge is redone with the general code (same bits where both apply)
             RState Lf = L, Rf = R;
-            const bool okL = gc_prim_fast(Lf, a.g, 0.5 * a.g, a.hlo), okR = gc_prim_fast(Rf, a.g, 0.5 * a.g, a.hlo);
+            const bool okL = gc_prim_fast(Lf, a.g, a.hg, a.hlo), okR = gc_prim_fast(Rf, a.g, a.hg, a.hlo);
             stdE = gc_riemann_fast(a.g, Lf, Rf, Z, s) && okL && okR;
         }
         if (!stdE) {
@@ -243,9 +244,6 @@ __device__ __forceinline__ void cpa8(unsigned sdst, const double *gsrc)
 template <int DIR, int SPH>
 __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 {
-    __shared__ double sred[MARCH_BLOCK / 32];
-    __shared__ unsigned long long sclip[MARCH_BLOCK / 32];
-    __shared__ double sclipm[MARCH_BLOCK / 32];
     extern __shared__ __align__(16) double dsm[];
     const unsigned sm0 = (unsigned)__cvta_generic_to_shared(dsm) + threadIdx.x * 16u;
 
@@ -264,14 +262,13 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
     const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
     const int jrow = pd.j0 + cfirst;                             // y-sweep: global row (+2) of the first cell read
-    const double hg = 0.5 * a.g;
     const bool mc = a.limiter != 0;
 
 #pragma unroll
     for (int k = 0; k < PK_RING; k++) sts2(sm0 + k * PK_SL, 0.0, 0.0);
     RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
     bool Lok = false;                                            // cell r-1 passed gc_prim_fast
-    double cflm = 0.0, clipm = 0.0; unsigned nclip = 0; int nanf = 0;
+    double cflm = 0.0;
 
     // staging: thread-private slots, filled by cp.async one group (x: 2 cells, y: 1 cell) ahead of their use
     const unsigned st0 = (DIR == 0) ? sm0 + PK_XST * PK_SL : (unsigned)__cvta_generic_to_shared(dsm) + PK_YSTAGE * PK_SL + threadIdx.x * 8u;
@@ -313,21 +310,17 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 
         // ---- parked state: edge r-2 (its set is overwritten by edge r below), the waves of edge r-1, Z(r-3).Z(r-2), fp(r-3)
         const unsigned wa = sm0 + (unsigned)(r & 1) * (6 * PK_SL), wb = sm0 + (unsigned)((r & 1) ^ 1) * (6 * PK_SL);
-        Waves W2; double Z1[8], dlo[3], fpp[3], std2d;
+        Waves W2; double Z1[8], dlo[3], fp3_0, std2d;
         lds2(wa, W2.Z[0][0], W2.Z[0][1]); lds2(wa + PK_SL, W2.Z[0][2], W2.Z[1][1]); lds2(wa + 2 * PK_SL, W2.Z[1][2], W2.Z[2][0]);
         lds2(wa + 3 * PK_SL, W2.Z[2][1], W2.Z[2][2]); lds2(wa + 4 * PK_SL, W2.s[0], W2.s[1]); lds2(wa + 5 * PK_SL, W2.s[2], std2d);
         W2.Z[1][0] = 0.0;
         lds2(wb, Z1[0], Z1[1]); lds2(wb + PK_SL, Z1[2], Z1[3]); lds2(wb + 2 * PK_SL, Z1[4], Z1[5]); lds2(wb + 3 * PK_SL, Z1[6], Z1[7]);
-        lds2(sm0 + PK_DOT * PK_SL, dlo[0], dlo[1]); lds2(sm0 + (PK_DOT + 1) * PK_SL, dlo[2], fpp[0]); lds2(sm0 + (PK_DOT + 2) * PK_SL, fpp[1], fpp[2]);
+        lds2(sm0 + PK_DOT * PK_SL, dlo[0], dlo[1]); lds2(sm0 + (PK_DOT + 1) * PK_SL, dlo[2], fp3_0);
         const bool std2 = __double2loint(std2d) != 0;
-        double q3h, q3p, q3t, rd3, rd2;                                                 // raw cell r-3; 1/(kappa dx) of cells r-3, r-2
-        if (DIR == 0) {
-            const unsigned sq = st0 + (((r - 3) >> 1) & 3) * (4 * PK_SL) + ((r + 1) & 1) * 8u;
-            q3h = lds1(sq); q3p = lds1(sq + PK_SL); q3t = lds1(sq + 2 * PK_SL); rd3 = rdrow; rd2 = rdrow;
-        } else {
-            const unsigned k3 = sm0 + (PK_RING + 2 * ((r + 1) & 3)) * PK_SL, k2 = sm0 + (PK_RING + 2 * ((r + 2) & 3)) * PK_SL;
-            lds2(k3, q3h, q3p); lds2(k3 + PK_SL, q3t, rd3);
-            rd2 = lds1(k2 + PK_SL + 8u);
+        double rd3 = rdrow, rd2 = rdrow;                                                // 1/(kappa dx) of cells r-3, r-2
+        if (DIR == 1) {
+            rd3 = lds1(sm0 + (PK_RING + 2 * ((r + 1) & 3) + 1) * PK_SL + 8u);
+            rd2 = lds1(sm0 + (PK_RING + 2 * ((r + 2) & 3) + 1) * PK_SL + 8u);
             const unsigned k0 = sm0 + (PK_RING + 2 * (r & 3)) * PK_SL;
             sts2(k0, qh, qp); sts2(k0 + PK_SL, qt, rd0);
         }
@@ -335,7 +328,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         // ---- A: cell r and edge r, guarded open-ocean code
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
         Waves Wn;
-        const bool okP = gc_prim_fast(R, a.g, hg, a.hlo);
+        const bool okP = gc_prim_fast(R, a.g, a.hg, a.hlo);
         const bool okR = gc_riemann_fast(a.g, Lst, R, Wn.Z, Wn.s) && okP && Lok;
 
         // ---- B: edge r-2, standard-edge code
@@ -371,6 +364,18 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         }
         Lst = R; Lok = okP;
 
+        // ---- what the update of cell r-3 needs comes back only now (not held in registers across A and B): fp(r-3), raw cell r-3
+        double fpp[3], q3h, q3p, q3t, unused_;
+        fpp[0] = fp3_0;
+        lds2(sm0 + (PK_DOT + 2) * PK_SL, fpp[1], fpp[2]);
+        if (DIR == 0) {
+            const unsigned sq = st0 + (((r - 3) >> 1) & 3) * (4 * PK_SL) + ((r + 1) & 1) * 8u;
+            q3h = lds1(sq); q3p = lds1(sq + PK_SL); q3t = lds1(sq + 2 * PK_SL);
+        } else {
+            const unsigned k3 = sm0 + (PK_RING + 2 * ((r + 1) & 3)) * PK_SL;
+            lds2(k3, q3h, q3p); lds2(k3 + PK_SL, q3t, unused_);
+        }
+
         // ---- edge r takes the place of edge r-2; Z(r-2).Z(r-1) and fp(r-2) for the next iteration
         const double stdn = __longlong_as_double((long long)((okR && live && r >= 1) ? 1 : 0));
         sts2(wa, Wn.Z[0][0], Wn.Z[0][1]); sts2(wa + PK_SL, Wn.Z[0][2], Wn.Z[1][1]); sts2(wa + 2 * PK_SL, Wn.Z[1][2], Wn.Z[2][0]);
@@ -404,14 +409,17 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
                 }
             } else {
                 if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
-                    if (uh < 0.0) { nclip++; clipm += (-uh) * (a.kappa[jrow + j] * a.dxdy); }
+                    if (uh < 0.0) {                                                      // rare: straight to the level's counters
+                        atomicAdd(&a.stats->nclip, 1ull);
+                        atomicAdd(&a.stats->clipped, (-uh) * (a.kappa[jrow + j] * a.dxdy));
+                    }
                     uh = dmax(uh, 0.0); up = 0.0; ut = 0.0;
                 }
                 if (a.friction && a.write_out) {                                                   // DESIGN.md 3.9; (hu, hv) = (ut, up)
                     const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, dt, uh, ut, up);
                     ut = q.x; up = q.y;
                 }
-                if (uh != uh || up != up || ut != ut) nanf = 1;
+                if (uh != uh || up != up || ut != ut) a.stats->nan_seen = 1;
                 if (a.write_out) { a.oh[o] = uh; a.ohv[o] = up; a.ohu[o] = ut; }
             }
         }
@@ -427,28 +435,9 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         }
     }
 
+    // A7: exact, order-independent max: warp shuffle, then one atomicMax per warp on the bit image (values >= 0)
     cflm = warp_max(cflm);
-    if (DIR == 1) {
-        nclip = __reduce_add_sync(0xffffffffu, nclip);
-        nanf = __any_sync(0xffffffffu, nanf);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) clipm += __shfl_xor_sync(0xffffffffu, clipm, o);
-    }
-    const int k = threadIdx.x;
-    if ((k & 31) == 0) { sred[k >> 5] = cflm; if (DIR == 1) { sclip[k >> 5] = nclip; sclipm[k >> 5] = clipm; if (nanf) a.stats->nan_seen = 1; } }
-    __syncthreads();
-    if (k == 0) {
-        double m = sred[0];
-#pragma unroll
-        for (int w = 1; w < MARCH_BLOCK / 32; w++) m = dmax(m, sred[w]);
-        if (m > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(m));
-        if (DIR == 1) {
-            unsigned long long n = 0; double cm = 0.0;
-#pragma unroll
-            for (int w = 0; w < MARCH_BLOCK / 32; w++) { n += sclip[w]; cm += sclipm[w]; }
-            if (n) { atomicAdd(&a.stats->nclip, n); atomicAdd(&a.stats->clipped, cm); }
-        }
-    }
+    if ((threadIdx.x & 31) == 0 && cflm > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(cflm));
 }
 
 __global__ void k_stats_reset(DevStats *s) { s->sdx_bits = 0ull; s->nclip = 0ull; s->clipped = 0.0; s->nan_seen = 0; }
@@ -483,7 +472,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     const gc_params &P = L->ctx->P;
     int cur = L->cur, nxt = 1 - cur;
     SweepArgs a;
-    a.pat = L->d_pat; a.g = P.g; a.eps = P.dry_tol; a.dt = dt; a.dt_dev = dt_dev;
+    a.pat = L->d_pat; a.g = P.g; a.hg = 0.5 * P.g; a.eps = P.dry_tol; a.dt = dt; a.dt_dev = dt_dev;
     // guarded open-ocean path (gc_riemann.cuh): its window argument assumes g within 2^+-20; otherwise it never applies
     a.hlo = (P.g >= 0x1p-20 && P.g <= 0x1p20) ? (P.dry_tol > 0x1p-100 ? P.dry_tol : 0x1p-100) : INFINITY;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out; a.stats = L->d_stats;
