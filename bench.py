@@ -119,7 +119,7 @@ def oracle_rate(n, steps, warmup=0):
     """The oracle as it stands, one thread: config-5 recipe at n x n, one patch.  -> (updates/s, seconds)"""
     import workloads
     from oracle import gco
-    from paper_1901_06798_b200 import driver
+    from harness import driver
     wl = workloads.cfg5(n)
     L = driver.setup_level(gco.Context(**wl.params), wl)
     dt = driver.probe_dt(L, wl.cfl)
@@ -171,7 +171,8 @@ def main():
     import numpy as np
     import torch
     import workloads
-    from paper_1901_06798_b200 import binding, driver
+    from paper_1901_06798_b200 import binding
+    from harness import driver
 
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)

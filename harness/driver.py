@@ -1,12 +1,10 @@
-"""Host control code: time-step control and the AMR recursion (section 3.1), regridding
-cadence and Berger-Rigoutsos clustering.  Everything here is bookkeeping: every
-arithmetic step of the method runs in the kernels behind the C ABI (include/gc.h).  The driver talks
-to a *backend* (an object with level_create(...) returning Level objects with the methods of
-binding.Level); the product backend is paper_1901_06798_b200.binding.Context.  Tests drive the
-oracle through the same code to compare the two.
+"""Neutral AMR harness: time-step control and the AMR recursion (section 3.1),
+regridding cadence and Berger-Rigoutsos clustering.  Everything here is bookkeeping: every
+arithmetic step of the method runs behind a *backend* -- an object with level_create(...) returning Level objects
+with the methods of paper_1901_06798_b200.binding.Level (the product, through the C ABI of include/gc.h) or of
+oracle.gco.Level (the oracle).  This package imports neither; tests drive both through it to compare them, and
+tests/test_harness_pins.py pins the recursion itself against a straight-line script and a uniformly fine run.
 """
-import os
-
 import numpy as np
 
 
@@ -284,10 +282,10 @@ class Hierarchy:
     """The AMR recursion of P:140-146 (steps 1-5) with regridding every `regrid_interval` steps of a level,
     driving one backend through the C-ABI calls.  Bookkeeping only."""
 
-    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7, gauges=None):
+    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7, gauges=None, keep_unchanged=True):
         self.ctx, self.wl, self.reflux, self.eff = ctx, wl, reflux, efficiency
         self.gauges = gauges             # GaugeRecorder or None (DESIGN.md 3.10)
-        self.keep_unchanged = os.environ.get("GC_REGRID_KEEP", "1") != "0"   # keep a level whose regrid reproduces its patch list
+        self.keep_unchanged = keep_unchanged   # keep a level whose regrid reproduces its patch list (bit-identical to recreating it)
         self.kept = 0
         nl = 1 + len(wl.ratios) if max_levels is None else min(max_levels, 1 + len(wl.ratios))
         self.ratios = list(wl.ratios)[:nl - 1]

@@ -1,6 +1,6 @@
 """Run one of the five BASELINE.json configurations on the GPU and report its end-to-end rate.
 
-    python -m paper_1901_06798_b200.run_config --config N [--scale S] [--max-steps M] [--max-wall SECONDS] [--graph K]
+    python -m harness.run_config --config N [--scale S] [--max-steps M] [--max-wall SECONDS] [--graph K]
 
 Prints ONE JSON line: total interior-cell updates over all levels / wall time of the whole run (ghost fills, level
 steps, regrids incl. flag download and host clustering, average-down, fix-up), the kernel launches, and how far the run
@@ -18,7 +18,8 @@ import numpy as np
 
 def run_single(cfg, wl, patches, max_steps, graph_k, device):
     import torch
-    from . import binding, driver
+    from paper_1901_06798_b200 import binding
+    from harness import driver
     s = torch.cuda.Stream(device=device)
     with torch.cuda.stream(s):
         ctx = binding.Context(device=device, stream=s, **wl.params)
@@ -75,7 +76,8 @@ def run_single(cfg, wl, patches, max_steps, graph_k, device):
 
 def run_amr(cfg, wl, max_steps, max_wall, device, max_levels=None):
     import torch
-    from . import binding, driver
+    from paper_1901_06798_b200 import binding
+    from harness import driver
     ctx = binding.Context(device=device, **wl.params)
     t_setup = time.time()
     H = driver.Hierarchy(ctx, wl, max_levels=max_levels)

@@ -21,7 +21,7 @@ OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_anchors.t
 def anchors():
     import workloads
     from oracle import gco
-    from paper_1901_06798_b200 import driver      # host control code shared by both backends; no kernels are loaded
+    from harness import driver                    # neutral AMR harness (host control code); nothing under paper_1901_06798_b200 is imported
     rows = []
 
     def put(key, values, cite):

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import workloads
-from paper_1901_06798_b200 import driver
+from harness import driver
 
 pytestmark = pytest.mark.gpu
 

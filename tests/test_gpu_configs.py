@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import workloads
-from paper_1901_06798_b200 import driver
+from harness import driver
 from test_gpu_amr import lockstep_hierarchies, same_storage
 
 pytestmark = pytest.mark.gpu

@@ -9,7 +9,7 @@ import pytest
 from scipy import ndimage
 
 import workloads
-from paper_1901_06798_b200 import driver
+from harness import driver
 
 G = 9.81
 CART = dict(coord=0, dry_tol=1e-3, bc=(1, 1, 1, 1))
@@ -236,8 +236,8 @@ def test_keeping_a_level_whose_regrid_reproduces_it_changes_no_bit(gco, monkeypa
         wl = workloads.Workload("amr3", base.params, 0.0, 0.0, base.dx, base.dy, 24, 24, base.bathy, base.eta0, cfl=0.9,
                                 ratios=(2, 3), flag=dict(tol_eta=0.25, buffer=1), regrid_interval=2, patch_max=18)
         n = 8
-    monkeypatch.setenv("GC_REGRID_KEEP", "1"); Ha, da = _run_hierarchy(gco, wl, n, **kw)
-    monkeypatch.setenv("GC_REGRID_KEEP", "0"); Hb, db = _run_hierarchy(gco, wl, n, **kw)
+    Ha, da = _run_hierarchy(gco, wl, n, keep_unchanged=True, **kw)
+    Hb, db = _run_hierarchy(gco, wl, n, keep_unchanged=False, **kw)
     assert Hb.kept == 0 and da == db and Ha.regrids == Hb.regrids and len(Ha.levels) == len(Hb.levels)
     if case.startswith("four_levels"):
         assert Ha.kept >= 30 and len(Ha.levels) == 4                         # the fixed-box levels came back unchanged every time

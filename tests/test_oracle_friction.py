@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 import workloads
-from paper_1901_06798_b200 import driver
+from harness import driver
 from test_oracle_2d import make_level, shoreline_case
 
 G = 9.81

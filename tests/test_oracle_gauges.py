@@ -8,7 +8,7 @@ import pytest
 from scipy.interpolate import RegularGridInterpolator
 
 import workloads
-from paper_1901_06798_b200 import driver
+from harness import driver
 from test_oracle_2d import make_level
 
 
