@@ -306,8 +306,8 @@ class Hierarchy:
             R *= r
         return self.wl.dx / R, self.wl.dy / R, self.wl.nx * R, self.wl.ny * R
 
-    def _flag_boxes(self, k):
-        """flag level k, cluster -> patches of level k+1 (in cells of level k+1), or None"""
+    def _flag_boxes(self, k, t):
+        """flag level k at its current time t, cluster -> patches of level k+1 (in cells of level k+1), or None"""
         L = self.levels[k]
         f = dict(self.wl.flag)
         # a box that refines level lv -> lv + 1 needs every coarser level underneath: it flags levels 1..lv (P:160)
@@ -315,11 +315,11 @@ class Hierarchy:
         wave = k + 1 <= self.wl.wave_levels and f.get("tol_eta", 0.0) > 0.0
         # nothing can flag this level now (no wave criterion here, no box whose window [t0, t1] holds t -- the test the
         # flag kernel applies): the pass would return no flags, so it is not launched and nothing is downloaded
-        if not wave and not any(b[4] <= self.t <= b[5] for b in boxes):
+        if not wave and not any(b[4] <= t <= b[5] for b in boxes):
             return None
         packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0) if wave else 0.0, tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
-                           buffer=f.get("buffer", 0), boxes=boxes, t=self.t)
-        self.flag_log.append((k, self.t, packed.copy()))
+                           buffer=f.get("buffer", 0), boxes=boxes, t=t)
+        self.flag_log.append((k, t, packed.copy()))
         if n == 0:
             return None
         bbox = level_bbox(L)
@@ -332,14 +332,16 @@ class Hierarchy:
         boxes = cluster(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
         return np.array([[(b[0] + bbox[0]) * r, (b[1] + bbox[1]) * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
 
-    def _regrid(self, k0, initial=False):
-        """rebuild levels k0+1.. from the flags of the level below each"""
+    def _regrid(self, k0, initial=False, t=None):
+        """rebuild levels k0+1.. from the flags of the level below each; t = the time the levels k0.. have reached
+        (a level regrids at the end of one of its own steps, when it and every finer level stand at the same time)"""
+        t = self.t if t is None else t
         self.regrids += 0 if initial else 1
         for k in range(k0, len(self.ratios)):
             if k >= len(self.levels):
                 break
             C = self.levels[k]
-            pats = self._flag_boxes(k)
+            pats = self._flag_boxes(k, t)
             old = self.levels[k + 1] if k + 1 < len(self.levels) else None
             if pats is None:
                 for L in self.levels[k + 1:]:
@@ -404,7 +406,7 @@ class Hierarchy:
                 L.flux_fixup(F)
             L.average_down_from(F)
         if k > 0 and k < len(self.ratios) and self.steps[k] % self.wl.regrid_interval == 0:
-            self._regrid(k)
+            self._regrid(k, t=t + dt)
 
     def step(self, dt):
         """one step of level 1 (and everything above it); returns the next dt of level 1"""
