@@ -1,13 +1,14 @@
 /* gco.h -- ORACLE (test infrastructure, NOT the product).
  *
- * Plain, slow, single-threaded fp64 CPU implementation of the per-level time step of
+ * Plain, slow fp64 CPU implementation (single-threaded unless gco_set_threads says otherwise) of the per-level time step of
  * GPU GeoClaw ("Efficient Tsunami Modeling on Adaptive Grids with GPUs", arXiv 1901.06798;
  * PAPER.md = P:<line>), written from the paper and from DESIGN.md section 3 (the readings of
  * every point the paper leaves open).  It shares no code with paper_1901_06798_b200/ (the CUDA
  * path) and neither includes the other.  Only tests/, __graft_entry__.smoke() and bench.py's
  * cpu_baseline / --impl reference legs may load it.
  *
- * Build: gcc -O2 -ffp-contract=off -fno-fast-math (see oracle/gco.py).  No FMA contraction, IEEE
+ * Build: gcc -O2 -ffp-contract=off -fno-fast-math (see oracle/gco.py).  C99 fma() exactly where DESIGN.md 3.3-3.4 write it, no
+ * other contraction, IEEE
  * sqrt and divide; min/max are written as ternaries (max2/min2) so that signed zeros and
  * ties behave identically everywhere.
  *
@@ -104,6 +105,10 @@ int gco_level_get_global(const gco_level *, int field, int which, double *dst, i
 int gco_fill_ghost_b(gco_level *);
 int gco_fill_ghost(gco_level *L, const gco_level *coarser, double alpha);
 int gco_level_step(gco_level *L, double dt, gco_step_stats *out);
+/* threads for gco_level_step's loop over patches (default 1; no result bit depends on it: patches are independent inside a step,
+ * SURVEY 8(d) "patch-level omp parallel for"); used by bench.py's N-core baseline and by the long parity runs */
+int gco_set_threads(int n);
+int gco_get_threads(void);
 /* ---- gauges (gco_amr.c); DESIGN.md 3.10 (reading S-19) ---- */
 /* Samples n points from the current state of L (ghost cells as they are): point k = (xy[2k], xy[2k+1]) must lie in the interior
  * of patch patch[k] (else GCO_ERR_BADARG).  out: 4 per point -- h, hu, hv, eta = h + b; bilinear between the four cell centres

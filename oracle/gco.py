@@ -13,15 +13,37 @@ import numpy as np
 _DIR = os.path.dirname(os.path.abspath(__file__))
 _SRC = ["gco_riemann.c", "gco_sweep.c", "gco_level.c", "gco_amr.c", "gco_flux.c"]
 _LIB = os.path.join(_DIR, "libgco.so")
-CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-Wall", "-shared", "-fPIC"]
+CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-Wall", "-shared", "-fPIC", "-fopenmp"]
+
+
+def _cpu_has_fma():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    return " fma " in line + " "
+    except OSError:
+        pass
+    return False
+
+
+def _flags():
+    """-mfma where the host has it: the C99 fma() calls DESIGN.md 3.1 specifies then compile to the hardware instruction instead
+    of a libm call (same correctly rounded result either way; -ffp-contract=off still forbids every other contraction)"""
+    return CFLAGS + (["-mfma"] if _cpu_has_fma() else [])
 
 
 def build(force=False):
     srcs = [os.path.join(_DIR, s) for s in _SRC]
     deps = srcs + [os.path.join(_DIR, "gco.h"), os.path.join(_DIR, "gco_int.h")]
-    if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in deps):
+    tag = os.path.join(_DIR, "libgco.flags")
+    want = " ".join(_flags())
+    have = open(tag).read() if os.path.exists(tag) else ""
+    if not force and have == want and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in deps):
         return _LIB
-    subprocess.check_call(["gcc"] + CFLAGS + ["-o", _LIB] + srcs + ["-lm"])
+    subprocess.check_call(["gcc"] + _flags() + ["-o", _LIB] + srcs + ["-lm"])
+    with open(tag, "w") as f:          # a library built for another host's instruction set (it travels with the tree) is rebuilt
+        f.write(want)
     return _LIB
 
 
@@ -75,6 +97,13 @@ def lib():
         _lib.gco_ctx_destroy.argtypes = [C.c_void_p]
         _lib.gco_sweep_line.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6 + [C.c_double] + [C.c_void_p] * 5 + [C.c_int, C.c_void_p]
     return _lib
+
+
+def set_threads(n):
+    """threads of the level step's loop over patches (default 1); returns the number in use.  n = 0: all host cores."""
+    n = (os.cpu_count() or 1) if n == 0 else int(n)
+    _chk(lib().gco_set_threads(n), "set_threads")
+    return lib().gco_get_threads()
 
 
 def _chk(rc, what):
