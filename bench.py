@@ -6,9 +6,21 @@ one spherical level of NxN cells (default 8192 x 8192, 0.5 arcmin) tiled into sq
 
 A "step" = gc_fill_ghost + gc_level_step_auto (dt chain on the device, no host sync) over the whole level.
 metric  = fp64 cell updates/s (interior cells x steps / device time, CUDA events, max over ranks).
-N > 1   = replicas only (the contract fixes one GPU per problem; no collective is invented): every rank
-          advances its own copy of the workload; value = units all ranks processed / max time.
---impl reference = the oracle (plain C, one thread) timed on a bounded sample of the same recipe on the host cores.
+config.tilings = the same step on the five tilings BASELINE.json's configs[4] names (sides 16 ... 256), each with its updates/s,
+          HBM GB/s at 56 B per update and fp64-pipe slot fraction (N = 1 only).
+roofline = the dominant sweep kernel against the DFMA rate measured in this run ("alu": the scheme is bound by the fp64 pipe,
+          DESIGN.md 6).  Its per-cell instruction counts and its DRAM traffic come from profiles/r02_counts.json, which
+          paper_1901_06798_b200/counts.py writes from an ncu capture together with a hash of the kernel sources; when the
+          sources have changed since, the counts are NOT printed (null) and the roofline falls back to the algorithmic bytes.
+e2e     = the same metric through the C ABI with HOST buffers: every step uploads its state from pinned host memory and reads the
+          result back.  "value": copies overlapped with the kernels (gc_level_upload_state_async / download, three streams, two
+          level pools used alternately, the pattern of P:174-186); "serial": copy, step, copy in sequence.
+cpu_baseline = the oracle (oracle/, plain C) on the SAME workload (8192 x 8192 in patches of 256), its loop over patches on all
+          host cores, core count stated, and on one core.
+N > 1   = replicas only (the contract fixes one GPU per problem; no collective is invented): every rank advances its
+          own copy of the workload; value = units all ranks processed / max time.  Launch with torch.distributed.run; --gpus must
+          equal WORLD_SIZE.
+--impl reference = the oracle alone, timed on the host cores on the same workload (rank 0 only).
 """
 import argparse
 import json
@@ -21,19 +33,10 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# Algorithmic work per cell per sweep, counted per kernel from the ncu source page of the default marching
-# kernels k_marchp<0> (x-sweep) / k_marchp<1> (y-sweep), profiles/r01_marchp.md: thread instructions / cells of one launch.
-#   x-sweep: 140.7 DMUL + 103.7 DADD + 81.2 DFMA (x 2 flops) = 407 flops, + 60.5 DSETP = 386 fp64-pipe instructions
-#   y-sweep: 143.9 DMUL + 104.8 DADD + 81.2 DFMA (x 2 flops) = 411 flops, + 64.6 DSETP = 394 fp64-pipe instructions
-# (divides and square roots expanded into their correctly rounded Newton sequences; no FMA contraction elsewhere)
-FLOP_PER_SWEEP = {"xsweep": 407.0, "ysweep": 411.0}
-FP64_SLOTS_PER_SWEEP = {"xsweep": 386.0, "ysweep": 394.0}
 BYTES_PER_UPDATE = 56.0   # read h, hu, hv, b + write h, hu, hv once; the two-pass design moves 112
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of each sweep kernel at the bench size 8192^2 / side 256, from the
-# ncu --set full capture summarised in profiles/r01_marchp.md (k_marchp; not valid for GC_MARCH=regs or GC_SWEEP=edge)
-NCU_TRAFFIC_BYTES = {"xsweep": 4.385e9, "ysweep": 3.906e9}
 METRIC = "fp64 cell updates/sec per level step (device-timed)"
 UNIT = "cell updates/s"
+COUNTS = os.path.join(ROOT, "profiles", "r02_counts.json")
 
 
 def peaks():
@@ -41,6 +44,17 @@ def peaks():
     if os.path.exists(p):
         return json.load(open(p)).get("hbm_gbs", 6650.0), "measured"
     return 6650.0, "fallback"
+
+
+def load_counts():
+    """per-kernel counts of the committed ncu capture, or None when the sources have changed since it was taken"""
+    if not os.path.exists(COUNTS):
+        return None, "profiles/r02_counts.json missing"
+    c = json.load(open(COUNTS))
+    from paper_1901_06798_b200.counts import source_hash
+    if c.get("source_sha256") != source_hash():
+        return None, "kernel sources changed since the capture (hash differs): counts withheld"
+    return c, "profiles/r02_counts.json (written by paper_1901_06798_b200/counts.py from %s)" % c.get("capture", "?")
 
 
 class ClockSampler:
@@ -115,36 +129,67 @@ def job_rate(units_per_rank, world, seconds):
     return world * units_per_rank / seconds
 
 
-def oracle_rate(n, steps, warmup=0):
-    """The oracle as it stands, one thread: config-5 recipe at n x n, one patch.  -> (updates/s, seconds)"""
+def host_fields(wl, n):
+    """the seeded analytic inputs of config 5 at every cell centre, generated on the host in row blocks -> dict of (n, n) arrays"""
+    import numpy as np
+    out = {f: np.empty((n, n)) for f in ("b", "h", "hu", "hv")}
+    rows = max(1, (1 << 24) // n)
+    for j0 in range(0, n, rows):
+        nr = min(rows, n - j0)
+        for f, v in zip(("b", "h", "hu", "hv"), wl.fields(i0=0, j0=j0, nx=n, ny=nr)):
+            out[f][j0:j0 + nr] = v
+    return out
+
+
+def oracle_leg(wl, n, side, fields, steps, warmup, threads, budget_s=None):
+    """The oracle as it stands on the bench workload (n x n in patches of `side`), its loop over patches on `threads` host
+    cores (0 = all).  steps = None: as many steps as fit budget_s after the first.  -> (updates/s, seconds, steps, threads)"""
     import workloads
     from oracle import gco
-    from harness import driver
-    wl = workloads.cfg5(n)
-    L = driver.setup_level(gco.Context(**wl.params), wl)
-    dt = driver.probe_dt(L, wl.cfl)
+    nt = gco.set_threads(threads)
+    L = gco.Context(**wl.params).level_create(1, wl.xlo, wl.ylo, wl.dx, wl.dy, n, n, 1, workloads.tile(n, n, side))
+    for f in ("b", "h", "hu", "hv"):
+        L.set_global(f, fields[f])
+    L.fill_ghost_b(); L.fill_ghost(None, 1.0)
+    dt = wl.cfl / L.step(0.0)["s_over_dx_max"]
+
+    def one(dt):
+        L.fill_ghost(None, 1.0)
+        return wl.cfl / L.step(dt)["s_over_dx_max"]
     for _ in range(warmup):
-        L.fill_ghost(None, 1.0); st = L.step(dt); dt = wl.cfl / st["s_over_dx_max"]
+        dt = one(dt)
     t0 = time.time()
-    for _ in range(steps):
-        L.fill_ghost(None, 1.0); st = L.step(dt); dt = wl.cfl / st["s_over_dx_max"]
+    dt = one(dt)
+    first = time.time() - t0
+    k = 1
+    if steps is None:
+        steps = max(1, min(50, int(budget_s / max(first, 1e-3))))
+    while k < steps:
+        dt = one(dt); k += 1
     el = time.time() - t0
-    return n * n * steps / el, el
+    L.destroy(); gco.set_threads(1)
+    return n * n * k / el, el, k, nt
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """--impl reference: there is no reference implementation to install (/root/reference holds the paper only); the oracle, as it
+    stands, is timed on the host cores on the same workload.  Rank 0 alone runs and prints; the other ranks exit 0 without work."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
-    n = 1024
-    rate, el = oracle_rate(n, args.steps, args.warmup)
-    sample = "config-5 recipe at %dx%d (one patch), %d steps, single thread" % (n, n, args.steps)
+    import workloads
+    n, side = args.n, args.side
+    wl = workloads.cfg5(n)
+    fields = host_fields(wl, n)
+    rate, el, k, nt = oracle_leg(wl, n, side, fields, max(args.steps, 1), args.warmup, 0)
+    sample = "cfg5 spherical %dx%d in patches of side %d (the whole workload), %d steps after %d warm-up, loop over patches on %d threads" \
+             % (n, n, side, k, args.warmup, nt)
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * el / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / k, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "cfg5 spherical single level, oracle sample", "sample": sample},
-        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "config": {"workload": "cfg5: spherical single level %dx%d at 0.5 arcmin, patches of side %d, ghost fill + level step (oracle)" % (n, n, side),
+                   "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": nt, "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -156,10 +201,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--n", type=int, default=8192, help="level is n x n cells")
-    ap.add_argument("--side", type=int, default=256, help="patch side")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--side", type=int, default=256, help="patch side of the headline line")
+    ap.add_argument("--e2e-steps", type=int, default=4)
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
-    ap.add_argument("--sweep", action="store_true", help="also report every tiling 16..256 in config.tilings")
+    ap.add_argument("--no-tilings", action="store_true", help="skip config.tilings (sides 16 ... 256)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end legs")
     ap.add_argument("--gauges", type=int, default=0,
                     help="bind this many seeded gauges and record them into a device-resident series every step (DESIGN.md 3.10)")
     ap.add_argument("--manning", type=float, default=0.0,
@@ -177,26 +223,27 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     rank, world, local, dist = init_ranks("nccl", torch.device("cuda", local))
+    assert args.gpus == world, "--gpus %d but WORLD_SIZE %d: launch N > 1 with torch.distributed.run (one rank per GPU)" % (args.gpus, world)
     dev = "cuda:%d" % local
-    W = max(args.warmup, 3)
+    W = args.warmup
     n = args.n
     wl = workloads.cfg5(n)
     if args.manning > 0.0:
         wl.params = dict(wl.params, manning_n=args.manning)
     ctx = binding.Context(device=dev, **wl.params)
+    fields = host_fields(wl, n)
 
     def make(side):
         L = ctx.level_create(1, wl.xlo, wl.ylo, wl.dx, wl.dy, n, n, 1, workloads.tile(n, n, side))
-        # inputs generated on the host in row blocks (bounded memory), handed over through the C ABI
-        rows = max(1, (1 << 24) // n)
+        rows = max(1, (1 << 24) // n)          # handed over through the C ABI in row blocks (bounded staging)
         for j0 in range(0, n, rows):
-            nr = min(rows, n - j0)
-            b, h, hu, hv = wl.fields(i0=0, j0=j0, nx=n, ny=nr)
-            L.set_global("b", b, 0, j0); L.set_global("h", h, 0, j0); L.set_global("hu", hu, 0, j0); L.set_global("hv", hv, 0, j0)
+            for f in ("b", "h", "hu", "hv"):
+                L.set_global(f, fields[f][j0:j0 + rows], 0, j0)
         L.fill_ghost_b()
         return L
 
-    def timed(L, K, warm):
+    def timed(L, K, warm, use_dist=True):
+        d = dist if use_dist else None
         dt0 = driver.probe_dt(L, wl.cfl)
         dt_dev = torch.tensor([dt0], dtype=torch.float64, device=dev)
         series = None
@@ -205,8 +252,9 @@ def main():
             pts = np.stack([wl.xlo + rng.uniform(0.0, 1.0, args.gauges) * n * wl.dx * (1 - 1e-12),
                             wl.ylo + rng.uniform(0.0, 1.0, args.gauges) * n * wl.dy * (1 - 1e-12)], axis=1)
             L.gauges_bind([driver.GaugeRecorder.patch_of(L, x, y) for x, y in pts], pts)
-            series = torch.empty((max(K, warm), args.gauges, 4), dtype=torch.float64, device=dev)
+            series = torch.empty((max(K, warm, 1), args.gauges, 4), dtype=torch.float64, device=dev)
             torch.cuda.synchronize()
+
         def one_step(k):
             L.fill_ghost(None, 1.0)
             if series is not None:
@@ -215,7 +263,7 @@ def main():
         for k in range(warm):
             one_step(k)
         torch.cuda.synchronize()
-        if dist: dist.barrier()
+        if d: d.barrier()
         torch.cuda.synchronize()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         lc0 = ctx.launch_count()
@@ -224,7 +272,7 @@ def main():
             one_step(k)
         e1.record()
         torch.cuda.synchronize()
-        if dist: dist.barrier()
+        if d: d.barrier()
         ms = e0.elapsed_time(e1)
         launches = ctx.launch_count() - lc0
         # same K steps again with the library's per-kernel event brackets (separate pass: brackets perturb a little)
@@ -237,6 +285,7 @@ def main():
         assert st["nan_seen"] == 0 and np.isfinite(dt_dev.item())
         return ms, launches, prof
 
+    cells = n * n
     L = make(args.side)
     sampler = ClockSampler(local)
     time.sleep(0.3)
@@ -245,89 +294,145 @@ def main():
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
     ms = max_over_ranks(ms, dist, dev)
-    cells = n * n
     value = job_rate(cells * args.steps, world, ms * 1e-3)
 
-    # end to end through the C ABI with HOST buffers: every step copies the state host -> device and back (the paper's own
-    # pipeline) around fill + step; pinned host memory
-    Ke = args.e2e_steps
-    host = [torch.empty((n, n), dtype=torch.float64).pin_memory() for _ in range(3)]
-    for k, f in enumerate(("h", "hu", "hv")):
-        host[k].copy_(torch.from_numpy(L.get_global(f)))
-    hnp = [t.numpy() for t in host]
-    dt = driver.probe_dt(L, wl.cfl)
-    torch.cuda.synchronize()
-    if dist: dist.barrier()
-    w0 = time.time()
-    for _ in range(Ke):
-        for k, f in enumerate(("h", "hu", "hv")):
-            L.set_global(f, hnp[k])
-        L.fill_ghost(None, 1.0)
-        st = L.step(dt)
-        dt = wl.cfl / st["s_over_dx_max"]
-        for k, f in enumerate(("h", "hu", "hv")):
-            ctx._chk(binding.lib().gc_level_get_global(L.h, k, 0, hnp[k].ctypes.data, 0, n, 0, 0, n, n), "get")
-    torch.cuda.synchronize()
-    e2e_s = time.time() - w0
-    e2e_s = max_over_ranks(e2e_s, dist, dev)
-    e2e = job_rate(cells * Ke, world, e2e_s)
-
-    tilings = None
-    if args.sweep and rank == 0:
-        tilings = {}
-        L.destroy(); L = None
-        for side in (16, 32, 64, 128, 256):
-            Ls = make(side)
-            m, _, pr = timed(Ls, args.steps, W)
-            tilings[str(side)] = {"updates_per_s": cells * args.steps / (m * 1e-3), "ms_per_step": m / args.steps,
-                                  "kernel_ms_per_step": {k: v[0] / args.steps for k, v in pr.items() if v[1]}}
-            Ls.destroy()
-
-    if rank != 0:
-        return
     hbm_peak, which = peaks()
     fp64_peak = ctx.fp64_peak()
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
+    counts, counts_src = load_counts()
+
+    def slot_fraction(side, rate):
+        """fp64-pipe issue slots per interior cell update (the x-sweep also covers the 4 ghost rows of every patch, S-5) x rate / peak"""
+        if counts is None:
+            return None
+        kx, ky = counts["kernels"]["xsweep"], counts["kernels"]["ysweep"]
+        return (kx["fp64_slots_per_cell"] * (1.0 + 4.0 / side) + ky["fp64_slots_per_cell"]) * rate / slot_peak
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): serial, then copies overlapped with the kernels
+    e2e = None
+    if not args.no_e2e:
+        Ke = max(args.e2e_steps, 2)
+        hin = [torch.from_numpy(fields[f]).clone().pin_memory() for f in ("h", "hu", "hv")]
+        hout = [torch.empty((n, n), dtype=torch.float64).pin_memory() for _ in range(3)]
+        hnp_in, hnp_out = [t.numpy() for t in hin], [t.numpy() for t in hout]
+        dt = driver.probe_dt(L, wl.cfl)
+        torch.cuda.synchronize()
+        if dist: dist.barrier()
+        w0 = time.time()
+        for _ in range(Ke):
+            for k, f in enumerate(("h", "hu", "hv")):
+                L.set_global(f, hnp_in[k])
+            L.fill_ghost(None, 1.0)
+            st = L.step(dt)
+            for k, f in enumerate(("h", "hu", "hv")):
+                ctx._chk(binding.lib().gc_level_get_global(L.h, k, 0, hnp_out[k].ctypes.data, 0, n, 0, 0, n, n), "get")
+        torch.cuda.synchronize()
+        serial_s = max_over_ranks(time.time() - w0, dist, dev)
+        # overlapped: two level pools used alternately, uploads and downloads on their own streams
+        L2 = make(args.side)
+        pools = [L, L2]
+        dts = [torch.tensor([dt], dtype=torch.float64, device=dev) for _ in range(2)]
+        s_up, s_dn = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+
+        def pipelined(K):
+            for s in range(K):
+                P = pools[s % 2]
+                P.upload_state_async(hin, s_up)
+                P.fill_ghost(None, 1.0)
+                P.step_auto(dts[s % 2], wl.cfl)
+                P.download_state_async(hout, s_dn)
+            s_dn.synchronize(); torch.cuda.synchronize()
+        pipelined(2)                                   # first use allocates the staging planes
+        if dist: dist.barrier()
+        w0 = time.time()
+        pipelined(Ke)
+        over_s = max_over_ranks(time.time() - w0, dist, dev)
+        assert np.isfinite(hnp_out[0]).all() and abs(float(hnp_out[0].mean()) - float(fields["h"].mean())) < 1.0
+        L2.destroy()
+        nbytes = 3 * cells * 8
+        e2e = {"value": job_rate(cells * Ke, world, over_s), "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+               "steps": Ke, "serial": job_rate(cells * Ke, world, serial_s),
+               "h2d_gbs": nbytes * Ke / over_s / 1e9,
+               "note": "every step uploads h, hu, hv from pinned host memory and reads the new state back, through the C ABI. value: "
+                       "gc_level_upload_state_async / gc_level_download_state_async on their own streams, two level pools used "
+                       "alternately, so one step's copies overlap the neighbouring steps' kernels (P:174-186); serial: "
+                       "gc_level_set_global, fill + step, gc_level_get_global in sequence (P:166)"}
+        del hin, hout
+
+    # ---- the five tilings of BASELINE.json configs[4] (N = 1 only: no barrier inside, nothing for other ranks to wait on)
+    tilings = None
+    if not args.no_tilings and world == 1:
+        tilings = {}
+        for side in (16, 32, 64, 128, 256):
+            if side == args.side:
+                m, pr = ms, prof
+            else:
+                if L is not None:
+                    L.destroy(); L = None
+                Ls = make(side)
+                m, _, pr = timed(Ls, args.steps, W, use_dist=False)
+                Ls.destroy()
+            rate = cells * args.steps / (m * 1e-3)
+            tilings[str(side)] = {"updates_per_s": rate, "ms_per_step": m / args.steps,
+                                  "hbm_gbs_at_56B": BYTES_PER_UPDATE * rate / 1e9, "hbm_frac": BYTES_PER_UPDATE * rate / 1e9 / hbm_peak,
+                                  "fp64_pipe_slot_frac": slot_fraction(side, rate),
+                                  "kernel_ms_per_step": {k: v[0] / args.steps for k, v in pr.items() if v[1]}}
+
+    if rank != 0:
+        if dist: dist.destroy_process_group()
+        return
     # dominant kernel = the largest slot of the per-kernel brackets
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms = prof[dom][0] / max(prof[dom][1], 1)
     share = {k: v[0] / max(sum(x[0] for x in prof.values()), 1e-12) for k, v in prof.items() if v[1]}
     # cells one launch of the dominant kernel updates: the x-sweep also covers the 4 ghost rows of every patch (S-5)
     per_launch = {"xsweep": cells * (1.0 + 4.0 / args.side), "ysweep": float(cells)}.get(dom, float(cells))
-    flop_sweep = FLOP_PER_SWEEP.get(dom, 411.0)
-    alu_achieved = flop_sweep * per_launch / (dom_ms * 1e-3) / 1e12
-    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
-    slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
-    slot_frac = FP64_SLOTS_PER_SWEEP.get(dom, 394.0) * per_launch / (dom_ms * 1e-3) / slot_peak
-    default_kernels = True
+    kc = counts["kernels"].get(dom) if counts else None
+    if kc:
+        achieved = kc["flop_per_cell"] * per_launch / (dom_ms * 1e-3) / 1e12
+        traffic = kc["dram_bytes_per_launch"] if (n, args.side) == (counts.get("n"), counts.get("side")) else None
+        roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+                    "frac": achieved / (fp64_peak / 1e12), "traffic": traffic,
+                    "peak_source": "DFMA micro-benchmark in this run (gc_probe_fp64_peak = 2 flop x 64 lanes x SMs x clock)",
+                    "flop_per_cell": kc["flop_per_cell"], "fp64_slots_per_cell": kc["fp64_slots_per_cell"],
+                    "thread_inst_per_cell": kc["thread_inst_per_cell"], "cells_per_launch": per_launch, "kernel_ms": dom_ms,
+                    "fp64_pipe_slot_frac": kc["fp64_slots_per_cell"] * per_launch / (dom_ms * 1e-3) / slot_peak,
+                    "counts_source": counts_src, "kernel_share_of_step": share}
+    else:
+        gbs = BYTES_PER_UPDATE * per_launch / (dom_ms * 1e-3) / 1e9       # one sweep reads 4 planes and writes 3: 56 B per cell
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                    "traffic": None, "peak_source": "MEASURED_PEAKS.json" if which == "measured" else "fallback 6650 GB/s",
+                    "cells_per_launch": per_launch, "kernel_ms": dom_ms, "counts_source": counts_src,
+                    "note": "the kernel is bound by the fp64 pipe (DESIGN.md 6); its instruction counts are withheld because the "
+                            "committed capture does not match the sources, so only the algorithmic-bytes figure is given",
+                    "kernel_share_of_step": share}
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "cfg5: spherical single level %dx%d at 0.5 arcmin, %dx%d patches of side %d, ghost fill + level step"
                                % (n, n, n // args.side, n // args.side, args.side),
-                   "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (L.ncells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9 if L else 0),
-                   "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl, "fmad": False,
-                   "manning_n": args.manning, "gauges": args.gauges},
-        "clocks": clocks,
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 3 * cells * 8, "d2h_bytes_per_step": 3 * cells * 8 + 40,
-                "steps": Ke, "note": "state copied host->device and back every step through the C ABI (P:166 pipeline)"},
-        "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                     "frac": alu_achieved / (fp64_peak / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(dom) if default_kernels else None,
-                     "peak_source": "DFMA micro-benchmark in this run (gc_probe_fp64_peak = 2 flop x 64 lanes x SMs x clock); "
-                                    "the scheme is compiled without FMA contraction, so add/mul code tops out at 0.5",
-                     "flop_per_cell_per_sweep": flop_sweep, "cells_per_launch": per_launch, "kernel_ms": dom_ms,
-                     "fp64_pipe_slot_frac": slot_frac, "kernel_share_of_step": share},
-        "hbm": {"achieved_gbs": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9, "peak_gbs": hbm_peak,
-                "frac": BYTES_PER_UPDATE * (cells * args.steps / (ms * 1e-3)) / 1e9 / hbm_peak, "of": which,
-                "bytes_per_update": BYTES_PER_UPDATE},
+                   "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (cells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9),
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl,
+                   "fma": "explicit, where DESIGN.md 3 writes it (both sides)", "manning_n": args.manning, "gauges": args.gauges},
+        "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
+        "hbm": {"achieved_gbs": BYTES_PER_UPDATE * value / world / 1e9, "peak_gbs": hbm_peak,
+                "frac": BYTES_PER_UPDATE * value / world / 1e9 / hbm_peak, "of": which, "bytes_per_update": BYTES_PER_UPDATE},
     }
+    if e2e:
+        out["e2e"] = e2e
     if tilings:
         out["config"]["tilings"] = tilings
-    if not args.no_cpu:
-        rate, el = oracle_rate(1024, 60)
-        out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                               "sample": "config-5 recipe at 1024x1024 (one patch), 60 steps, %.1f s" % el}
+    if not args.no_cpu and world == 1:
+        if L is not None:
+            L.destroy()
+        rate, el, k, nt = oracle_leg(wl, n, args.side, fields, None, 0, 0, budget_s=12.0)
+        rate1, el1, k1, _ = oracle_leg(wl, n, args.side, fields, 1, 0, 1)
+        out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": nt, "kind": "oracle",
+                               "sample": "the bench workload itself (%dx%d in patches of side %d): %d steps in %.1f s, loop over patches on "
+                                         "%d threads" % (n, n, args.side, k, el, nt),
+                               "one_core": {"value": rate1, "steps": k1, "seconds": el1}}
     print(json.dumps(out))
     if dist:
         dist.destroy_process_group()

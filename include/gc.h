@@ -128,6 +128,18 @@ int gc_level_set_global(gc_level *, int field, const double *src, int is_device,
 int gc_level_get_global(const gc_level *, int field, int which, double *dst, int is_device, int64_t ld,
                         int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
 
+/* Asynchronous whole-level state transfer for pipelines ("overlapping memory copies with kernel execution").
+ * host[0..2]: PINNED HOST arrays of h, hu, hv over the whole level, ny_level rows of nx_level doubles (a pageable array makes
+ * the copies synchronous but stays correct).  copy_stream: a cudaStream_t (as void*) other than the context's stream.
+ * upload: enqueues the three host->device copies on copy_stream into staging planes the library owns, then -- on the context's
+ * stream, after an event -- the scatter into the pool ("new" buffer, every storage cell inside the level incl. ghost cells).
+ * download: the gather of the interior cells of the "new" buffer on the context's stream (cells no patch covers read 0), then the
+ * three device->host copies on copy_stream.  Both return without synchronising; consecutive calls on a level are ordered by
+ * events, so a caller only has to synchronise copy_stream before it reads a downloaded array or reuses an uploaded one.
+ * First use allocates 3 staging planes of nx_level * ny_level doubles per direction (released with the level). */
+int gc_level_upload_state_async(gc_level *L, const double *const host[3] /*HOST, pinned*/, void *copy_stream);
+int gc_level_download_state_async(gc_level *L, double *const host[3] /*HOST, pinned*/, void *copy_stream);
+
 /* A2-A4 (P:143 step 2): fill the ghost cells of the current state.  Order: same-level
  * copy incl. corners; remaining in-domain ghosts from `coarser` interpolated in space (limited linear in
  * eta, u, v) and time (alpha = (t - t_coarse_old) / dt_coarse, linear between coarser's OLD and NEW buffers,
@@ -167,25 +179,6 @@ int gc_level_init_from(gc_level *newfine, const gc_level *oldfine, const gc_leve
  * Q_C += side * delta / area to the uncovered coarse neighbours, then the clean-up rule, and re-zeroes. */
 int gc_flux_attach(gc_level *coarse, gc_level *fine);
 int gc_flux_fixup(gc_level *coarse, gc_level *fine);
-
-/* Kernel accounting.  gc_launch_count: kernels launched by this context so far.  gc_profile_enable(on): bracket
- * every kernel group with CUDA events on the context's stream; gc_profile_read synchronises, returns per slot the
- * summed milliseconds and the number of bracketed groups since the last read (arrays of GC_PROFILE_SLOTS), and clears.
- * Slots: 0 same-level copy, 1 physical BC, 2 x-sweep, 3 y-sweep, 4 coarse fill, 5 average-down / regrid transfer,
- * 6 flags, 7 flux registers, 8 misc (stats, dt), 9 fused sweep. */
-#define GC_PROFILE_SLOTS 10
-int64_t gc_launch_count(const gc_ctx *);
-int gc_profile_enable(gc_ctx *, int on);
-int gc_profile_read(gc_ctx *, double *ms /*HOST*/, int64_t *count /*HOST*/);
-
-/* Self-test of the branch-free correctly rounded divide / reciprocal / square root the marching kernels use
- * (csrc/gc_math.cuh) against the IEEE operators: for each i, a[i]/b[i], 1/b[i], sqrt(a[i]) (a, b: HOST arrays of n).
- * nmismatch = results that differ in any bit although the fast path accepted the operands (must be 0);
- * nfallback = operations whose operands were outside the fast window (they are redone with the operators). */
-int gc_selftest_math(gc_ctx *, const double *a, const double *b, int64_t n, int64_t *nmismatch, int64_t *nfallback);
-
-/* Measured fp64 ALU throughput of this device (DFMA micro-benchmark, flop/s); for the "alu" roofline. */
-int gc_probe_fp64_peak(gc_ctx *, double *flops_out /*HOST*/);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,7 @@ SYMBOLS = [
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
-    "gc_ctx_set_option",
+    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async",
 ]
 
 
@@ -57,6 +57,8 @@ def lib():
     L.gc_ctx_create.argtypes = [vp, vp, ALLOC_FN, FREE_FN, vp, vp]
     L.gc_ctx_destroy.argtypes = [vp]
     L.gc_ctx_set_option.argtypes = [vp, i, i64]
+    L.gc_level_upload_state_async.argtypes = [vp, vp, vp]
+    L.gc_level_download_state_async.argtypes = [vp, vp, vp]
     L.gc_last_error.argtypes = [vp]; L.gc_last_error.restype = C.c_char_p
     L.gc_level_create.argtypes = [vp, i, d, d, d, d, i64, i64, i, i, vp, vp]
     L.gc_level_destroy.argtypes = [vp]
@@ -171,6 +173,15 @@ class Level:
     def step_auto(self, dt_dev, cfl):
         """dt_dev: 1-element float64 CUDA tensor holding dt; updated in place to the next dt."""
         self.ctx._chk(lib().gc_level_step_auto(self.h, dt_dev.data_ptr(), cfl), "gc_level_step_auto")
+
+    def upload_state_async(self, host3, copy_stream):
+        """host3: three pinned CPU tensors (h, hu, hv) of shape (nyl, nxl), float64; copy_stream: a torch.cuda.Stream"""
+        ptrs = (C.c_void_p * 3)(*[t.data_ptr() for t in host3])
+        self.ctx._chk(lib().gc_level_upload_state_async(self.h, ptrs, C.c_void_p(copy_stream.cuda_stream)), "gc_level_upload_state_async")
+
+    def download_state_async(self, host3, copy_stream):
+        ptrs = (C.c_void_p * 3)(*[t.data_ptr() for t in host3])
+        self.ctx._chk(lib().gc_level_download_state_async(self.h, ptrs, C.c_void_p(copy_stream.cuda_stream)), "gc_level_download_state_async")
 
     def stats(self):
         st = StepStats()

@@ -293,6 +293,8 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
 
     // same-level copy rectangles: grown box of p  x  interior of q (A2, incl. corners)
     std::vector<CopyRect> rects;
+    std::vector<int2> rrange((size_t)std::max(np, 1));
+    int64_t ghost_cells = 0;
     std::vector<int32_t> bcp;
     std::vector<uint8_t> mask;
     for (int p = 0; p < np; p++) {
@@ -324,11 +326,13 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
                 for (size_t k = first; k < rects.size(); k++) if (rects[k].dst == r.dst) { dup = true; break; }
                 if (dup) continue;
                 rects.push_back(r);
+                ghost_cells += (int64_t)r.w * r.h;
                 if (need_mask)
                     for (int64_t y = y0; y < y1; y++) for (int64_t x = x0; x < x1; x++)
                         mask[(size_t)(y - P.j0 + 2) * D.pitch + (x - P.i0 + 2)] = 1;
             }
         }
+        rrange[(size_t)p] = make_int2((int)first, (int)(rects.size() - first));
         if (need_mask) {   // in-domain ghost cells without a same-level source come from the coarser level (A3)
             for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < P.nx + 4; i++) {
                 if (i >= 2 && i < P.nx + 2 && j >= 2 && j < P.ny + 2) continue;
@@ -341,15 +345,20 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
         }
     }
     L->ncopy = (int)rects.size(); L->d_copy = upload(L, rects);
+    L->d_copy_range = upload(L, rrange);
+    {   // warps per patch: about 256 ghost cells per warp, at most 16
+        const int64_t per = np > 0 ? ghost_cells / np : 0;
+        L->copy_wpp = (int)std::min<int64_t>(16, std::max<int64_t>(1, per / 256));
+    }
     L->nbcp = (int)bcp.size(); L->d_bcp = upload(L, bcp);
     L->d_stats = (DevStats *)gc_dev_alloc(ctx, sizeof(DevStats)); L->allocs.push_back(L->d_stats);
-    L->d_partial = (double *)gc_dev_alloc(ctx, sizeof(double) * (np > 0 ? np : 1)); L->allocs.push_back(L->d_partial);
+    L->d_partial = (double *)gc_dev_alloc(ctx, sizeof(double) * (size_t)std::max(gc_mass_partials(L), 1)); L->allocs.push_back(L->d_partial);
     L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->d_cfstart = nullptr; L->ncf = 0; L->ncfcells = 0;
     L->avg_gen = 0; L->d_avg = nullptr; L->d_avgstart = nullptr; L->navg = 0; L->navgcells = 0;
     L->nbr_buffer = -1; L->d_nbrstart = nullptr; L->d_nbrlist = nullptr; L->r_reg = 1;
     L->reg_fine = nullptr; L->reg_coarse = nullptr; L->d_reg = nullptr; L->nreg = 0;
     L->d_delta = nullptr; L->d_base = nullptr; L->d_fixstart = nullptr; L->d_fixreg = nullptr; L->nfix = 0;
-    if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_xl || !L->d_yl || !L->d_copy || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
+    if (!L->d_pat || !L->d_xt || !L->d_yt || !L->d_xl || !L->d_yl || !L->d_copy || !L->d_copy_range || !L->d_bcp || !L->d_stats || !L->d_partial || !L->d_kappa) {
         gc_level_destroy(L);
         return gc_fail(ctx, GC_ERR_NOMEM, "gc_level_create: table allocation failed");
     }
@@ -368,6 +377,7 @@ extern "C" int gc_level_destroy(gc_level *L)
     if (!L) return GC_OK;
     gc_amr_on_destroy(L);
     cudaStreamSynchronize(L->ctx->stream);
+    for (cudaEvent_t e : {L->ev_up_copied, L->ev_up_free, L->ev_dn_ready, L->ev_dn_free}) if (e) { cudaEventSynchronize(e); cudaEventDestroy(e); }
     for (void *p : L->allocs) gc_dev_free(L->ctx, p);
     delete L;
     return GC_OK;
@@ -445,6 +455,64 @@ extern "C" int gc_level_set_patches(gc_level *L, int field, const double *src, i
     gc_launch_set_patches(L, plane_of(L, field, GC_NEW), L->d_goff, dsrc);
     if (tmp) { cudaStreamSynchronize(c->stream); if (transient) gc_dev_free(c, tmp); }   // the caller's array is free on return
     return gc_cuda_check(c, "gc_level_set_patches");
+}
+
+// ---- asynchronous whole-level state transfer (copies overlapped with kernels)
+static int xfer_prepare(gc_level *L, bool up)
+{
+    gc_ctx *c = L->ctx;
+    double **st = up ? L->xfer_up : L->xfer_dn;
+    if (!st[0]) {
+        const size_t bytes = (size_t)L->nxl * (size_t)L->nyl * 8;
+        for (int f = 0; f < 3; f++) {
+            st[f] = (double *)gc_dev_alloc(c, bytes);
+            if (!st[f]) return gc_fail(c, GC_ERR_NOMEM, "state transfer: staging allocation failed");
+            L->allocs.push_back(st[f]);
+        }
+    }
+    cudaEvent_t *ev[2] = { up ? &L->ev_up_copied : &L->ev_dn_ready, up ? &L->ev_up_free : &L->ev_dn_free };
+    for (int k = 0; k < 2; k++)
+        if (!*ev[k] && cudaEventCreateWithFlags(ev[k], cudaEventDisableTiming) != cudaSuccess) return gc_cuda_check(c, "state transfer: event");
+    return GC_OK;
+}
+
+extern "C" int gc_level_upload_state_async(gc_level *L, const double *const host[3], void *copy_stream)
+{
+    if (!L || !host || !host[0] || !host[1] || !host[2]) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_upload_state_async: bad argument");
+    gc_ctx *c = L->ctx;
+    const bool first = L->xfer_up[0] == nullptr;
+    int rc = xfer_prepare(L, true);
+    if (rc) return rc;
+    cudaStream_t cs = (cudaStream_t)copy_stream;
+    const size_t bytes = (size_t)L->nxl * (size_t)L->nyl * 8;
+    if (!first) cudaStreamWaitEvent(cs, L->ev_up_free, 0);          // the previous upload's scatter has read the staging planes
+    for (int f = 0; f < 3; f++) cudaMemcpyAsync(L->xfer_up[f], host[f], bytes, cudaMemcpyHostToDevice, cs);
+    cudaEventRecord(L->ev_up_copied, cs);
+    cudaStreamWaitEvent(c->stream, L->ev_up_copied, 0);
+    for (int f = 0; f < 3; f++) gc_launch_set_global(L, L->q[L->cur][f], L->xfer_up[f], L->nxl, 0, 0, L->nxl, L->nyl);
+    cudaEventRecord(L->ev_up_free, c->stream);
+    return gc_cuda_check(c, "gc_level_upload_state_async");
+}
+
+extern "C" int gc_level_download_state_async(gc_level *L, double *const host[3], void *copy_stream)
+{
+    if (!L || !host || !host[0] || !host[1] || !host[2]) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_download_state_async: bad argument");
+    gc_ctx *c = L->ctx;
+    const bool first = L->xfer_dn[0] == nullptr;
+    int rc = xfer_prepare(L, false);
+    if (rc) return rc;
+    cudaStream_t cs = (cudaStream_t)copy_stream;
+    const size_t bytes = (size_t)L->nxl * (size_t)L->nyl * 8;
+    if (!first) cudaStreamWaitEvent(c->stream, L->ev_dn_free, 0);   // the previous download's copies have left the staging planes
+    for (int f = 0; f < 3; f++) {
+        if (L->ncells != L->nxl * L->nyl) cudaMemsetAsync(L->xfer_dn[f], 0, bytes, c->stream);   // cells no patch covers read as 0
+        gc_launch_get_global(L, L->q[L->cur][f], L->xfer_dn[f], L->nxl, 0, 0, L->nxl, L->nyl);
+    }
+    cudaEventRecord(L->ev_dn_ready, c->stream);
+    cudaStreamWaitEvent(cs, L->ev_dn_ready, 0);
+    for (int f = 0; f < 3; f++) cudaMemcpyAsync(host[f], L->xfer_dn[f], bytes, cudaMemcpyDeviceToHost, cs);
+    cudaEventRecord(L->ev_dn_free, cs);
+    return gc_cuda_check(c, "gc_level_download_state_async");
 }
 
 extern "C" int gc_level_get_global(const gc_level *L, int field, int which, double *dst, int is_device, int64_t ld,
@@ -561,12 +629,13 @@ extern "C" double gc_level_mass(const gc_level *L)
 {
     if (!L) return NAN;
     gc_launch_mass(L);
-    std::vector<double> part(L->np > 0 ? L->np : 1, 0.0);
-    cudaMemcpyAsync(part.data(), L->d_partial, sizeof(double) * L->np, cudaMemcpyDeviceToHost, L->ctx->stream);
+    const int npart = L->np > 0 ? gc_mass_partials(L) : 0;
+    std::vector<double> part((size_t)std::max(npart, 1), 0.0);
+    cudaMemcpyAsync(part.data(), L->d_partial, sizeof(double) * npart, cudaMemcpyDeviceToHost, L->ctx->stream);
     cudaStreamSynchronize(L->ctx->stream);
     if (gc_cuda_check(L->ctx, "gc_level_mass")) return NAN;
     double m = 0.0;
-    for (int p = 0; p < L->np; p++) m += part[p];
+    for (int p = 0; p < npart; p++) m += part[p];
     return m;
 }
 

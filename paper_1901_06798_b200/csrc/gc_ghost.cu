@@ -3,31 +3,66 @@
 // The paper keeps ghost filling on the CPU because a per-patch kernel has only O(a) parallelism;
 // here ONE launch covers every patch of the level through host-built work lists, so the parallelism is
 // O(total perimeter).
+#include <algorithm>
 #include "gc_internal.h"
 
-// ---- A2: one warp per rectangle (w x h cells), up to three planes
-__global__ void k_copy_rects(const CopyRect *rects, int n, double *f0, double *f1, double *f2, int nf)
+// ---- A2: same-level copy.  The host lists, per patch, the rectangles its ghost cells take from the interiors of its
+// neighbours (two x faces of width 2, two y faces of height 2, four 2 x 2 corners on a regular tiling).  A patch is served by
+// `wpp` warps (one for small patches, several when the perimeter is long) that walk its rectangles together: a wide rectangle
+// row by row with the lanes along x (coalesced), a narrow one several rows per pass (lane -> (row, column): one division per
+// rectangle, none per cell).  Two rows are in flight per lane and plane before anything is stored.  Pure data movement:
+// every ghost cell written once, 48 bytes of algorithmic traffic per cell (3 planes read + written).
+template <int NF>
+__device__ __forceinline__ void copy_pair(double *f0, double *f1, double *f2, int64_t d0, int64_t s0, int64_t d1, int64_t s1, bool two)
 {
-    int warp = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5);
-    int lane = threadIdx.x & 31;
-    if (warp >= n) return;
-    CopyRect r = rects[warp];
-    int cells = r.w * r.h;
-    for (int c = lane; c < cells; c += 32) {
-        int y = c / r.w, x = c - y * r.w;
-        int64_t d = r.dst + (int64_t)y * r.dpitch + x, s = r.src + (int64_t)y * r.spitch + x;
-        f0[d] = f0[s];
-        if (nf > 1) { f1[d] = f1[s]; f2[d] = f2[s]; }
+    double a0 = f0[s0], a1 = 0.0, a2 = 0.0, b0 = 0.0, b1 = 0.0, b2 = 0.0;
+    if (NF > 1) { a1 = f1[s0]; a2 = f2[s0]; }
+    if (two) { b0 = f0[s1]; if (NF > 1) { b1 = f1[s1]; b2 = f2[s1]; } }
+    f0[d0] = a0; if (NF > 1) { f1[d0] = a1; f2[d0] = a2; }
+    if (two) { f0[d1] = b0; if (NF > 1) { f1[d1] = b1; f2[d1] = b2; } }
+}
+
+template <int NF>
+__global__ void __launch_bounds__(256, 5) k_copy_rects(const CopyRect *rects, const int2 *range, int np, int wpp, double *f0, double *f1, double *f2)
+{
+    const int gw = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5);
+    const int lane = threadIdx.x & 31;
+    const int patch = gw / wpp, sub = gw - patch * wpp;
+    if (patch >= np) return;
+    const int2 pr = range[patch];
+    for (int i = 0; i < pr.y; i++) {
+        const CopyRect r = rects[pr.x + i];
+        if (r.w >= 32) {
+            for (int y = 2 * sub; y < r.h; y += 2 * wpp) {
+                const bool two = y + 1 < r.h;
+                for (int x = lane; x < r.w; x += 32)
+                    copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
+                                  r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, two);
+            }
+        } else {
+            int rpp, ly, lx;                                           // rows per pass; this lane's row and column in a pass
+            if (r.w == 2) { rpp = 16; ly = lane >> 1; lx = lane & 1; }                 // x faces, corners: no division
+            else if (r.w == 16) { rpp = 2; ly = lane >> 4; lx = lane & 15; }
+            else { rpp = 32 / r.w; ly = lane / r.w; lx = lane - ly * r.w; }
+            if (ly < rpp) {
+                for (int y = 2 * sub * rpp + ly; y < r.h; y += 2 * wpp * rpp) {
+                    const bool two = y + rpp < r.h;
+                    copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + lx, r.src + (int64_t)y * r.spitch + lx,
+                                  r.dst + (int64_t)(y + rpp) * r.dpitch + lx, r.src + (int64_t)(y + rpp) * r.spitch + lx, two);
+                }
+            }
+        }
     }
 }
 
 void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf)
 {
     if (L->ncopy == 0) return;
-    int threads = 256;
-    int64_t blocks = ((int64_t)L->ncopy * 32 + threads - 1) / threads;
+    const int threads = 256, wpp = L->copy_wpp;
+    const int64_t blocks = ((int64_t)L->np * wpp * 32 + threads - 1) / threads;
     ProfScope ps(L->ctx, GC_SLOT_COPY);
-    k_copy_rects<<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->ncopy, f0, f1, f2, nf);
+    if (nf > 1) k_copy_rects<3><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->d_copy_range, L->np, wpp, f0, f1, f2);
+    else k_copy_rects<1><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->d_copy_range, L->np, wpp, f0, f1, f2);
 }
 
 // ---- A4: physical boundary.  pass 0: x faces over rows inside the domain; pass 1: y faces over all columns.
@@ -89,14 +124,23 @@ void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int i
                                                   bc[0], bc[1], bc[2], bc[3]);
 }
 
-// ---- field transfer
+// ---- field transfer.  Grids are patches x chunks of GC_CHUNK cells, so that a level that is one large patch spreads over the
+// chip (a block per patch ran config 4's 1800 x 900 coarse level on one SM)
+#define GC_CHUNK 8192
+static dim3 gc_chunk_grid(const gc_level *L, int grow)
+{
+    int64_t mx = 1;
+    for (const gc_patch &P : L->pat) mx = std::max<int64_t>(mx, (int64_t)(P.nx + grow) * (P.ny + grow));
+    return dim3((unsigned)L->np, (unsigned)((mx + GC_CHUNK - 1) / GC_CHUNK));
+}
 __global__ void k_set_global(const PatchDesc *pat, double *plane, const double *src, int64_t ld,
                              int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
     PatchDesc pd = pat[blockIdx.x];
     const int W = pd.nx + 4;
     int n = W * (pd.ny + 4);
-    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += blockDim.x) {
         int j = t / W, i = t - j * W;
         int64_t gi = (int64_t)pd.i0 + i - 2 - gi0, gj = (int64_t)pd.j0 + j - 2 - gj0;
         if (gi < 0 || gi >= gnx || gj < 0 || gj >= gny) continue;
@@ -112,7 +156,8 @@ __global__ void k_set_patches(const PatchDesc *pat, const int64_t *goff, double 
     const double *sp = src + goff[blockIdx.x];
     const int W = pd.nx + 4;
     const int n = W * (pd.ny + 4);
-    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += blockDim.x) {
         const int j = t / W, i = t - j * W;
         const int64_t gi = (int64_t)pd.i0 + i - 2, gj = (int64_t)pd.j0 + j - 2;
         if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
@@ -122,7 +167,7 @@ __global__ void k_set_patches(const PatchDesc *pat, const int64_t *goff, double 
 void gc_launch_set_patches(gc_level *L, double *plane, const int64_t *goff, const double *src)
 {
     ProfScope ps(L->ctx, GC_SLOT_MISC);
-    if (L->np) k_set_patches<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, goff, plane, src, L->nxl, L->nyl);
+    if (L->np) k_set_patches<<<gc_chunk_grid(L, 4), 256, 0, L->ctx->stream>>>(L->d_pat, goff, plane, src, L->nxl, L->nyl);
 }
 
 __global__ void k_get_global(const PatchDesc *pat, const double *plane, double *dst, int64_t ld,
@@ -130,7 +175,8 @@ __global__ void k_get_global(const PatchDesc *pat, const double *plane, double *
 {
     PatchDesc pd = pat[blockIdx.x];
     int n = pd.nx * pd.ny;
-    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += blockDim.x) {
         int j = t / pd.nx, i = t - j * pd.nx;
         int64_t gi = (int64_t)pd.i0 + i - gi0, gj = (int64_t)pd.j0 + j - gj0;
         if (gi < 0 || gi >= gnx || gj < 0 || gj >= gny) continue;
@@ -141,12 +187,12 @@ __global__ void k_get_global(const PatchDesc *pat, const double *plane, double *
 void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
     ProfScope ps(L->ctx, GC_SLOT_MISC);
-    if (L->np) k_set_global<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, plane, src, ld, gi0, gj0, gnx, gny);
+    if (L->np) k_set_global<<<gc_chunk_grid(L, 4), 256, 0, L->ctx->stream>>>(L->d_pat, plane, src, ld, gi0, gj0, gnx, gny);
 }
 void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny)
 {
     ProfScope ps(L->ctx, GC_SLOT_MISC);
-    if (L->np) k_get_global<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, plane, dst, ld, gi0, gj0, gnx, gny);
+    if (L->np) k_get_global<<<gc_chunk_grid(L, 0), 256, 0, L->ctx->stream>>>(L->d_pat, plane, dst, ld, gi0, gj0, gnx, gny);
 }
 
 __global__ void k_copy2d(double *dst, int64_t dld, const double *src, int64_t sld, int w, int h)
@@ -169,7 +215,8 @@ __global__ void k_wet_mask(const PatchDesc *pat, const double *h, double eps, ui
 {
     PatchDesc pd = pat[blockIdx.x];
     int n = pd.nx * pd.ny;
-    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += blockDim.x) {
         int j = t / pd.nx, i = t - j * pd.nx;
         mask[pd.ioff + t] = h[pd.off + (int64_t)(j + 2) * pd.pitch + i + 2] > eps ? 1 : 0;
     }
@@ -177,18 +224,20 @@ __global__ void k_wet_mask(const PatchDesc *pat, const double *h, double eps, ui
 void gc_launch_wet_mask(const gc_level *L, uint8_t *mask)
 {
     ProfScope ps(L->ctx, GC_SLOT_MISC);
-    if (L->np) k_wet_mask<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->ctx->P.dry_tol, mask);
+    if (L->np) k_wet_mask<<<gc_chunk_grid(L, 0), 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->ctx->P.dry_tol, mask);
 }
 
-// ---- mass: per patch, fixed-order reduction (thread-strided partial sums, then a fixed tree); the host adds
-// the per-patch partials in patch order.  Deterministic for a given patch list.
+// ---- mass: grid = patches x chunks of GC_CHUNK cells; each block reduces its chunk in a fixed order (thread-strided partial
+// sums, then a fixed tree) into partial[patch * nchunk + chunk]; the host adds the partials in index order.  Deterministic for
+// a given patch list.
 __global__ void k_mass(const PatchDesc *pat, const double *h, const double *kappa, double dxdy, double *partial)
 {
     __shared__ double sm[256];
     PatchDesc pd = pat[blockIdx.x];
     int n = pd.nx * pd.ny;
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
     double acc = 0.0;
-    for (int t = threadIdx.x; t < n; t += 256) {
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += 256) {
         int j = t / pd.nx, i = t - j * pd.nx;
         acc += h[pd.off + (int64_t)(j + 2) * pd.pitch + i + 2] * (kappa[pd.j0 + j + 2] * dxdy);
     }
@@ -198,10 +247,11 @@ __global__ void k_mass(const PatchDesc *pat, const double *h, const double *kapp
         if (threadIdx.x < o) sm[threadIdx.x] += sm[threadIdx.x + o];
         __syncthreads();
     }
-    if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
+    if (threadIdx.x == 0) partial[(size_t)blockIdx.x * gridDim.y + blockIdx.y] = sm[0];
 }
+int gc_mass_partials(const gc_level *L) { const dim3 g = gc_chunk_grid(L, 0); return (int)(g.x * g.y); }
 void gc_launch_mass(const gc_level *L)
 {
     ProfScope ps(L->ctx, GC_SLOT_MISC);
-    if (L->np) k_mass<<<L->np, 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->d_kappa, L->dx * L->dy, L->d_partial);
+    if (L->np) k_mass<<<gc_chunk_grid(L, 0), 256, 0, L->ctx->stream>>>(L->d_pat, L->q[L->cur][0], L->d_kappa, L->dx * L->dy, L->d_partial);
 }

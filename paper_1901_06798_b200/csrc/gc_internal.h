@@ -6,6 +6,7 @@
 #include <unordered_map>
 #include <vector>
 #include "../../include/gc.h"
+#include "../../include/gc_test.h"
 
 #define GC_G 2  // ghost width
 #define GC_MARCH_MIN_CELLS 2000000   // levels at least this large use the line-marching sweep kernels
@@ -125,7 +126,8 @@ struct gc_level {
     SweepTile *d_xt, *d_yt; int nxt, nyt;            // edge-parallel tiles (small levels)
     LineDesc *d_xl, *d_yl; int64_t nxl_lines, nyl_lines;   // marching lines (large levels)
     int use_march;
-    CopyRect *d_copy; int ncopy;
+    CopyRect *d_copy; int ncopy;                     // same-level copy rectangles, grouped by destination patch
+    int2 *d_copy_range; int copy_wpp;               // per patch: (first rectangle, count); warps serving one patch
     int32_t *d_bcp; int nbcp;                       // patches touching the physical boundary
     std::vector<int64_t> coarse_ghost;              // plane offsets + global indices of ghosts to be filled from the coarser level
     std::vector<int32_t> coarse_ghost_ij;           // (gi, gj) pairs
@@ -133,7 +135,7 @@ struct gc_level {
     const gc_level *cf_for; uint64_t cf_gen; CoarseFillRect *d_cf; int64_t *d_cfstart; int ncf; int64_t ncfcells;
     uint64_t gen;                                   // unique id of this level object
     DevStats *d_stats;
-    double *d_partial;                              // np doubles (mass partials)
+    double *d_partial;                              // mass partials (gc_mass_partials of them)
     std::vector<void *> allocs;
     // flux registers (this level as the coarse side) + capture slots
     const gc_level *reg_fine; gc_level *reg_coarse;   // cleared by gc_level_destroy of either side
@@ -146,6 +148,10 @@ struct gc_level {
     int nbr_buffer; int32_t *d_nbrstart, *d_nbrlist;
     int64_t *d_goff = nullptr; int64_t gtot = 0;      // packed offsets of gc_level_set_patches (built at first use)
     GaugeLoc *d_gauge = nullptr; int ngauge = 0;     // gauges bound to this level (gc_gauges_bind)
+    // asynchronous whole-level state transfer (gc_level_upload_state_async / gc_level_download_state_async): staging planes of
+    // nxl * nyl doubles per field and direction, events that order the copy stream against the context's stream
+    double *xfer_up[3] = {nullptr, nullptr, nullptr}, *xfer_dn[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_up_copied = nullptr, ev_up_free = nullptr, ev_dn_ready = nullptr, ev_dn_free = nullptr;
 };
 
 void gc_launch_gauges(const gc_level *L, double *out);
@@ -176,6 +182,7 @@ void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, i
 void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *src, int64_t sld, int w, int h);
 void gc_launch_wet_mask(const gc_level *L, uint8_t *mask);
 void gc_launch_mass(const gc_level *L);
+int gc_mass_partials(const gc_level *L);    // number of partial sums gc_launch_mass writes to d_partial
 // gc_amr.cu
 void gc_launch_coarse_fill(gc_level *L, const gc_level *C, const CoarseFillRect *rects, const int64_t *start, int n, int64_t ncells,
                            double alpha, int use_old, int slot);

@@ -517,6 +517,12 @@ __global__ void k_math_selftest(const double *a, const double *b, int64_t n, uns
     { MathFast mf; double q = mf.sqrt_(x);
       if (mf.failed()) atomicAdd(out + 1, 1ull);
       else if (__double_as_longlong(q) != __double_as_longlong(mi.sqrt_(x))) atomicAdd(out, 1ull); }
+    // the unchecked sequences of the guarded open-ocean path, on operands inside their window
+    if (gc_in_window(x) && gc_in_window(y)) {
+        if (__double_as_longlong(gc_fdiv(x, y)) != __double_as_longlong(x / y)) atomicAdd(out, 1ull);
+        if (__double_as_longlong(gc_frcp(y)) != __double_as_longlong(1.0 / y)) atomicAdd(out, 1ull);
+        if (x > 0.0 && __double_as_longlong(gc_fsqrt(x)) != __double_as_longlong(sqrt(x))) atomicAdd(out, 1ull);
+    }
 }
 void gc_launch_math_selftest(cudaStream_t s, const double *a, const double *b, int64_t n, unsigned long long *out)
 {

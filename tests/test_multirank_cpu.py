@@ -87,7 +87,7 @@ def test_single_process_needs_no_group():
 def test_reference_arm_runs_on_rank_0_only():
     """bench.py --impl reference under torchrun's environment with 2 ranks: rank 0 times the oracle and prints the one JSON
     line (n_gpus as given); rank 1 exits 0 with no output and without building or touching the oracle's work"""
-    res = launch(2, ["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0"])
+    res = launch(2, ["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--n", "1024"])   # a small level: CPU suite
     for rc, out, err in res:
         assert rc == 0, err[-2000:]
     assert res[1][1].strip() == ""
@@ -95,6 +95,6 @@ def test_reference_arm_runs_on_rank_0_only():
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["steps"] == 1 and d["value"] > 0
-    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1 and d["cpu_baseline"]["value"] == d["value"]
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == (os.cpu_count() or 1) and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["gpu_launches"] == 0 and d["vs_baseline"] is None
