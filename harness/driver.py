@@ -49,6 +49,13 @@ def set_initial(L, wl, state=True):
                     L.set_patches("b", arr)
                     L.fill_ghost_b()
                     return
+        if not state:
+            packed_b = pack_bathy_native(L, wl)
+            L.set_patches("b", packed_b)
+            cache.insert(0, (key, packed_b))
+            del cache[6:]
+            L.fill_ghost_b()
+            return
         sizes = [(int(p[2]) + 4) * (int(p[3]) + 4) for p in pats]
         packed = {f: np.zeros(int(np.sum(sizes, dtype=np.int64))) for f in names}
         o = 0
@@ -116,23 +123,31 @@ def _signature_cut(sig):
 def cluster(flags, valid=None, efficiency=0.7, max_side=64):
     """flags: 2-D uint8 (ny, nx) of one level.  valid (optional, same shape): cells a box may contain.
     Returns a list of (i0, j0, nx, ny) boxes (cells of that level), disjoint, covering every flagged cell,
-    sorted by (j0, i0)."""
+    sorted by (j0, i0).  Signatures and box counts come from two running sums (along y per column, along x per row) and a
+    summed-area table, so a box costs O(nx + ny) instead of O(nx ny)."""
     out = []
     fl = np.asarray(flags, dtype=bool)
-    stack = [(0, 0, fl.shape[1], fl.shape[0])]
+    NY, NX = fl.shape
+    cy = np.zeros((NY + 1, NX), dtype=np.int64); np.cumsum(fl, axis=0, out=cy[1:])          # cy[j, i] = flags in column i below row j
+    cx = np.zeros((NY, NX + 1), dtype=np.int64); np.cumsum(fl, axis=1, out=cx[:, 1:])       # cx[j, i] = flags in row j left of column i
+    bad = None
+    if valid is not None:                                                                    # summed-area table of the invalid cells
+        bad = np.zeros((NY + 1, NX + 1), dtype=np.int64)
+        np.cumsum(np.cumsum(~np.asarray(valid, dtype=bool), axis=0), axis=1, out=bad[1:, 1:])
+    stack = [(0, 0, NX, NY)]
     while stack:
         i0, j0, nx, ny = stack.pop()
-        sub = fl[j0:j0 + ny, i0:i0 + nx]
-        if not sub.any():
+        sx = cy[j0 + ny, i0:i0 + nx] - cy[j0, i0:i0 + nx]                # flags per column of the box
+        xs = np.nonzero(sx)[0]
+        if len(xs) == 0:
             continue
-        sx = sub.sum(axis=0); sy = sub.sum(axis=1)
-        xs = np.nonzero(sx)[0]; ys = np.nonzero(sy)[0]
-        i0, nx = i0 + int(xs[0]), int(xs[-1] - xs[0] + 1)
+        sy = cx[j0:j0 + ny, i0 + nx] - cx[j0:j0 + ny, i0]                # flags per row of the box
+        ys = np.nonzero(sy)[0]
+        i0, nx = i0 + int(xs[0]), int(xs[-1] - xs[0] + 1)                # shrink to the bounding box of the flags
         j0, ny = j0 + int(ys[0]), int(ys[-1] - ys[0] + 1)
-        sub = fl[j0:j0 + ny, i0:i0 + nx]
-        sx = sub.sum(axis=0).astype(np.int64); sy = sub.sum(axis=1).astype(np.int64)
-        ok_valid = True if valid is None else bool(valid[j0:j0 + ny, i0:i0 + nx].all())
-        eff = sub.sum() / float(nx * ny)
+        sx = sx[int(xs[0]):int(xs[-1]) + 1]; sy = sy[int(ys[0]):int(ys[-1]) + 1]
+        ok_valid = True if bad is None else (bad[j0 + ny, i0 + nx] - bad[j0, i0 + nx] - bad[j0 + ny, i0] + bad[j0, i0]) == 0
+        eff = int(sx.sum()) / float(nx * ny)
         if eff >= efficiency and ok_valid and nx <= max_side and ny <= max_side:
             out.append((i0, j0, nx, ny))
             continue
@@ -140,12 +155,12 @@ def cluster(flags, valid=None, efficiency=0.7, max_side=64):
         if nx > max_side or ny > max_side:             # chop oversize boxes first, in the middle of the long side
             cut = ("x", nx // 2) if nx >= ny else ("y", ny // 2)
         else:
-            cx = _signature_cut(sx); cy = _signature_cut(sy)
-            hx = cx is not None and sx[cx] == 0; hy = cy is not None and sy[cy] == 0
+            cx_ = _signature_cut(sx); cy_ = _signature_cut(sy)
+            hx = cx_ is not None and sx[cx_] == 0; hy = cy_ is not None and sy[cy_] == 0
             if hx or hy:
-                cut = ("x", cx) if (hx and (not hy or nx >= ny)) else ("y", cy)
-            elif cx is not None or cy is not None:
-                cut = ("x", cx) if (cx is not None and (cy is None or nx >= ny)) else ("y", cy)
+                cut = ("x", cx_) if (hx and (not hy or nx >= ny)) else ("y", cy_)
+            elif cx_ is not None or cy_ is not None:
+                cut = ("x", cx_) if (cx_ is not None and (cy_ is None or nx >= ny)) else ("y", cy_)
             elif nx > 1 or ny > 1:
                 cut = ("x", nx // 2) if nx >= ny else ("y", ny // 2)
         if cut is None:                                 # a single cell: accept (flagged cells are valid by construction)
@@ -156,6 +171,86 @@ def cluster(flags, valid=None, efficiency=0.7, max_side=64):
         else:
             stack.append((i0, j0 + cut[1], nx, ny - cut[1])); stack.append((i0, j0, nx, cut[1]))
     out.sort(key=lambda b: (b[1], b[0]))
+    return out
+
+
+_native_lib = None
+
+
+def native():
+    """harness/libamr_host.so (amr_host.c: the same clustering, nesting mask and unpacking in C), built on first use"""
+    global _native_lib
+    if _native_lib is None:
+        import ctypes as C
+        from harness import build as hb
+        lib = C.CDLL(hb.build())
+        vp, i = C.c_void_p, C.c_int
+        lib.amr_unpack.argtypes = [vp, vp, i, i, i, i, i, vp]; lib.amr_unpack.restype = None
+        lib.amr_nesting_mask.argtypes = [vp, i, i, i, i, i, i, i, vp]; lib.amr_nesting_mask.restype = None
+        lib.amr_cluster.argtypes = [vp, vp, i, i, C.c_double, i, vp, i]; lib.amr_cluster.restype = i
+        _native_lib = lib
+    return _native_lib
+
+
+def cluster_native(flags, valid=None, efficiency=0.7, max_side=64):
+    """cluster() in C: identical boxes (tests/test_harness_pins.py)"""
+    fl = np.ascontiguousarray(flags, dtype=np.uint8)
+    va = None if valid is None else np.ascontiguousarray(valid, dtype=np.uint8)
+    cap = 1024
+    while True:
+        out = np.empty((cap, 4), dtype=np.int32)
+        n = native().amr_cluster(fl.ctypes.data, None if va is None else va.ctypes.data, fl.shape[0], fl.shape[1],
+                                 float(efficiency), int(max_side), out.ctypes.data, cap)
+        if n >= 0:
+            return [tuple(b) for b in out[:n].tolist()]
+        cap *= 8
+
+
+def unpack_cells_native(L, packed, bbox):
+    bi, bj, ei, ej = bbox
+    pats = np.ascontiguousarray(L.patches, dtype=np.int32)
+    pk = np.ascontiguousarray(packed, dtype=np.uint8)
+    out = np.empty((ej - bj, ei - bi), dtype=np.uint8)
+    native().amr_unpack(pk.ctypes.data, pats.ctypes.data, len(pats), bi, bj, ei, ej, out.ctypes.data)
+    return out
+
+
+def nesting_mask_native(L, bbox):
+    bi, bj, ei, ej = bbox
+    pats = np.ascontiguousarray(L.patches, dtype=np.int32)
+    ok = np.empty((ej - bj, ei - bi), dtype=np.uint8)
+    native().amr_nesting_mask(pats.ctypes.data, len(pats), bi, bj, ei, ej, int(L.nxl), int(L.nyl), ok.ctypes.data)
+    return ok.view(bool)
+
+
+def pack_bathy_native(L, wl):
+    """every patch's storage-shaped bathymetry block, back to back, copied from the workload's tile cache in one native call
+    (amr_pack_from_tiles); the tiles a patch touches are evaluated first where the cache does not hold them yet.  Same values
+    as wl.bathy_box patch by patch (tests/test_harness_pins.py): a cell's value does not depend on who asks."""
+    import ctypes as C
+    pats = np.ascontiguousarray(L.patches, dtype=np.int32)
+    T = wl.TILE
+    ntx, nty = (int(L.nxl) + T - 1) // T, (int(L.nyl) + T - 1) // T
+    lo_i = np.maximum(pats[:, 0] - 2, 0) // T; hi_i = np.minimum(pats[:, 0] + pats[:, 2] + 1, L.nxl - 1) // T
+    lo_j = np.maximum(pats[:, 1] - 2, 0) // T; hi_j = np.minimum(pats[:, 1] + pats[:, 3] + 1, L.nyl - 1) // T
+    need = set()
+    for a0, a1, c0, c1 in set(zip(lo_i.tolist(), hi_i.tolist(), lo_j.tolist(), hi_j.tolist())):
+        for tj in range(c0, c1 + 1):
+            for ti in range(a0, a1 + 1):
+                need.add((ti, tj))
+    table = np.zeros(ntx * nty, dtype=np.uint64)
+    keep = []
+    for ti, tj in need:
+        t = wl.bathy_tile(L.dx, L.dy, ti, tj)
+        keep.append(t)
+        table[tj * ntx + ti] = t.ctypes.data
+    n = int(((pats[:, 2].astype(np.int64) + 4) * (pats[:, 3] + 4)).sum())
+    out = np.empty(n, dtype=np.float64)
+    lib = native()
+    lib.amr_pack_from_tiles.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    rc = lib.amr_pack_from_tiles(table.ctypes.data, ntx, nty, T, pats.ctypes.data, len(pats), int(L.nxl), int(L.nyl), out.ctypes.data)
+    assert rc == 0, "tile missing"
+    del keep
     return out
 
 
@@ -323,13 +418,17 @@ class Hierarchy:
         if n == 0:
             return None
         bbox = level_bbox(L)
-        fl = unpack_cells(L, packed, bbox=bbox).astype(bool)
-        ok = nesting_mask(L, bbox=bbox)
+        fl = unpack_cells_native(L, packed, bbox).view(bool)          # bytes 0 / 1
+        # everything below happens inside the bounding box of the flags (clustering starts by shrinking to it anyway)
+        rows = np.flatnonzero(fl.any(axis=1)); cols = np.flatnonzero(fl.any(axis=0))
+        bbox = (bbox[0] + int(cols[0]), bbox[1] + int(rows[0]), bbox[0] + int(cols[-1]) + 1, bbox[1] + int(rows[-1]) + 1)
+        fl = np.ascontiguousarray(fl[rows[0]:rows[-1] + 1, cols[0]:cols[-1] + 1])
+        ok = nesting_mask_native(L, bbox)
         fl &= ok
         if not fl.any():
             return None
         r = self.ratios[k]
-        boxes = cluster(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
+        boxes = cluster_native(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
         return np.array([[(b[0] + bbox[0]) * r, (b[1] + bbox[1]) * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
 
     def _regrid(self, k0, initial=False, t=None):

@@ -119,3 +119,43 @@ def test_two_level_run_converges_to_the_uniformly_fine_run(gco):
         H.destroy()
     assert errs[0] > 3 * errs[-1] and errs[-1] < 2e-3, errs           # 1.2 m hump: the finest tolerance is within 2 mm of the fine run
     assert all(a >= b * 0.999 for a, b in zip(errs, errs[1:])), errs   # and the error does not grow as the tolerance shrinks
+
+
+def test_native_bookkeeping_equals_the_python_definition(gco):
+    """harness/amr_host.c (clustering, nesting mask, flag unpacking in C) against the Python functions that define them"""
+    rng = np.random.default_rng(42)
+    for t in range(150):
+        ny, nx = (int(v) for v in rng.integers(1, 90, 2))
+        fl = np.zeros((ny, nx), dtype=bool)
+        for _ in range(int(rng.integers(1, 6))):
+            a, b = sorted(int(v) for v in rng.integers(0, ny, 2)); c, d = sorted(int(v) for v in rng.integers(0, nx, 2))
+            fl[a:b + 1, c:d + 1] = True
+        fl |= rng.random(fl.shape) < rng.choice([0.0, 0.01, 0.1])
+        valid = np.ones_like(fl)
+        if t % 2:
+            valid[:int(rng.integers(0, 4))] = False; valid[:, -int(rng.integers(1, 4)):] = False
+        fl &= valid
+        kw = dict(valid=valid if t % 3 else None, efficiency=0.7, max_side=int(rng.choice([1, 4, 16, 64])))
+        assert driver.cluster(fl, **kw) == driver.cluster_native(fl, **kw), t
+    ctx = gco.Context(**CART)
+    pats = np.array([[4, 2, 10, 6], [14, 2, 6, 12], [4, 8, 10, 6], [0, 20, 30, 4]], dtype=np.int32)
+    L = ctx.level_create(1, 0.0, 0.0, 1.0, 1.0, 30, 24, 1, pats)
+    packed = (rng.random(L.ncells) < 0.3).astype(np.uint8)
+    for bbox in (None, driver.level_bbox(L), (3, 1, 22, 15)):
+        full = (0, 0, L.nxl, L.nyl) if bbox is None else bbox
+        assert np.array_equal(driver.nesting_mask(L, bbox=bbox), driver.nesting_mask_native(L, full))
+    for bbox in (None, driver.level_bbox(L)):
+        full = (0, 0, L.nxl, L.nyl) if bbox is None else bbox
+        assert np.array_equal(driver.unpack_cells(L, packed, bbox=bbox), driver.unpack_cells_native(L, packed, full))
+    # bathymetry blocks packed natively from the tile cache = bathy_box patch by patch
+    wl = workloads.cfg4(120, 60)
+    Lb = ctx.level_create(2, wl.xlo, wl.ylo, wl.dx / 5, wl.dy / 5, 600, 300, 5, np.array([[0, 0, 300, 40], [250, 40, 350, 260], [5, 295, 40, 5]], dtype=np.int32))
+    got = driver.pack_bathy_native(Lb, wl)
+    o = 0
+    for i0, j0, nx, ny in Lb.patches:
+        a0, a1, c0, c1 = max(i0 - 2, 0), min(i0 + nx + 2, 600), max(j0 - 2, 0), min(j0 + ny + 2, 300)
+        want = np.zeros((ny + 4, nx + 4))
+        want[c0 - (j0 - 2):c1 - (j0 - 2), a0 - (i0 - 2):a1 - (i0 - 2)] = wl.bathy_box(Lb.dx, Lb.dy, a0, c0, a1 - a0, c1 - c0)
+        assert np.array_equal(got[o:o + want.size].reshape(want.shape), want)
+        o += want.size
+    assert o == got.size

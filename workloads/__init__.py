@@ -79,6 +79,18 @@ class Workload:
                 out[c0 - j0:c1 - j0, a0 - i0:a1 - i0] = tile[c0 - tj * T:c1 - tj * T, a0 - ti * T:a1 - ti * T]
         return out
 
+    def bathy_tile(self, dx, dy, ti, tj):
+        """the cached T x T tile (ti, tj) of the level with cell size (dx, dy), evaluated on first use"""
+        key = (id(self.bathy), dx, dy, ti, tj)
+        tile = self._tiles.get(key)
+        if tile is None:
+            if sum(t.nbytes for t in self._tiles.values()) > self.TILE_CACHE_BYTES:
+                self._tiles.clear()
+            X, Y = self.centers(dx, dy, ti * self.TILE, tj * self.TILE, self.TILE, self.TILE)
+            tile = np.ascontiguousarray(self.bathy(X, Y), dtype=np.float64)
+            self._tiles[key] = tile
+        return tile
+
     def fields(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
         """b, h, hu, hv at cell centres of the box [i0,i0+nx) x [j0,j0+ny) of a level with the given cell size."""
         X, Y = self.centers(level_dx, level_dy, i0, j0, nx, ny)
