@@ -75,6 +75,29 @@ def set_initial(L, wl, state=True):
     L.fill_ghost_b()
 
 
+def deform_ramp(wl, t):
+    """weight of the seafloor deformation at time t: 0 before t0, 1 from t1 on, linear in between"""
+    d = wl.deform
+    if d is None or t < d["t0"]:
+        return 0.0
+    if t >= d["t1"]:
+        return 1.0
+    return (t - d["t0"]) / (d["t1"] - d["t0"])
+
+
+def deform_to(L, wl, t):
+    """bring the bathymetry of level L to time t: b += (rho(t) - rho already applied) dz, then its ghost cells outside the domain"""
+    if wl.deform is None:
+        return
+    rho = deform_ramp(wl, t)
+    w = rho - getattr(L, "rho_applied", 0.0)
+    if w != 0.0:
+        d = wl.deform
+        L.bathy_update(d["x0"], d["y0"], d["ddx"], d["ddy"], d["dz"], w)
+        L.fill_ghost_b()
+        L.rho_applied = rho
+
+
 def probe_dt(L, cfl, coarser=None, alpha=1.0):
     """dt_0 from a probe step with dt = 0: dt = cfl / max(s / (kappa dx))."""
     L.fill_ghost(coarser, alpha)
@@ -82,12 +105,16 @@ def probe_dt(L, cfl, coarser=None, alpha=1.0):
     return cfl / st["s_over_dx_max"]
 
 
-def run_single_level(L, nsteps, cfl, dt0=None, record=None):
+def run_single_level(L, nsteps, cfl, dt0=None, record=None, wl=None):
     """nsteps level steps with dt_{n+1} = cfl / sigma_n (sigma = max s/(kappa dx) of step n).
-    Returns the list of (dt, stats)."""
+    Returns the list of (dt, stats).  wl with a deformation: the bathymetry is brought to each step's start time first."""
     dt = probe_dt(L, cfl) if dt0 is None else dt0
     hist = []
+    t = 0.0
     for n in range(nsteps):
+        if wl is not None:
+            deform_to(L, wl, t)
+        t += dt
         L.fill_ghost(None, 1.0)
         st = L.step(dt)
         hist.append((dt, st))
@@ -459,6 +486,7 @@ class Hierarchy:
             dx, dy, nxl, nyl = self._geom(k + 1)
             N = self.ctx.level_create(k + 2, self.wl.xlo, self.wl.ylo, dx, dy, nxl, nyl, self.ratios[k], pats)
             set_initial(N, self.wl, state=initial)
+            deform_to(N, self.wl, t)             # the new level's bathymetry at the regrid time, before it is interpolated onto
             if not initial:
                 C.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
                 N.init_from(old, C)
@@ -484,6 +512,7 @@ class Hierarchy:
     def _advance(self, k, dt, alpha, t):
         """one step of level k from its time t (alpha: that time as a fraction of the coarser level's current step)"""
         L = self.levels[k]
+        deform_to(L, self.wl, t)                 # B(x, y, t) at the start of the step (DESIGN.md 3.12)
         L.fill_ghost(self.levels[k - 1] if k > 0 else None, alpha)
         if self.gauges is not None:
             self.gauges.record(k, L, t)

@@ -148,6 +148,22 @@ int gc_level_download_state_async(gc_level *L, double *const host[3] /*HOST, pin
 int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha);
 int gc_fill_ghost_b(gc_level *L);
 
+/* Time-dependent bathymetry B(x, y, t) (the seafloor-deformation source that starts both of the paper's tsunamis, P:273
+ * "deformation information on uniform grids", "ground deformation file", reading S-20).  dz: vertical
+ * seafloor displacement in metres (+ up) on a uniform node grid, node (m, n) at (x0 + m ddx, y0 + n ddy) in the level's
+ * coordinates, my rows of mx values (HOST, or DEVICE if dz_is_device); bilinear between nodes, zero outside the grid.
+ * gc_bathy_update: b <- fma(w, dz(cell centre), b) on every storage cell of L whose centre lies inside the domain (ghost cells
+ * included; follow with gc_fill_ghost_b for the cells outside).  h, hu, hv are not touched: the water column rides on the
+ * seafloor, so the surface moves with it.  The caller supplies w, the increment of its ramp over [t0, t1] since its last call on
+ * this level (a new level starts from the undeformed bathymetry it was given). */
+typedef struct {
+    double x0, y0, ddx, ddy;
+    int64_t mx, my;             /* nodes per direction, >= 2 */
+    const double *dz;
+    int dz_is_device;
+} gc_deform;
+int gc_bathy_update(gc_level *L, const gc_deform *D /*HOST struct*/, double w);
+
 /* A5-A7 (P:142 step 1; eqs. 13-15): x-sweep then y-sweep over every patch of the level, dry clean-up,
  * exact order-independent max reduction of the wave speeds, swap NEW/OLD.  dt == 0 is a probe: state and
  * buffers unchanged, speeds returned.  out: HOST struct, or NULL = keep the statistics on the device (no

@@ -109,6 +109,15 @@ int gco_level_step(gco_level *L, double dt, gco_step_stats *out);
  * SURVEY 8(d) "patch-level omp parallel for"); used by bench.py's N-core baseline and by the long parity runs */
 int gco_set_threads(int n);
 int gco_get_threads(void);
+/* ---- time-dependent bathymetry (gco_bathy.c); DESIGN.md 3.12 (reading S-20) ---- */
+typedef struct {
+    double x0, y0, ddx, ddy;   /* node (m, n) at (x0 + m ddx, y0 + n ddy), in the level's coordinates */
+    int64_t mx, my;            /* nodes per direction, >= 2 */
+    const double *dz;          /* my rows of mx values: vertical seafloor displacement in metres, + up */
+} gco_deform;
+double gco_deform_at(const gco_deform *D, double x, double y);     /* bilinear between nodes, 0 outside the grid */
+/* b <- fma(w, dz(cell centre), b) on every storage cell inside the domain; h, hu, hv untouched (eta moves with the seafloor) */
+int gco_bathy_update(gco_level *L, const gco_deform *D, double w);
 /* ---- gauges (gco_amr.c); DESIGN.md 3.10 (reading S-19) ---- */
 /* Samples n points from the current state of L (ghost cells as they are): point k = (xy[2k], xy[2k+1]) must lie in the interior
  * of patch patch[k] (else GCO_ERR_BADARG).  out: 4 per point -- h, hu, hv, eta = h + b; bilinear between the four cell centres

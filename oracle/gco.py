@@ -11,7 +11,7 @@ import subprocess
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-_SRC = ["gco_riemann.c", "gco_sweep.c", "gco_level.c", "gco_amr.c", "gco_flux.c"]
+_SRC = ["gco_riemann.c", "gco_sweep.c", "gco_level.c", "gco_amr.c", "gco_flux.c", "gco_bathy.c"]
 _LIB = os.path.join(_DIR, "libgco.so")
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-Wall", "-shared", "-fPIC", "-fopenmp"]
 
@@ -56,6 +56,24 @@ class Params(C.Structure):
 class FlagParams(C.Structure):
     _fields_ = [("tol_eta", C.c_double), ("tol_slope", C.c_double), ("offshore_only", C.c_int),
                 ("buffer", C.c_int), ("nboxes", C.c_int), ("boxes", C.POINTER(C.c_double))]
+
+
+class Deform(C.Structure):
+    _fields_ = [("x0", C.c_double), ("y0", C.c_double), ("ddx", C.c_double), ("ddy", C.c_double),
+                ("mx", C.c_int64), ("my", C.c_int64), ("dz", C.POINTER(C.c_double))]
+
+
+def make_deform(x0, y0, ddx, ddy, dz):
+    """-> (Deform, array kept alive): dz is (my, mx), node (m, n) at (x0 + m ddx, y0 + n ddy)"""
+    a = np.ascontiguousarray(dz, dtype=np.float64)
+    d = Deform(float(x0), float(y0), float(ddx), float(ddy), a.shape[1], a.shape[0], a.ctypes.data_as(C.POINTER(C.c_double)))
+    return d, a
+
+
+def deform_at(x0, y0, ddx, ddy, dz, x, y):
+    d, keep = make_deform(x0, y0, ddx, ddy, dz)
+    f = lib().gco_deform_at; f.restype = C.c_double; f.argtypes = [C.POINTER(Deform), C.c_double, C.c_double]
+    return f(C.byref(d), float(x), float(y))
 
 
 class StepStats(C.Structure):
@@ -232,6 +250,12 @@ class Level:
         _chk(lib().gco_gauges_sample(self.h, len(patch), patch.ctypes.data_as(C.POINTER(C.c_int32)), xy.ctypes.data_as(_dp),
                                      out.ctypes.data_as(_dp)), "gauges_sample")
         return out
+
+    def bathy_update(self, x0, y0, ddx, ddy, dz, w):
+        """b <- fma(w, dz(cell centre), b); dz (my, mx) on the node grid (x0 + m ddx, y0 + n ddy)"""
+        d, keep = make_deform(x0, y0, ddx, ddy, dz)
+        lib().gco_bathy_update.argtypes = [C.c_void_p, C.POINTER(Deform), C.c_double]
+        _chk(lib().gco_bathy_update(self.h, C.byref(d), float(w)), "bathy_update")
 
     def wet_mask(self):
         m = np.zeros(self.ncells, dtype=np.uint8)

@@ -18,7 +18,7 @@ SYMBOLS = [
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
-    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async",
+    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update",
 ]
 
 
@@ -26,6 +26,11 @@ class Params(C.Structure):
     _fields_ = [("coord", C.c_int), ("g", C.c_double), ("dry_tol", C.c_double), ("sea_level", C.c_double),
                 ("earth_radius", C.c_double), ("limiter", C.c_int), ("bc", C.c_int * 4),
                 ("manning_n", C.c_double), ("friction_depth", C.c_double)]
+
+
+class Deform(C.Structure):
+    _fields_ = [("x0", C.c_double), ("y0", C.c_double), ("ddx", C.c_double), ("ddy", C.c_double),
+                ("mx", C.c_int64), ("my", C.c_int64), ("dz", C.c_void_p), ("dz_is_device", C.c_int)]
 
 
 class FlagParams(C.Structure):
@@ -57,6 +62,7 @@ def lib():
     L.gc_ctx_create.argtypes = [vp, vp, ALLOC_FN, FREE_FN, vp, vp]
     L.gc_ctx_destroy.argtypes = [vp]
     L.gc_ctx_set_option.argtypes = [vp, i, i64]
+    L.gc_bathy_update.argtypes = [vp, vp, d]
     L.gc_level_upload_state_async.argtypes = [vp, vp, vp]
     L.gc_level_download_state_async.argtypes = [vp, vp, vp]
     L.gc_last_error.argtypes = [vp]; L.gc_last_error.restype = C.c_char_p
@@ -173,6 +179,12 @@ class Level:
     def step_auto(self, dt_dev, cfl):
         """dt_dev: 1-element float64 CUDA tensor holding dt; updated in place to the next dt."""
         self.ctx._chk(lib().gc_level_step_auto(self.h, dt_dev.data_ptr(), cfl), "gc_level_step_auto")
+
+    def bathy_update(self, x0, y0, ddx, ddy, dz, w):
+        """gc_bathy_update: b <- fma(w, dz(cell centre), b); dz (my, mx) numpy array on the node grid (x0 + m ddx, y0 + n ddy)"""
+        a = np.ascontiguousarray(dz, dtype=np.float64)
+        d = Deform(float(x0), float(y0), float(ddx), float(ddy), a.shape[1], a.shape[0], a.ctypes.data, 0)
+        self.ctx._chk(lib().gc_bathy_update(self.h, C.byref(d), C.c_double(float(w))), "gc_bathy_update")
 
     def upload_state_async(self, host3, copy_stream):
         """host3: three pinned CPU tensors (h, hu, hv) of shape (nyl, nxl), float64; copy_stream: a torch.cuda.Stream"""

@@ -545,6 +545,24 @@ extern "C" int gc_fill_ghost_b(gc_level *L)
     return gc_cuda_check(L->ctx, "gc_fill_ghost_b");
 }
 
+extern "C" int gc_bathy_update(gc_level *L, const gc_deform *D, double w)
+{
+    if (!L || !D || !D->dz || D->mx < 2 || D->my < 2 || !(D->ddx > 0.0) || !(D->ddy > 0.0) || !(w == w))
+        return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_bathy_update: bad argument");
+    gc_ctx *c = L->ctx;
+    const double *dz = D->dz; double *tmp = nullptr; bool transient = false;
+    const size_t bytes = (size_t)D->mx * (size_t)D->my * 8;
+    if (!D->dz_is_device) {
+        tmp = (double *)gc_stage_get(c, bytes, &transient);
+        if (!tmp) return gc_fail(c, GC_ERR_NOMEM, "gc_bathy_update: staging allocation failed");
+        cudaMemcpyAsync(tmp, D->dz, bytes, cudaMemcpyHostToDevice, c->stream);
+        dz = tmp;
+    }
+    gc_launch_bathy_update(L, D->x0, D->y0, D->ddx, D->ddy, D->mx, D->my, dz, w);
+    if (tmp) { cudaStreamSynchronize(c->stream); if (transient) gc_dev_free(c, tmp); }   // the caller's array is free on return
+    return gc_cuda_check(c, "gc_bathy_update");
+}
+
 int gc_fill_coarse_ghosts(gc_level *L, const gc_level *C, double alpha);   // gc_api_amr.cu
 void gc_amr_on_destroy(gc_level *L);                                       // gc_api_amr.cu
 int gc_flux_after_step(gc_level *L, double dt, const double *dt_dev);     // gc_api_amr.cu

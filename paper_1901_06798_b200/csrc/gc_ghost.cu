@@ -210,6 +210,47 @@ void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *sr
     if (n > 0) k_copy2d<<<blocks, 256, 0, s>>>(dst, dld, src, sld, w, h);
 }
 
+// ---- time-dependent bathymetry (P:52 B(x, y, t); P:273, P:333 deformation on uniform grids, reading S-20):
+// b <- fma(w, dz(cell centre), b) on every storage cell whose centre lies inside the domain; dz bilinear between the nodes of
+// the deformation grid, 0 outside it.  Same expressions in the same order as the specification (IEEE divide, no contraction
+// but the one fma).  Grid = patches x chunks.
+struct DeformArgs { double x0, y0, ddx, ddy; long long mx, my; const double *dz; };
+__device__ __forceinline__ double gc_deform_at(const DeformArgs &D, double x, double y)
+{
+    const double s = (x - D.x0) / D.ddx, t = (y - D.y0) / D.ddy;
+    if (!(s >= 0.0) || !(t >= 0.0) || !(s <= (double)(D.mx - 1)) || !(t <= (double)(D.my - 1))) return 0.0;
+    long long m = (long long)floor(s), n = (long long)floor(t);
+    if (m > D.mx - 2) m = D.mx - 2;
+    if (n > D.my - 2) n = D.my - 2;
+    const double a = s - (double)m, c = t - (double)n;
+    const double *z = D.dz + n * D.mx + m;
+    const double lo = (1.0 - a) * z[0] + a * z[1];
+    const double hi = (1.0 - a) * z[D.mx] + a * z[D.mx + 1];
+    return (1.0 - c) * lo + c * hi;
+}
+__global__ void k_bathy_update(const PatchDesc *pat, double *b, DeformArgs D, double w, double xlo, double ylo, double dx, double dy,
+                               int64_t nxl, int64_t nyl)
+{
+    const PatchDesc pd = pat[blockIdx.x];
+    const int W = pd.nx + 4;
+    const int n = W * (pd.ny + 4);
+    const int t1 = min(n, (int)(blockIdx.y + 1) * GC_CHUNK);
+    for (int t = blockIdx.y * GC_CHUNK + threadIdx.x; t < t1; t += blockDim.x) {
+        const int j = t / W, i = t - j * W;
+        const int64_t gi = (int64_t)pd.i0 + i - 2, gj = (int64_t)pd.j0 + j - 2;
+        if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
+        const double x = xlo + ((double)gi + 0.5) * dx, y = ylo + ((double)gj + 0.5) * dy;
+        const int64_t c = pd.off + (int64_t)j * pd.pitch + i;
+        b[c] = __fma_rn(w, gc_deform_at(D, x, y), b[c]);
+    }
+}
+void gc_launch_bathy_update(gc_level *L, double x0, double y0, double ddx, double ddy, int64_t mx, int64_t my, const double *d_dz, double w)
+{
+    ProfScope ps(L->ctx, GC_SLOT_MISC);
+    DeformArgs D; D.x0 = x0; D.y0 = y0; D.ddx = ddx; D.ddy = ddy; D.mx = mx; D.my = my; D.dz = d_dz;
+    if (L->np) k_bathy_update<<<gc_chunk_grid(L, 4), 256, 0, L->ctx->stream>>>(L->d_pat, L->b, D, w, L->xlo, L->ylo, L->dx, L->dy, L->nxl, L->nyl);
+}
+
 // ---- wet mask (h > eps), interior-packed
 __global__ void k_wet_mask(const PatchDesc *pat, const double *h, double eps, uint8_t *mask)
 {

@@ -181,6 +181,7 @@ void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t
 void gc_launch_get_global(const gc_level *L, const double *plane, double *dst, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);
 void gc_launch_copy2d(cudaStream_t s, double *dst, int64_t dld, const double *src, int64_t sld, int w, int h);
 void gc_launch_wet_mask(const gc_level *L, uint8_t *mask);
+void gc_launch_bathy_update(gc_level *L, double x0, double y0, double ddx, double ddy, int64_t mx, int64_t my, const double *d_dz, double w);
 void gc_launch_mass(const gc_level *L);
 int gc_mass_partials(const gc_level *L);    // number of partial sums gc_launch_mass writes to d_partial
 // gc_amr.cu

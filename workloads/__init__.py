@@ -39,6 +39,7 @@ class Workload:
     patch_max: int = 64
     forced_boxes: Tuple = ()          # (level, x0, x1, y0, y1, t0, t1): refine level -> level+1 inside
     wave_levels: int = 99             # the wave criteria (tol_eta, ...) flag levels 1..wave_levels only; finer levels come from boxes
+    deform: dict = None               # seafloor deformation: dict(x0, y0, ddx, ddy, dz (my, mx), t0, t1) or None
     _tiles: dict = field(default_factory=dict, repr=False, compare=False)   # bathy_box cache
 
     def centers(self, level_dx=None, level_dy=None, i0=0, j0=0, nx=None, ny=None):
@@ -198,6 +199,23 @@ def cfg4(nx=1800, ny=900):
     return Workload("cfg4", dict(coord=1, dry_tol=1e-3, bc=(0, 0, 0, 0)), xlo, ylo, d, d, nx, ny, bathy, eta0,
                     cfl=0.9, t_end=36000.0, ratios=(5, 6, 4), flag=dict(tol_eta=0.02, offshore_only=1, buffer=3),
                     regrid_interval=3, patch_min=50, patch_max=200, forced_boxes=boxes, wave_levels=1)
+
+
+def cfg4_deformation(nx=1800, ny=900, t_rise=120.0, spacing=0.1):
+    """Config 4 started the way the paper starts its tsunamis: the ocean is at rest and the +5 m / -2 m dipole is a
+    seafloor deformation on a uniform node grid of `spacing` degrees around the source, applied over [0, t_rise] seconds
+     -- instead of an initial surface displacement over a static bed."""
+    wl = cfg4(nx, ny)
+    src_x, src_y = wl.xlo + 0.08 * nx * wl.dx, wl.ylo + 0.62 * ny * wl.dy
+    x0, y0 = max(wl.xlo, src_x - 8.0), src_y - 10.0
+    mx, my = int(round((src_x + 6.0 - x0) / spacing)) + 1, int(round(20.0 / spacing)) + 1
+    X, Y = np.meshgrid(x0 + spacing * np.arange(mx), y0 + spacing * np.arange(my))
+    dz = np.ascontiguousarray(wl.eta0(X, Y), dtype=np.float64)
+    dz[np.abs(dz) < 1e-4] = 0.0                                    # a deformation file has a finite footprint
+    wl.deform = dict(x0=float(x0), y0=float(y0), ddx=float(spacing), ddy=float(spacing), dz=dz, t0=0.0, t1=float(t_rise))
+    wl.eta0 = lambda x, y: np.zeros(np.broadcast(x, y).shape)
+    wl.name = "cfg4-deformation"
+    return wl
 
 
 def cfg5(n=8192):
