@@ -16,6 +16,18 @@ import time
 import numpy as np
 
 
+def fallback_of(L):
+    """P:345 accounting of a level still alive at the end of the run: the share of the marching kernels' warp iterations in which
+    some lane left the guarded open-ocean code, and the share of lane-level edges redone with the general code (0 / None for a
+    level swept by the edge-parallel kernels)"""
+    c = L.fallback_counts()
+    if c["warp_iters"] == 0:
+        return dict(level=int(L.level), cells=int(L.ncells), marching=False)
+    return dict(level=int(L.level), cells=int(L.ncells), marching=True, warp_iters=int(c["warp_iters"]),
+                warp_iter_fraction=c["fb_warp_iters"] / c["warp_iters"],
+                edge_fraction=0.5 * (c["fb_solves"] + c["fb_fluxes"]) / (32.0 * c["warp_iters"]))
+
+
 def run_single(cfg, wl, patches, max_steps, graph_k, device):
     import torch
     from paper_1901_06798_b200 import binding
@@ -69,7 +81,8 @@ def run_single(cfg, wl, patches, max_steps, graph_k, device):
         assert st["nan_seen"] == 0
         out = dict(levels=1, patches=int(len(L.patches)), steps=done, sim_time=float(t_dev.item()), updates=int(L.ncells) * done,
                    wall_s=wall, device_ms=e0.elapsed_time(e1), launches=int(ctx.launch_count() - lc0) + launched_by_graph,
-                   graph_steps=int(graph_k or 0) if g is not None else 0, wet_cells=int(L.wet_mask().sum()), mass=L.mass())
+                   graph_steps=int(graph_k or 0) if g is not None else 0, wet_cells=int(L.wet_mask().sum()), mass=L.mass(),
+                   fallback=[fallback_of(L)])
         L.destroy()
     return out
 
@@ -96,7 +109,8 @@ def run_amr(cfg, wl, max_steps, max_wall, device, max_levels=None):
     wall = time.time() - w0
     out = dict(levels=len(H.levels), patches=[int(len(L.patches)) for L in H.levels], cells=[int(L.ncells) for L in H.levels],
                steps=n, sim_time=H.t, t_end=wl.t_end, finished=bool(H.t >= wl.t_end), updates=int(H.updates), regrids=int(H.regrids),
-               wall_s=wall, setup_s=t_setup, launches=int(ctx.launch_count() - lc0))
+               wall_s=wall, setup_s=t_setup, launches=int(ctx.launch_count() - lc0),
+               fallback=[fallback_of(L) for L in H.levels])
     H.destroy()
     return out
 
@@ -113,8 +127,13 @@ def main():
                     help="config 4: switch the forced coastal boxes on at t = 0 instead of 6 h / 6.5 h, so that all four levels exist at once")
     ap.add_argument("--graph", type=int, default=0, help="single-level configs: replay the step as a CUDA graph of this many steps")
     ap.add_argument("--device", default="cuda:0")
+    ap.add_argument("--family", choices=["auto", "edge", "march"], default="auto", help="sweep kernel family (gc_ctx_set_option)")
+    ap.add_argument("--seg", type=int, default=0, help="marching segment length in cells (0 = by level size)")
     a = ap.parse_args()
     import workloads
+    from paper_1901_06798_b200 import binding
+    binding.DEFAULT_OPTIONS[binding.OPT_SWEEP_FAMILY] = {"auto": 0, "edge": 1, "march": 2}[a.family]
+    binding.DEFAULT_OPTIONS[binding.OPT_MARCH_SEG] = a.seg
     if a.config == 1:
         wl = workloads.cfg1(a.scale or 64); res = run_single(1, wl, None, a.max_steps, a.graph, a.device)
     elif a.config == 2:

@@ -20,6 +20,13 @@ int64_t gc_launch_count(const gc_ctx *);
 int gc_profile_enable(gc_ctx *, int on);
 int gc_profile_read(gc_ctx *, double *ms /*HOST*/, int64_t *count /*HOST*/);
 
+/* How often the line-marching sweep kernels left their guarded open-ocean code on this level, cumulative since it was created
+ * (the paper's hazard: divergence at shorelines).  out[0] = warp iterations of the marching kernels (one iteration = one
+ * cell per lane); out[1] = those in which at least one lane's cell or edge went through the general code; out[2], out[3] =
+ * lane-level Riemann solves / edge fluxes redone with the general code.  Levels swept by the edge-parallel kernels report 0.
+ * Synchronises the context's stream. */
+int gc_level_fallback_counts(const gc_level *L, int64_t out[4] /*HOST*/);
+
 /* Self-test of the branch-free correctly rounded divide / reciprocal / square root the marching kernels use
  * (csrc/gc_math.cuh) against the IEEE operators: for each i, a[i]/b[i], 1/b[i], sqrt(a[i]) (a, b: HOST arrays of n).
  * nmismatch = results that differ in any bit although the fast path accepted the operands (must be 0);

@@ -352,6 +352,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     }
     L->nbcp = (int)bcp.size(); L->d_bcp = upload(L, bcp);
     L->d_stats = (DevStats *)gc_dev_alloc(ctx, sizeof(DevStats)); L->allocs.push_back(L->d_stats);
+    if (L->d_stats) cudaMemsetAsync(L->d_stats, 0, sizeof(DevStats), ctx->stream);
     L->d_partial = (double *)gc_dev_alloc(ctx, sizeof(double) * (size_t)std::max(gc_mass_partials(L), 1)); L->allocs.push_back(L->d_partial);
     L->cf_for = nullptr; L->cf_gen = 0; L->d_cf = nullptr; L->d_cfstart = nullptr; L->ncf = 0; L->ncfcells = 0;
     L->avg_gen = 0; L->d_avg = nullptr; L->d_avgstart = nullptr; L->navg = 0; L->navgcells = 0;
@@ -592,6 +593,18 @@ extern "C" int gc_level_stats(const gc_level *L, gc_step_stats *out)
     if (rc) return rc;
     double sdx; memcpy(&sdx, &s.sdx_bits, 8);
     out->s_over_dx_max = sdx; out->cfl_max = 0.0; out->clipped_mass = s.clipped; out->n_clipped = (int64_t)s.nclip; out->nan_seen = s.nan_seen;
+    return GC_OK;
+}
+
+extern "C" int gc_level_fallback_counts(const gc_level *L, int64_t out[4])
+{
+    if (!L || !out) return GC_ERR_BADARG;
+    DevStats s;
+    cudaMemcpyAsync(&s, L->d_stats, sizeof s, cudaMemcpyDeviceToHost, L->ctx->stream);
+    cudaStreamSynchronize(L->ctx->stream);
+    int rc = gc_cuda_check(L->ctx, "gc_level_fallback_counts");
+    if (rc) return rc;
+    out[0] = (int64_t)s.warp_iters; out[1] = (int64_t)s.fb_warp_iters; out[2] = (int64_t)s.fb_solves; out[3] = (int64_t)s.fb_fluxes;
     return GC_OK;
 }
 

@@ -324,11 +324,17 @@ extern "C" int gc_flux_attach(gc_level *C, gc_level *F)
     std::vector<int32_t> fstart(1, 0), freg;
     for (auto &gr : groups) { for (int32_t n : gr) freg.push_back(n); fstart.push_back((int32_t)freg.size()); }
 
+    // allocate the new arrays first and swap on success: a failed attach leaves the previous attachment as it was
+    FluxReg *n_reg = upload_tmp(ctx, regs); int32_t *n_fixstart = upload_tmp(ctx, fstart), *n_fixreg = upload_tmp(ctx, freg);
+    double *n_delta = (double *)gc_dev_alloc(ctx, std::max<size_t>(regs.size(), 1) * 3 * sizeof(double));
+    double *n_base = (double *)gc_dev_alloc(ctx, std::max<size_t>(regs.size(), 1) * 4 * sizeof(double));
+    if (!n_reg || !n_fixstart || !n_fixreg || !n_delta || !n_base) {
+        cudaStreamSynchronize(ctx->stream);
+        gc_dev_free(ctx, n_reg); gc_dev_free(ctx, n_fixstart); gc_dev_free(ctx, n_fixreg); gc_dev_free(ctx, n_delta); gc_dev_free(ctx, n_base);
+        return gc_fail(ctx, GC_ERR_NOMEM, "gc_flux_attach: allocation failed");
+    }
     drop_alloc(C, C->d_reg); drop_alloc(C, C->d_delta); drop_alloc(C, C->d_base); drop_alloc(C, C->d_fixstart); drop_alloc(C, C->d_fixreg);
-    C->d_reg = upload_tmp(ctx, regs); C->d_fixstart = upload_tmp(ctx, fstart); C->d_fixreg = upload_tmp(ctx, freg);
-    C->d_delta = (double *)gc_dev_alloc(ctx, std::max<size_t>(regs.size(), 1) * 3 * sizeof(double));
-    C->d_base = (double *)gc_dev_alloc(ctx, std::max<size_t>(regs.size(), 1) * 4 * sizeof(double));
-    if (!C->d_reg || !C->d_fixstart || !C->d_fixreg || !C->d_delta || !C->d_base) return gc_fail(ctx, GC_ERR_NOMEM, "gc_flux_attach: allocation failed");
+    C->d_reg = n_reg; C->d_fixstart = n_fixstart; C->d_fixreg = n_fixreg; C->d_delta = n_delta; C->d_base = n_base;
     C->allocs.push_back(C->d_reg); C->allocs.push_back(C->d_fixstart); C->allocs.push_back(C->d_fixreg);
     C->allocs.push_back(C->d_delta); C->allocs.push_back(C->d_base);
     cudaMemsetAsync(C->d_delta, 0, std::max<size_t>(regs.size(), 1) * 3 * sizeof(double), ctx->stream);

@@ -9,7 +9,7 @@
 #include "../../include/gc_test.h"
 
 #define GC_G 2  // ghost width
-#define GC_MARCH_MIN_CELLS 2000000   // levels at least this large use the line-marching sweep kernels
+#define GC_MARCH_MIN_CELLS 800000    // levels at least this large use the line-marching sweep kernels
 
 // patch descriptor as the kernels see it (A1): interior box, element offset of the patch in a field plane, row pitch
 struct PatchDesc {
@@ -73,6 +73,10 @@ struct DevStats {
     double clipped;
     int nan_seen;
     int pad;
+    // cumulative since the level was created (never reset by a step): how often the marching kernels left the guarded open-ocean
+    // code (divergence at shorelines).  warp_iters: warp iterations in all; fb_warp_iters: of these, the ones in which some
+    // lane ran the general code; fb_solves / fb_fluxes: lane-level Riemann solves / edge fluxes redone with the general code
+    unsigned long long warp_iters, fb_warp_iters, fb_solves, fb_fluxes;
 };
 
 // profiling slots (gc_profile_read): kernels grouped by the SURVEY 8(a) row they implement

@@ -346,6 +346,14 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         const bool badA = live && !(r >= 1 ? okR : okP);
         const bool badB = needB && !okB;
         if (__any_sync(0xffffffffu, badA || badB)) {
+            {   // P:345 accounting: one lane per warp, only on this (rare in open ocean) path
+                const unsigned ma = __ballot_sync(0xffffffffu, badA), mb = __ballot_sync(0xffffffffu, badB);
+                if ((threadIdx.x & 31) == 0) {
+                    atomicAdd(&a.stats->fb_warp_iters, 1ull);
+                    atomicAdd(&a.stats->fb_solves, (unsigned long long)__popc(ma));
+                    atomicAdd(&a.stats->fb_fluxes, (unsigned long long)__popc(mb));
+                }
+            }
             if (badA) {
                 MathIeee mi;
                 R.h = qh; R.p = qp; R.t = qt; R.b = qb;
@@ -437,7 +445,10 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 
     // A7: exact, order-independent max: warp shuffle, then one atomicMax per warp on the bit image (values >= 0)
     cflm = warp_max(cflm);
-    if ((threadIdx.x & 31) == 0 && cflm > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(cflm));
+    if ((threadIdx.x & 31) == 0) {
+        if (cflm > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(cflm));
+        atomicAdd(&a.stats->warp_iters, (unsigned long long)(nst_warp + 1));
+    }
 }
 
 __global__ void k_stats_reset(DevStats *s) { s->sdx_bits = 0ull; s->nclip = 0ull; s->clipped = 0.0; s->nan_seen = 0; }
