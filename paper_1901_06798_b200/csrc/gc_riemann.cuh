@@ -210,7 +210,7 @@ __device__ __forceinline__ bool gc_prim_fast(RState &S, double g, double hg, dou
     S.u = S.p * rh; S.v = S.t * rh;
     S.phi = __fma_rn(S.p, S.u, hg * (S.h * S.h));
     S.c = gc_fsqrt(g * S.h);
-    return (S.h > hlo) && (S.h <= 0x1p100);
+    return (S.h > hlo) & (S.h <= 0x1p100);
 }
 
 // R3-R8 of an edge whose two cells passed gc_prim_fast.  Writes all of Z and s (garbage when it returns false).
@@ -220,7 +220,7 @@ __device__ __forceinline__ bool gc_riemann_fast(double g, const RState &L, const
     // guard G
     const double cmn = dmin(cL, cR);
     const double c4 = 0.25 * cmn;
-    bool ok = (fabs(cL - cR) <= c4) && (fabs(L.u) <= c4) && (fabs(R.u) <= c4) && (cmn >= 0.1);
+    bool ok = (fabs(cL - cR) <= c4) & (fabs(L.u) <= c4) & (fabs(R.u) <= c4) & (cmn >= 0.1);      // bitwise: no short-circuit branches
     // R4 (= R6 under G)
     const double hsum = hL + hR;
     const double ghbar = g * (0.5 * hsum);                               // max(0.5 (hL + hR), 0) = 0.5 (hL + hR): both wet
@@ -244,7 +244,7 @@ __device__ __forceinline__ bool gc_riemann_fast(double g, const RState &L, const
     // hsd > 1e-100 and |dh| < 1e100 keep every product away from underflow / overflow.  Otherwise: general code.
     {
         const double hs = hsd * 0.9999999;
-        ok = ok && (hsd > 1.0e-100) && (fabs(dh) < 1.0e100) && (dh * l3 < hs) && (dh * l1 < hs);
+        ok = ok & (hsd > 1.0e-100) & (fabs(dh) < 1.0e100) & (dh * l3 < hs) & (dh * l1 < hs);
     }
     {
         const double a = -hL * delb, c = -hR * delb;

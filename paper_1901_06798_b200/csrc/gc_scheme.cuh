@@ -108,8 +108,8 @@ __device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double
 // Same values as gc_edge_flux: the fluctuation sums are formed in the same order, a skipped term is added as +0.0 (no bit
 // changes: the partial sums start at +0.0 and are therefore never -0.0), -|s0| = s0 exactly, Z[1][0] is +0.0 by construction
 // (so its square drops out of zz: fma(x, x, +0) = fl(x x) for every x).  The three limiter divides use the unchecked
-// sequence: the function returns false -- and the caller redoes the edge with gc_edge_flux -- unless all six operands are
-// inside its window (a zero wave or a zero upwind product is outside) and s[1] != 0.  dtdx_ave = 0.5 fma(dt, rdL, dt rdR).
+// sequence: the function returns false -- and the caller redoes the edge with gc_edge_flux -- unless, for every family, the
+// wave is exactly zero (then Phi = 1) or both operands are inside its window (a zero upwind product is outside), and s[1] != 0.  dtdx_ave = 0.5 fma(dt, rdL, dt rdR).
 __device__ __forceinline__ double gc_mc_fast(double theta)
 {
     return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));                      // MC
@@ -133,11 +133,15 @@ __device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&
     const double zz1 = __fma_rn(W.Z[1][2], W.Z[1][2], W.Z[1][1] * W.Z[1][1]);
     const double zz2 = __fma_rn(W.Z[2][2], W.Z[2][2], __fma_rn(W.Z[2][1], W.Z[2][1], W.Z[2][0] * W.Z[2][0]));
     const double zi0 = dhi[0], zi1 = pos1 ? dlo[1] : dhi[1], zi2 = dlo[2];
-    const bool ok = (neg1 || pos1) && gc_in_window(zz0) && gc_in_window(zz1) && gc_in_window(zz2)
-                    && gc_in_window(zi0) && gc_in_window(zi1) && gc_in_window(zi2);
-    const double c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi0, zz0));
-    const double c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi1, zz1));
-    const double c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * gc_mc_fast(gc_fdiv(zi2, zz2));
+    // a family whose wave is exactly zero (an ocean at rest: most of the domain before the tsunami arrives) takes Phi = 1, as in
+    // gc_edge_flux; its quotient is garbage and discarded.  A non-zero wave needs both operands inside the divide's window.
+    const bool z0 = gc_is_zero(zz0), z1 = gc_is_zero(zz1), z2 = gc_is_zero(zz2);
+    const bool ok = (neg1 | pos1) & (z0 | (gc_in_window(zz0) & gc_in_window(zi0))) & (z1 | (gc_in_window(zz1) & gc_in_window(zi1)))
+                    & (z2 | (gc_in_window(zz2) & gc_in_window(zi2)));           // bitwise on purpose: no short-circuit branches
+    const double p0 = gc_mc_fast(gc_fdiv(zi0, zz0)), p1 = gc_mc_fast(gc_fdiv(zi1, zz1)), p2 = gc_mc_fast(gc_fdiv(zi2, zz2));
+    const double c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * (z0 ? 1.0 : p0);
+    const double c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * (z1 ? 1.0 : p1);
+    const double c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * (z2 ? 1.0 : p2);
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const double F = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + c1 * W.Z[1][c];                         // eq. 9, outer families first

@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         RState R; R.h = qh; R.p = qp; R.t = qt; R.b = qb;
         Waves Wn;
         const bool okP = gc_prim_fast(R, a.g, a.hg, a.hlo);
-        const bool okR = gc_riemann_fast(a.g, Lst, R, Wn.Z, Wn.s) && okP && Lok;
+        const bool okR = gc_riemann_fast(a.g, Lst, R, Wn.Z, Wn.s) & okP & Lok;
 
         // ---- B: edge r-2, standard-edge code
         double dhi[3];                                                                  // Z(r-2) . Z(r-1) per family
@@ -338,14 +338,14 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         dhi[2] = __fma_rn(W2.Z[2][2], Z1[7], __fma_rn(W2.Z[2][1], Z1[6], W2.Z[2][0] * Z1[5]));
         const double dtdx_ave = 0.5 * __fma_rn(dt, rd3, dt * rd2);
         double fm[3], fp[3];
-        const bool okB = gc_edge_flux_std(W2, dlo, dhi, dtdx_ave, fm, fp) && std2 && mc;
+        const bool okB = gc_edge_flux_std(W2, dlo, dhi, dtdx_ave, fm, fp) & std2 & mc;
         double cfle = gc_edge_cfl_std(W2, rd3, rd2);
 
         // ---- lanes whose cell / edge is of another kind: general code, IEEE operators (same bits where both apply)
-        const bool needB = r >= 4 && r <= nst;
-        const bool badA = live && !(r >= 1 ? okR : okP);
-        const bool badB = needB && !okB;
-        if (__any_sync(0xffffffffu, badA || badB)) {
+        const bool needB = (r >= 4) & (r <= nst);
+        const bool badA = live & !(r >= 1 ? okR : okP);
+        const bool badB = needB & !okB;
+        if (__any_sync(0xffffffffu, badA | badB)) {
             {   // P:345 accounting: one lane per warp, only on this (rare in open ocean) path
                 const unsigned ma = __ballot_sync(0xffffffffu, badA), mb = __ballot_sync(0xffffffffu, badB);
                 if ((threadIdx.x & 31) == 0) {
@@ -385,7 +385,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         }
 
         // ---- edge r takes the place of edge r-2; Z(r-2).Z(r-1) and fp(r-2) for the next iteration
-        const double stdn = __longlong_as_double((long long)((okR && live && r >= 1) ? 1 : 0));
+        const double stdn = __longlong_as_double((long long)((okR & live & (r >= 1)) ? 1 : 0));
         sts2(wa, Wn.Z[0][0], Wn.Z[0][1]); sts2(wa + PK_SL, Wn.Z[0][2], Wn.Z[1][1]); sts2(wa + 2 * PK_SL, Wn.Z[1][2], Wn.Z[2][0]);
         sts2(wa + 3 * PK_SL, Wn.Z[2][1], Wn.Z[2][2]); sts2(wa + 4 * PK_SL, Wn.s[0], Wn.s[1]); sts2(wa + 5 * PK_SL, Wn.s[2], stdn);
         sts2(sm0 + PK_DOT * PK_SL, dhi[0], dhi[1]); sts2(sm0 + (PK_DOT + 1) * PK_SL, dhi[2], fp[0]); sts2(sm0 + (PK_DOT + 2) * PK_SL, fp[1], fp[2]);
