@@ -109,7 +109,8 @@ __device__ __forceinline__ double gc_edge_cfl(const Waves &W, double rdL, double
 // changes: the partial sums start at +0.0 and are therefore never -0.0), -|s0| = s0 exactly, Z[1][0] is +0.0 by construction
 // (so its square drops out of zz: fma(x, x, +0) = fl(x x) for every x).  The three limiter divides use the unchecked
 // sequence: the function returns false -- and the caller redoes the edge with gc_edge_flux -- unless, for every family, the
-// wave is exactly zero (then Phi = 1) or both operands are inside its window (a zero upwind product is outside), and s[1] != 0.  dtdx_ave = 0.5 fma(dt, rdL, dt rdR).
+// wave is exactly zero (then Phi = 1) or it is inside the window and the upwind product is zero (Phi = that signed zero) or inside
+// the window too.  dtdx_ave = 0.5 fma(dt, rdL, dt rdR).
 __device__ __forceinline__ double gc_mc_fast(double theta)
 {
     return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));                      // MC
@@ -123,10 +124,10 @@ __device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&
     am[0] = 0.0 + W.Z[0][0];
     ap[0] = 0.0 + W.Z[2][0];
 #pragma unroll
-    for (int c = 1; c < 3; c++) {
-        const double z = W.Z[1][c];
-        am[c] = (0.0 + W.Z[0][c]) + (neg1 ? z : 0.0);
-        ap[c] = (0.0 + (pos1 ? z : 0.0)) + W.Z[2][c];
+    for (int c = 1; c < 3; c++) {                       // s1 = 0 (still water over a flat bed): half of the wave each way (S-4)
+        const double z = W.Z[1][c], hz = 0.5 * z;
+        am[c] = (0.0 + W.Z[0][c]) + (neg1 ? z : (pos1 ? 0.0 : hz));
+        ap[c] = (0.0 + (pos1 ? z : (neg1 ? 0.0 : hz))) + W.Z[2][c];
     }
     // eq. 10 (S-1), eq. 11: upwind neighbour e+1 for family 1 (s < 0), e-1 for family 3 (s > 0), by sign for family 2
     const double zz0 = __fma_rn(W.Z[0][2], W.Z[0][2], __fma_rn(W.Z[0][1], W.Z[0][1], W.Z[0][0] * W.Z[0][0]));
@@ -135,16 +136,21 @@ __device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&
     const double zi0 = dhi[0], zi1 = pos1 ? dlo[1] : dhi[1], zi2 = dlo[2];
     // a family whose wave is exactly zero (an ocean at rest: most of the domain before the tsunami arrives) takes Phi = 1, as in
     // gc_edge_flux; its quotient is garbage and discarded.  A non-zero wave needs both operands inside the divide's window.
+    // A zero upwind product (the neighbour's wave vanishes: common in still water, where the corrector wave is rounding noise and
+    // now and then exactly 0) gives theta = zi / zz = zi, a signed zero, and Phi(+-0) = +-0 with that sign: Phi = zi itself.
     const bool z0 = gc_is_zero(zz0), z1 = gc_is_zero(zz1), z2 = gc_is_zero(zz2);
-    const bool ok = (neg1 | pos1) & (z0 | (gc_in_window(zz0) & gc_in_window(zi0))) & (z1 | (gc_in_window(zz1) & gc_in_window(zi1)))
-                    & (z2 | (gc_in_window(zz2) & gc_in_window(zi2)));           // bitwise on purpose: no short-circuit branches
+    const bool y0 = gc_is_zero(zi0), y1 = gc_is_zero(zi1), y2 = gc_is_zero(zi2);
+    const bool on1 = neg1 | pos1;                                                 // sgn(0) = 0: no correction from a steady wave
+    const bool ok = (z0 | (gc_in_window(zz0) & (y0 | gc_in_window(zi0)))) & (!on1 | z1 | (gc_in_window(zz1) & (y1 | gc_in_window(zi1))))
+                    & (z2 | (gc_in_window(zz2) & (y2 | gc_in_window(zi2))));    // bitwise on purpose: no short-circuit branches
     const double p0 = gc_mc_fast(gc_fdiv(zi0, zz0)), p1 = gc_mc_fast(gc_fdiv(zi1, zz1)), p2 = gc_mc_fast(gc_fdiv(zi2, zz2));
-    const double c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * (z0 ? 1.0 : p0);
-    const double c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * (z1 ? 1.0 : p1);
-    const double c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * (z2 ? 1.0 : p2);
+    const double c0 = (-0.5 * __fma_rn(s0, dtdx_ave, 1.0)) * (z0 ? 1.0 : (y0 ? zi0 : p0));
+    const double c1 = ((pos1 ? 0.5 : -0.5) * __fma_rn(-fabs(s1), dtdx_ave, 1.0)) * (z1 ? 1.0 : (y1 ? zi1 : p1));
+    const double c2 = (0.5 * __fma_rn(-s2, dtdx_ave, 1.0)) * (z2 ? 1.0 : (y2 ? zi2 : p2));
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        const double F = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + c1 * W.Z[1][c];                         // eq. 9, outer families first
+        const double t1 = c1 * W.Z[1][c];
+        const double F = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + (on1 ? t1 : 0.0);                       // eq. 9, outer families first
         fm[c] = F + am[c]; fp[c] = F - ap[c];
     }
     return ok;
