@@ -12,12 +12,14 @@
 // row by row with the lanes along x (coalesced), a narrow one several rows per pass (lane -> (row, column): one division per
 // rectangle, none per cell).  Two rows are in flight per lane and plane before anything is stored.  Pure data movement:
 // every ghost cell written once, 48 bytes of algorithmic traffic per cell (3 planes read + written).
+// (the cells read are interior cells, the cells written ghost cells: the two sets are disjoint, so the loads may take the
+// read-only path and move ahead of the stores)
 template <int NF>
 __device__ __forceinline__ void copy_pair(double *f0, double *f1, double *f2, int64_t d0, int64_t s0, int64_t d1, int64_t s1, bool two)
 {
-    double a0 = f0[s0], a1 = 0.0, a2 = 0.0, b0 = 0.0, b1 = 0.0, b2 = 0.0;
-    if (NF > 1) { a1 = f1[s0]; a2 = f2[s0]; }
-    if (two) { b0 = f0[s1]; if (NF > 1) { b1 = f1[s1]; b2 = f2[s1]; } }
+    double a0 = __ldg(f0 + s0), a1 = 0.0, a2 = 0.0, b0 = 0.0, b1 = 0.0, b2 = 0.0;
+    if (NF > 1) { a1 = __ldg(f1 + s0); a2 = __ldg(f2 + s0); }
+    if (two) { b0 = __ldg(f0 + s1); if (NF > 1) { b1 = __ldg(f1 + s1); b2 = __ldg(f2 + s1); } }
     f0[d0] = a0; if (NF > 1) { f1[d0] = a1; f2[d0] = a2; }
     if (two) { f0[d1] = b0; if (NF > 1) { f1[d1] = b1; f2[d1] = b2; } }
 }
@@ -30,25 +32,35 @@ __global__ void __launch_bounds__(256, 5) k_copy_rects(const CopyRect *rects, co
     const int patch = gw / wpp, sub = gw - patch * wpp;
     if (patch >= np) return;
     const int2 pr = range[patch];
-    for (int i = 0; i < pr.y; i++) {
-        const CopyRect r = rects[pr.x + i];
-        if (r.w >= 32) {
-            for (int y = 2 * sub; y < r.h; y += 2 * wpp) {
-                const bool two = y + 1 < r.h;
-                for (int x = lane; x < r.w; x += 32)
-                    copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
-                                  r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, two);
-            }
-        } else {
-            int rpp, ly, lx;                                           // rows per pass; this lane's row and column in a pass
-            if (r.w == 2) { rpp = 16; ly = lane >> 1; lx = lane & 1; }                 // x faces, corners: no division
-            else if (r.w == 16) { rpp = 2; ly = lane >> 4; lx = lane & 15; }
-            else { rpp = 32 / r.w; ly = lane / r.w; lx = lane - ly * r.w; }
-            if (ly < rpp) {
-                for (int y = 2 * sub * rpp + ly; y < r.h; y += 2 * wpp * rpp) {
-                    const bool two = y + rpp < r.h;
-                    copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + lx, r.src + (int64_t)y * r.spitch + lx,
-                                  r.dst + (int64_t)(y + rpp) * r.dpitch + lx, r.src + (int64_t)(y + rpp) * r.spitch + lx, two);
+    for (int i0 = 0; i0 < pr.y; i0 += 32) {
+        // the patch's rectangle descriptors arrive with one load (lane k takes rectangle i0 + k) and are handed round by shuffles:
+        // one memory round trip instead of one per rectangle
+        CopyRect mine; mine.dst = 0; mine.src = 0; mine.w = 0; mine.h = 0; mine.dpitch = 0; mine.spitch = 0;
+        if (i0 + lane < pr.y) mine = rects[pr.x + i0 + lane];
+        const int cnt = min(32, pr.y - i0);
+        for (int i = 0; i < cnt; i++) {
+            CopyRect r;
+            r.dst = __shfl_sync(0xffffffffu, mine.dst, i); r.src = __shfl_sync(0xffffffffu, mine.src, i);
+            r.w = __shfl_sync(0xffffffffu, mine.w, i); r.h = __shfl_sync(0xffffffffu, mine.h, i);
+            r.dpitch = __shfl_sync(0xffffffffu, mine.dpitch, i); r.spitch = __shfl_sync(0xffffffffu, mine.spitch, i);
+            if (r.w >= 32) {
+                for (int y = 2 * sub; y < r.h; y += 2 * wpp) {
+                    const bool two = y + 1 < r.h;
+                    for (int x = lane; x < r.w; x += 32)
+                        copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
+                                      r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, two);
+                }
+            } else {
+                int rpp, ly, lx;                                           // rows per pass; this lane's row and column in a pass
+                if (r.w == 2) { rpp = 16; ly = lane >> 1; lx = lane & 1; }                 // x faces, corners: no division
+                else if (r.w == 16) { rpp = 2; ly = lane >> 4; lx = lane & 15; }
+                else { rpp = 32 / r.w; ly = lane / r.w; lx = lane - ly * r.w; }
+                if (ly < rpp) {
+                    for (int y = 2 * sub * rpp + ly; y < r.h; y += 2 * wpp * rpp) {
+                        const bool two = y + rpp < r.h;
+                        copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + lx, r.src + (int64_t)y * r.spitch + lx,
+                                      r.dst + (int64_t)(y + rpp) * r.dpitch + lx, r.src + (int64_t)(y + rpp) * r.spitch + lx, two);
+                    }
                 }
             }
         }
