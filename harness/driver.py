@@ -408,6 +408,9 @@ class Hierarchy:
         self.ctx, self.wl, self.reflux, self.eff = ctx, wl, reflux, efficiency
         self.gauges = gauges             # GaugeRecorder or None
         self.keep_unchanged = keep_unchanged   # keep a level whose regrid reproduces its patch list (bit-identical to recreating it)
+        self.reuse_box_flags = keep_unchanged  # and do not re-flag a level whose flags can only come from unchanged forced boxes
+        self._boxflag_cache = {}
+        self._attached = {}              # level index k -> (coarse, fine) level objects whose flux registers are attached
         self.kept = 0
         nl = 1 + len(wl.ratios) if max_levels is None else min(max_levels, 1 + len(wl.ratios))
         self.ratios = list(wl.ratios)[:nl - 1]
@@ -439,6 +442,21 @@ class Hierarchy:
         # flag kernel applies): the pass would return no flags, so it is not launched and nothing is downloaded
         if not wave and not any(b[4] <= t <= b[5] for b in boxes):
             return None
+        # flags that come from forced boxes alone are a function of the level's patch list and of the set of active boxes: a level
+        # that regrids every few of its steps over the same patches inside the same boxes is not flagged again (no launch, no
+        # download, no clustering; the flagging passes that are run are still logged for the parity check)
+        ckey = None
+        if not wave and self.reuse_box_flags:
+            ckey = (k, np.ascontiguousarray(L.patches).tobytes(), tuple(b for b in boxes if b[4] <= t <= b[5]))
+            hit = self._boxflag_cache.get(k)
+            if hit is not None and hit[0] == ckey:
+                return None if hit[1] is None else hit[1].copy()
+        pats = self._flag_and_cluster(k, t, L, f, wave, boxes)
+        if ckey is not None:
+            self._boxflag_cache[k] = (ckey, None if pats is None else pats.copy())
+        return pats
+
+    def _flag_and_cluster(self, k, t, L, f, wave, boxes):
         packed, n = L.flag(tol_eta=f.get("tol_eta", 0.0) if wave else 0.0, tol_slope=0.0, offshore_only=f.get("offshore_only", 0),
                            buffer=f.get("buffer", 0), boxes=boxes, t=t)
         self.flag_log.append((k, t, packed.copy()))
@@ -479,8 +497,10 @@ class Hierarchy:
                 # would copy every interior cell from the old level, and every ghost cell is rewritten before it is read (DESIGN.md
                 # 3.6), so the level stays as it is: bit-identical to recreating it (tests/test_oracle_amr.py)
                 C.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
-                if self.reflux:
-                    C.flux_attach(old)
+                a = self._attached.get(k)
+                if self.reflux and not (a is not None and a[0] is C and a[1] is old):
+                    C.flux_attach(old)             # (else both levels are unchanged and their registers just fixed up and re-zeroed)
+                    self._attached[k] = (C, old)
                 self.kept += 1
                 continue
             dx, dy, nxl, nyl = self._geom(k + 1)
@@ -497,6 +517,7 @@ class Hierarchy:
                 self.levels.append(N); self.alpha_now.append(1.0); self.steps.append(0); self.sdx.append(0.0)
             if self.reflux:
                 C.flux_attach(N)
+                self._attached[k] = (C, N)
         if self.gauges is not None:
             self.gauges.rebind(self.levels)
 

@@ -245,6 +245,11 @@ def test_keeping_a_level_whose_regrid_reproduces_it_changes_no_bit(gco, monkeypa
         assert np.array_equal(La.patches, Lb.patches)
         for f in ("h", "hu", "hv", "b"):
             assert np.array_equal(La.get_global(f, fill=0.0), Lb.get_global(f, fill=0.0)), (case, La.level, f)
-    assert len(Ha.flag_log) == len(Hb.flag_log)
-    for (ka, ta, fa), (kb, tb, fb) in zip(Ha.flag_log, Hb.flag_log):
-        assert ka == kb and ta == tb and np.array_equal(fa, fb)
+    # the keeping run does not flag again a level whose flags can only come from unchanged forced boxes: its log is a sub-sequence
+    # of the other's, and every pass it did run saw the same flags
+    ref = {}
+    for kb, tb, fb in Hb.flag_log:
+        ref.setdefault((kb, tb), []).append(fb)                # (a level can be flagged twice at one time: its own regrid, then a coarser level's)
+    assert 0 < len(Ha.flag_log) <= len(Hb.flag_log)
+    for ka, ta, fa in Ha.flag_log:
+        assert any(np.array_equal(fa, fb) for fb in ref[(ka, ta)])
