@@ -49,6 +49,10 @@ def set_initial(L, wl, state=True):
                     L.set_patches("b", arr)
                     L.fill_ghost_b()
                     return
+        if not state and L.nxl * L.nyl <= CANVAS_MAX_CELLS:
+            set_bathy_from_canvas(L, wl)       # no host assembly, no upload: the level's cells are gathered from a resident canvas
+            L.fill_ghost_b()
+            return
         if not state:
             packed_b = pack_bathy_native(L, wl)
             L.set_patches("b", packed_b)
@@ -248,6 +252,39 @@ def nesting_mask_native(L, bbox):
     ok = np.empty((ej - bj, ei - bi), dtype=np.uint8)
     native().amr_nesting_mask(pats.ctypes.data, len(pats), bi, bj, ei, ej, int(L.nxl), int(L.nyl), ok.ctypes.data)
     return ok.view(bool)
+
+
+CANVAS_MAX_CELLS = 1 << 27      # 1 GiB of doubles: larger levels (their fine levels come from fixed boxes and are cached) are packed
+
+
+def _tiles_needed(L, T):
+    pats = np.ascontiguousarray(L.patches, dtype=np.int32)
+    lo_i = np.maximum(pats[:, 0] - 2, 0) // T; hi_i = np.minimum(pats[:, 0] + pats[:, 2] + 1, L.nxl - 1) // T
+    lo_j = np.maximum(pats[:, 1] - 2, 0) // T; hi_j = np.minimum(pats[:, 1] + pats[:, 3] + 1, L.nyl - 1) // T
+    need = set()
+    for a0, a1, c0, c1 in set(zip(lo_i.tolist(), hi_i.tolist(), lo_j.tolist(), hi_j.tolist())):
+        for tj in range(c0, c1 + 1):
+            for ti in range(a0, a1 + 1):
+                need.add((ti, tj))
+    return need
+
+
+def set_bathy_from_canvas(L, wl):
+    """b of every patch of L from a canvas over the whole level that lives with the backend (device memory for the CUDA path):
+    the tiles the patches touch are evaluated and put on the canvas once, then one set_global gathers every storage cell inside the
+    level.  Same values as wl.bathy_box patch by patch: a cell's value does not depend on who asks."""
+    T = wl.TILE
+    store = wl.__dict__.setdefault("_canvas", {})
+    key = (id(L.ctx), L.dx, L.dy, int(L.nxl), int(L.nyl))
+    if key not in store:
+        store[key] = (L.ctx, L.ctx.canvas_new(L.nyl, L.nxl), set())
+    _, canvas, have = store[key]
+    for ti, tj in _tiles_needed(L, T) - have:
+        t = wl.bathy_tile(L.dx, L.dy, ti, tj)
+        h, w = min(T, int(L.nyl) - tj * T), min(T, int(L.nxl) - ti * T)
+        L.ctx.canvas_put(canvas, tj * T, ti * T, t[:h, :w])
+        have.add((ti, tj))
+    L.set_global("b", canvas)
 
 
 def pack_bathy_native(L, wl):

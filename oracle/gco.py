@@ -307,6 +307,13 @@ class Context:
     def level_create(self, level, xlo, ylo, dx, dy, nxl, nyl, ratio, patches):
         return Level(self, level, xlo, ylo, dx, dy, nxl, nyl, ratio, patches)
 
+    # the harness's bathymetry canvas (an array over a whole level, filled tile by tile, handed to set_global): host memory here
+    def canvas_new(self, ny, nx):
+        return np.zeros((int(ny), int(nx)))
+
+    def canvas_put(self, canvas, j0, i0, block):
+        canvas[j0:j0 + block.shape[0], i0:i0 + block.shape[1]] = block
+
     def destroy(self):
         if self.h:
             lib().gco_ctx_destroy(self.h); self.h = None

@@ -295,6 +295,15 @@ class Context:
         for key, value in DEFAULT_OPTIONS.items():
             self.set_option(key, value)
 
+    # a device-resident array over a whole level that the harness fills tile by tile and hands to set_global (bathymetry canvas)
+    def canvas_new(self, ny, nx):
+        with self.torch.cuda.stream(self.stream):
+            return self.torch.zeros((int(ny), int(nx)), dtype=self.torch.float64, device=self.device)
+
+    def canvas_put(self, canvas, j0, i0, block):
+        with self.torch.cuda.stream(self.stream):
+            canvas[j0:j0 + block.shape[0], i0:i0 + block.shape[1]].copy_(self.torch.from_numpy(np.ascontiguousarray(block)))
+
     def set_option(self, key, value):
         """gc_ctx_set_option: tuning knobs that change no result bit (OPT_SWEEP_FAMILY, OPT_MARCH_SEG); read at level creation."""
         self._chk(lib().gc_ctx_set_option(self.h, int(key), C.c_int64(int(value))), "gc_ctx_set_option")
