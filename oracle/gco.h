@@ -85,6 +85,10 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
                     double *ho, double *po, double *to, double *fm, double *fp,
                     int count_cfl, double *sdx);
 
+void gco_line_terms(const gco_params *P, int n, const double *h, const double *p, const double *t,
+                    const double *b, const double *rdx, const double *efac, double dt,
+                    double *am, double *ap, double *F, double *s);
+
 /* ---- level API (gco_level.c / gco_amr.c); mirrors include/gc.h with host pointers ---- */
 int gco_ctx_create(const gco_params *, gco_ctx **out);
 int gco_ctx_destroy(gco_ctx *);

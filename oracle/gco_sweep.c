@@ -15,19 +15,18 @@
 static double max2(double a, double b) { return a > b ? a : b; }
 static double min2(double a, double b) { return a < b ? a : b; }
 
-void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p, const double *t,
+/* steps (1)-(5) on one line: fluctuations am = A-dQ, ap = A+dQ and limited correction flux F at edges 2..n+2 (3 doubles each,
+ * index [e*3+k]), speeds s at edges 1..n+3.  Shared by the dimensionally split sweep below and the unsplit step (gco_unsplit.c). */
+void gco_line_terms(const gco_params *P, int n, const double *h, const double *p, const double *t,
                     const double *b, const double *rdx, const double *efac, double dt,
-                    double *ho, double *po, double *to, double *fm_out, double *fp_out,
-                    int count_cfl, double *sdx)
+                    double *am_out, double *ap_out, double *F_out, double *s_out)
 {
     int ne = n + 4; /* edge index e = 1..n+3 used */
     double (*Z)[3][3] = malloc(sizeof(double[3][3]) * ne);
     double (*s)[3] = malloc(sizeof(double[3]) * ne);
     double (*am)[3] = malloc(sizeof(double[3]) * ne);
     double (*ap)[3] = malloc(sizeof(double[3]) * ne);
-    double (*fm)[3] = malloc(sizeof(double[3]) * ne);
-    double (*fp)[3] = malloc(sizeof(double[3]) * ne);
-    int e, c, w, k;
+    int e, w, k;
 
     /* (1)-(3): Riemann problems, edge scaling, fluctuations (eq. 5-6; tie S-4) */
     for (e = 1; e <= n + 3; e++) {
@@ -49,7 +48,7 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
         }
     }
 
-    /* (4)-(6): limited second-order correction at edges 2..n+2 */
+    /* (4)-(5): limited second-order correction at edges 2..n+2 */
     for (e = 2; e <= n + 2; e++) {
         double F[3] = {0.0, 0.0, 0.0};
         double T[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
@@ -73,11 +72,30 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
             }
             for (k = 0; k < 3; k++) F[k] = (T[0][k] + T[2][k]) + T[1][k];
         }
-        for (k = 0; k < 3; k++) {
-            fm[e][k] = F[k] + am[e][k];
-            fp[e][k] = F[k] - ap[e][k];
-        }
+        for (k = 0; k < 3; k++) { am_out[e * 3 + k] = am[e][k]; ap_out[e * 3 + k] = ap[e][k]; F_out[e * 3 + k] = F[k]; }
     }
+    for (e = 1; e <= n + 3; e++) for (w = 0; w < 3; w++) s_out[e * 3 + w] = s[e][w];
+    free(Z); free(s); free(am); free(ap);
+}
+
+void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p, const double *t,
+                    const double *b, const double *rdx, const double *efac, double dt,
+                    double *ho, double *po, double *to, double *fm_out, double *fp_out,
+                    int count_cfl, double *sdx)
+{
+    int ne = n + 4; /* edge index e = 1..n+3 used */
+    double *am = malloc(sizeof(double) * 3 * ne), *ap = malloc(sizeof(double) * 3 * ne), *F = malloc(sizeof(double) * 3 * ne);
+    double *s = malloc(sizeof(double) * 3 * ne);
+    double (*fm)[3] = malloc(sizeof(double[3]) * ne);
+    double (*fp)[3] = malloc(sizeof(double[3]) * ne);
+    int e, c, w, k;
+
+    gco_line_terms(P, n, h, p, t, b, rdx, efac, dt, am, ap, F, s);          /* (1)-(5) */
+    for (e = 2; e <= n + 2; e++)                                              /* (6) */
+        for (k = 0; k < 3; k++) {
+            fm[e][k] = F[e * 3 + k] + am[e * 3 + k];
+            fp[e][k] = F[e * 3 + k] - ap[e * 3 + k];
+        }
 
     /* (7) update of cells 2..n+1 */
     for (c = 2; c <= n + 1; c++) {
@@ -92,12 +110,12 @@ void gco_sweep_line(const gco_params *P, int n, const double *h, const double *p
         double m = *sdx;
         for (e = 2; e <= n + 2; e++)
             for (w = 0; w < 3; w++) {
-                m = max2(m, max2(s[e][w], 0.0) * rdx[e]);
-                m = max2(m, max2(-s[e][w], 0.0) * rdx[e - 1]);
+                m = max2(m, max2(s[e * 3 + w], 0.0) * rdx[e]);
+                m = max2(m, max2(-s[e * 3 + w], 0.0) * rdx[e - 1]);
             }
         *sdx = m;
     }
     if (fm_out) for (e = 2; e <= n + 2; e++) for (k = 0; k < 3; k++) fm_out[e * 3 + k] = fm[e][k];
     if (fp_out) for (e = 2; e <= n + 2; e++) for (k = 0; k < 3; k++) fp_out[e * 3 + k] = fp[e][k];
-    free(Z); free(s); free(am); free(ap); free(fm); free(fp);
+    free(am); free(ap); free(F); free(s); free(fm); free(fp);
 }
