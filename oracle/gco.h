@@ -109,6 +109,9 @@ int gco_level_get_global(const gco_level *, int field, int which, double *dst, i
 int gco_fill_ghost_b(gco_level *);
 int gco_fill_ghost(gco_level *L, const gco_level *coarser, double alpha);
 int gco_level_step(gco_level *L, double dt, gco_step_stats *out);
+/* ---- unsplit step with transverse Riemann solves (gco_unsplit.c); DESIGN.md 3.13 (reading S-21) ---- */
+void gco_transverse(double g, double eps, double h, double pn, double pt, const double a[3], double bm[3], double bp[3]);
+int gco_level_step_unsplit(gco_level *L, double dt, gco_step_stats *out);
 /* threads for gco_level_step's loop over patches (default 1; no result bit depends on it: patches are independent inside a step,
  * SURVEY 8(d) "patch-level omp parallel for"); used by bench.py's N-core baseline and by the long parity runs */
 int gco_set_threads(int n);

@@ -11,7 +11,7 @@ import subprocess
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-_SRC = ["gco_riemann.c", "gco_sweep.c", "gco_level.c", "gco_amr.c", "gco_flux.c", "gco_bathy.c"]
+_SRC = ["gco_riemann.c", "gco_sweep.c", "gco_level.c", "gco_amr.c", "gco_flux.c", "gco_bathy.c", "gco_unsplit.c"]
 _LIB = os.path.join(_DIR, "libgco.so")
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-Wall", "-shared", "-fPIC", "-fopenmp"]
 
@@ -155,6 +155,14 @@ def friction(dt, h, hu, hv, **kw):
     return a.value, b.value
 
 
+def transverse(g, eps, h, pn, pt, a):
+    """split of the vector a (target frame) by the target direction's Jacobian at (h, pn, pt) -> (bm, bp)"""
+    bm = np.zeros(3); bp = np.zeros(3); av = np.ascontiguousarray(a, dtype=np.float64)
+    f = lib().gco_transverse; f.restype = None; f.argtypes = [C.c_double] * 5 + [_dp, _dp, _dp]
+    f(g, eps, h, pn, pt, av.ctypes.data_as(_dp), bm.ctypes.data_as(_dp), bp.ctypes.data_as(_dp))
+    return bm, bp
+
+
 def riemann(g, eps, hL, pL, tL, bL, hR, pR, tR, bR):
     Z = np.zeros((3, 3)); s = np.zeros(3)
     lib().gco_riemann(g, eps, hL, pL, tL, bL, hR, pR, tR, bR, Z.ctypes.data_as(_dp), s.ctypes.data_as(_dp))
@@ -240,6 +248,14 @@ class Level:
     def step(self, dt):
         st = StepStats()
         _chk(lib().gco_level_step(self.h, dt, C.byref(st)), "level_step")
+        return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
+                    n_clipped=st.n_clipped, nan_seen=st.nan_seen)
+
+    def step_unsplit(self, dt):
+        """one unsplit level step with transverse Riemann solves"""
+        st = StepStats()
+        lib().gco_level_step_unsplit.argtypes = [C.c_void_p, C.c_double, C.c_void_p]
+        _chk(lib().gco_level_step_unsplit(self.h, dt, C.byref(st)), "level_step_unsplit")
         return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
                     n_clipped=st.n_clipped, nan_seen=st.nan_seen)
 
