@@ -174,6 +174,13 @@ int gc_level_step(gc_level *L, double dt, gc_step_stats *out);
  * capturable. */
 int gc_level_step_auto(gc_level *L, double *dt_dev, double cfl_target);
 int gc_level_stats(const gc_level *, gc_step_stats *out /*HOST*/);
+/* The same level step by the UNSPLIT wave-propagation method with transverse Riemann solves -- "the original GeoClaw ... with the
+ * unsplit algorithm" that the paper simplifies to dimensional splitting and validates against (DESIGN.md 3.13,
+ * reading S-21): every edge's fluctuations and limited correction flux from Q^n, each edge's vectors A-dQ + F~ and A+dQ - F~ split
+ * by the transverse Jacobian of the cell they enter into parts that modify the neighbouring edges' correction fluxes, one update.
+ * Same arguments, statistics and dt = 0 probe as gc_level_step.  Flux registers (gc_flux_attach) are defined for the split step
+ * only: GC_ERR_STATE on a level that has any.  First use allocates 18 planes of scratch (released with the level). */
+int gc_level_step_unsplit(gc_level *L, double dt, gc_step_stats *out);
 
 /* wet mask (h > dry_tol) of the current state: one byte per interior cell, patch after patch, row-major. */
 int gc_wet_mask(const gc_level *, uint8_t *mask, int is_device);

@@ -18,7 +18,7 @@ SYMBOLS = [
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
-    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update", "gc_level_fallback_counts",
+    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update", "gc_level_fallback_counts", "gc_level_step_unsplit",
 ]
 
 
@@ -81,6 +81,7 @@ def lib():
     L.gc_gauges_sample.argtypes = [vp, vp, i]
     L.gc_level_step.argtypes = [vp, d, vp]
     L.gc_level_step_auto.argtypes = [vp, vp, d]
+    L.gc_level_step_unsplit.argtypes = [vp, d, vp]
     L.gc_level_stats.argtypes = [vp, vp]
     L.gc_wet_mask.argtypes = [vp, vp, i]
     L.gc_level_mass.argtypes = [vp]; L.gc_level_mass.restype = d
@@ -174,6 +175,13 @@ class Level:
             return None
         st = StepStats()
         self.ctx._chk(lib().gc_level_step(self.h, dt, C.byref(st)), "gc_level_step")
+        return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
+                    n_clipped=st.n_clipped, nan_seen=st.nan_seen)
+
+    def step_unsplit(self, dt):
+        """gc_level_step_unsplit: one unsplit level step with transverse Riemann solves"""
+        st = StepStats()
+        self.ctx._chk(lib().gc_level_step_unsplit(self.h, dt, C.byref(st)), "gc_level_step_unsplit")
         return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
                     n_clipped=st.n_clipped, nan_seen=st.nan_seen)
 

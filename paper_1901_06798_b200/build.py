@@ -10,7 +10,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = ["gc_api.cu", "gc_api_amr.cu", "gc_sweep.cu", "gc_ghost.cu", "gc_amr.cu"]
+SRC = ["gc_api.cu", "gc_api_amr.cu", "gc_sweep.cu", "gc_ghost.cu", "gc_amr.cu", "gc_unsplit.cu"]
 LIB = os.path.join(HERE, "libgeoclaw_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared"]

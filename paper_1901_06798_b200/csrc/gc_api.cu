@@ -629,6 +629,25 @@ extern "C" int gc_level_step(gc_level *L, double dt, gc_step_stats *out)
     return GC_OK;
 }
 
+extern "C" int gc_level_step_unsplit(gc_level *L, double dt, gc_step_stats *out)
+{
+    if (!L || !(dt >= 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step_unsplit: bad argument");
+    if (L->reg_fine || L->reg_coarse) return gc_fail(L->ctx, GC_ERR_STATE, "gc_level_step_unsplit: flux registers are defined for the split step only");
+    gc_launch_stats_reset(L);
+    int rc = gc_launch_unsplit(L, dt, dt > 0.0 ? 1 : 0);
+    if (rc) return gc_fail(L->ctx, rc, "gc_level_step_unsplit: scratch allocation failed");
+    if (dt > 0.0) L->cur = 1 - L->cur;
+    rc = gc_cuda_check(L->ctx, "gc_level_step_unsplit");
+    if (rc) return rc;
+    if (out) {
+        rc = gc_level_stats(L, out);
+        if (rc) return rc;
+        out->cfl_max = dt * out->s_over_dx_max;
+        if (out->nan_seen) return gc_fail(L->ctx, GC_ERR_NAN, "gc_level_step_unsplit: NaN in the updated state");
+    }
+    return GC_OK;
+}
+
 extern "C" int gc_level_step_auto(gc_level *L, double *dt_dev, double cfl_target)
 {
     if (!L || !dt_dev || !(cfl_target > 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step_auto: bad argument");

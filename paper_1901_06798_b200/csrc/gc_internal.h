@@ -151,6 +151,7 @@ struct gc_level {
     uint64_t avg_gen; AvgRect *d_avg; int64_t *d_avgstart; int navg; int64_t navgcells;
     int nbr_buffer; int32_t *d_nbrstart, *d_nbrlist;
     int64_t *d_goff = nullptr; int64_t gtot = 0;      // packed offsets of gc_level_set_patches (built at first use)
+    double *d_uns = nullptr;                         // scratch of the unsplit step: 18 planes (gc_unsplit.cu)
     GaugeLoc *d_gauge = nullptr; int ngauge = 0;     // gauges bound to this level (gc_gauges_bind)
     // asynchronous whole-level state transfer (gc_level_upload_state_async / gc_level_download_state_async): staging planes of
     // nxl * nyl doubles per field and direction, events that order the copy stream against the context's stream
@@ -177,6 +178,8 @@ void gc_launch_stats_reset(gc_level *L);
 void gc_launch_next_dt(gc_level *L, double *dt_dev, double cfl_target);
 void gc_launch_math_selftest(cudaStream_t s, const double *a, const double *b, int64_t n, unsigned long long *out);
 void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, int threads);
+// gc_unsplit.cu
+int gc_launch_unsplit(gc_level *L, double dt, int write_out);
 // gc_ghost.cu
 void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);
 void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int is_state);

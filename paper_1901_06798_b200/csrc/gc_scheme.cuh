@@ -53,13 +53,14 @@ __device__ __forceinline__ double gc_mc(M &m, double zi, double zz)
     return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));  // MC; fma(.5, t, .5) = .5 (1 + t) bit for bit
 }
 
-// (3)-(6) for edge e.  dlo[w] = Z_{e-1}^w . Z_e^w, dhi[w] = Z_{e+1}^w . Z_e^w (eq. 11: I = e-1 if s > 0, e+1 if s < 0).
+// (3)-(5) for edge e: fluctuations am = A-dQ, ap = A+dQ and limited correction flux F.  dlo[w] = Z_{e-1}^w . Z_e^w, dhi[w] = Z_{e+1}^w . Z_e^w (eq. 11: I = e-1 if s > 0, e+1 if s < 0).
 // rdL, rdR = 1/(kappa dx) of the left / right cell.
 template <class M>
-__device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
-                                             double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
+__device__ __forceinline__ void gc_edge_terms(M &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
+                                              double dt, double rdL, double rdR, double (&am)[3], double (&ap)[3], double (&F)[3])
 {
-    double am[3] = {0.0, 0.0, 0.0}, ap[3] = {0.0, 0.0, 0.0}, F[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int c = 0; c < 3; c++) { am[c] = 0.0; ap[c] = 0.0; F[c] = 0.0; }
     double T[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
 #pragma unroll
     for (int w = 0; w < 3; w++) {
@@ -87,6 +88,14 @@ __device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double 
 #pragma unroll
         for (int c = 0; c < 3; c++) F[c] = (T[0][c] + T[2][c]) + T[1][c];             // outer families first: mirror-symmetric
     }
+}
+// (3)-(6): fm = F~ + A-dQ, fp = F~ - A+dQ
+template <class M>
+__device__ __forceinline__ void gc_edge_flux(M &m, const Waves &W, const double (&dlo)[3], const double (&dhi)[3], int limiter,
+                                             double dt, double rdL, double rdR, double (&fm)[3], double (&fp)[3])
+{
+    double am[3], ap[3], F[3];
+    gc_edge_terms(m, W, dlo, dhi, limiter, dt, rdL, rdR, am, ap, F);
 #pragma unroll
     for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
 }
