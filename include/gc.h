@@ -67,7 +67,8 @@ typedef struct {
 typedef struct {
     double cfl_max;       /* nu = dt * s_over_dx_max (eq. 15) */
     double s_over_dx_max; /* max over both sweeps, all patches, interior lines, of |s| / (kappa dx) */
-    double clipped_mass;  /* sum over interior cells of (-h) * area for cells with h < 0 set to 0 by the clean-up */
+    double clipped_mass;  /* sum over interior cells of (-h) * area for cells with h < 0 set to 0 by the clean-up; accumulated with
+                             floating-point atomics, so its last bits depend on the order (every other statistic and the state do not) */
     int64_t n_clipped;    /* number of such cells */
     int32_t nan_seen;     /* 1 if any updated value is NaN */
 } gc_step_stats;
