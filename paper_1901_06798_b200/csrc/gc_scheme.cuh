@@ -124,12 +124,11 @@ __device__ __forceinline__ double gc_mc_fast(double theta)
 {
     return dmax(0.0, dmin(dmin(__fma_rn(0.5, theta, 0.5), 2.0), 2.0 * theta));                      // MC
 }
-__device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&dlo)[3], const double (&dhi)[3],
-                                                 double dtdx_ave, double (&fm)[3], double (&fp)[3])
+__device__ __forceinline__ bool gc_edge_terms_std(const Waves &W, const double (&dlo)[3], const double (&dhi)[3],
+                                                  double dtdx_ave, double (&am)[3], double (&ap)[3], double (&F)[3])
 {
     const double s0 = W.s[0], s1 = W.s[1], s2 = W.s[2];
     const bool neg1 = s1 < 0.0, pos1 = s1 > 0.0;
-    double am[3], ap[3];
     am[0] = 0.0 + W.Z[0][0];
     ap[0] = 0.0 + W.Z[2][0];
 #pragma unroll
@@ -159,9 +158,18 @@ __device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const double t1 = c1 * W.Z[1][c];
-        const double F = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + (on1 ? t1 : 0.0);                       // eq. 9, outer families first
-        fm[c] = F + am[c]; fp[c] = F - ap[c];
+        F[c] = (c0 * W.Z[0][c] + c2 * W.Z[2][c]) + (on1 ? t1 : 0.0);                                 // eq. 9, outer families first
     }
+    return ok;
+}
+// (6) on top of it: fm = F~ + A-dQ, fp = F~ - A+dQ
+__device__ __forceinline__ bool gc_edge_flux_std(const Waves &W, const double (&dlo)[3], const double (&dhi)[3],
+                                                 double dtdx_ave, double (&fm)[3], double (&fp)[3])
+{
+    double am[3], ap[3], F[3];
+    const bool ok = gc_edge_terms_std(W, dlo, dhi, dtdx_ave, am, ap, F);
+#pragma unroll
+    for (int c = 0; c < 3; c++) { fm[c] = F[c] + am[c]; fp[c] = F[c] - ap[c]; }
     return ok;
 }
 

@@ -1,16 +1,27 @@
 // gc_unsplit.cu -- the unsplit wave-propagation step with transverse Riemann solves.
 //
 // P:309 and P:371 name it ("the original GeoClaw ... with the unsplit algorithm"); the paper's GPU code simplifies it to
-// dimensional splitting.  DESIGN.md 3.13 (reading S-21) fixes the formulas.  Two kernels per step, both reading Q^n only:
-//   k_uns_edges<DIR>  thread <-> edge: fluctuations A-dQ, A+dQ and limited correction flux F~ of every x-edge of rows 1..ny+2
-//                     (every y-edge of columns 1..nx+2), by the device functions of the split sweeps (three Riemann problems per
-//                     edge for the limiter: redundant, simple), stored per edge; eq. 15 over interior lines
-//   k_uns_update      thread <-> interior cell: the transverse splits that reach the cell's four edges (16 per cell, in the
-//                     order DESIGN.md 3.13 fixes), the modified correction fluxes, the update, clean-up, friction
-// A first correct version of a "next" row: every expression in the order of the specification (bit-identical to the oracle,
-// tests/test_gpu_unsplit.py); it stores 18 doubles per cell between the two kernels and is not tuned.
+// dimensional splitting.  DESIGN.md 3.13 (reading S-21) fixes the formulas.  Three kernels per step, all reading Q^n only:
+//   k_uns_xedges  thread <-> x-edge: fluctuations A-dQ, A+dQ and limited correction flux F~ of the edges e = 2..nx+2 of rows
+//                 1..ny+2.  The solved edges of a patch (e = 1..nx+3 of every row) form one flat sequence; a block takes windows of
+//                 128 consecutive ones, 126 apart, hands the waves to the neighbours through shared memory (double-buffered: one
+//                 barrier per window) and finishes the 126 in the middle.  Coalesced; 1.03 Riemann problems per edge.
+//   k_uns_yedges  thread <-> column segment (32 y-edges of one of the columns 1..nx+2), lanes <-> consecutive columns, marching
+//                 upwards with the last two wave sets in registers: coalesced, no barrier, 1.06 Riemann problems per edge.
+//                 Both store (A-dQ, A+dQ, F~) per edge: 18 doubles per cell; eq. 15 over the edges of interior lines.
+//   k_uns_update  thread <-> column segment of interior cells, lanes <-> consecutive columns (30 updating + 1 halo lane each
+//                 side), marching upwards.  Row r: the four transverse splits of cell r (a+ of its left and a- of
+//                 its right x-edge by the y-Jacobian, b+ of its lower and b- of its upper y-edge by the x-Jacobian, each computed
+//                 ONCE -- the Jacobian's 1/h, sqrt(g h), 1/(l3 - l1) once per cell and direction); the up-going parts wait one row
+//                 in registers, the right- and left-going parts reach the neighbour columns by warp shuffles; G~' of the lower
+//                 edge, F~' of the left edge (the right one from the next lane), then the update of cell r-1, clean-up, friction.
+// Every expression in the order of the specification (bit-identical to the oracle, tests/test_gpu_unsplit.py).
 #include "gc_internal.h"
 #include "gc_scheme.cuh"
+
+#define UNS_SEG 32          // edges / cells per marching segment
+#define UNS_WIN 126         // finished x-edges per window of 128 solved ones
+#define UNS_WPB 8           // windows per block of k_uns_xedges
 
 struct UnsArgs {
     const PatchDesc *pat;
@@ -33,12 +44,14 @@ __device__ __forceinline__ RState uns_cell(const UnsArgs &a, int64_t o, int dir)
     return S;
 }
 
-// solve one edge: the guarded open-ocean code where it applies, else the general code (same bits where both apply)
-__device__ __forceinline__ void uns_solve(const UnsArgs &a, const RState &L0, const RState &R0, double ef, Waves &W)
+// solve one edge: the guarded open-ocean code where it applies, else the general code (same bits where both apply).
+// Returns true for a "standard" edge (guarded code: s[0] < 0 < s[2]), which the control-flow-free gc_edge_terms_std may finish.
+__device__ __forceinline__ bool uns_solve(const UnsArgs &a, const RState &L0, const RState &R0, double ef, Waves &W)
 {
     RState L = L0, R = R0;
-    const bool okL = gc_prim_fast(L, a.g, 0.5 * a.g, a.eps > 0x1p-100 ? a.eps : 0x1p-100);
-    const bool okR = gc_prim_fast(R, a.g, 0.5 * a.g, a.eps > 0x1p-100 ? a.eps : 0x1p-100);
+    const double hlo = a.eps > 0x1p-100 ? a.eps : 0x1p-100;
+    const bool okL = gc_prim_fast(L, a.g, 0.5 * a.g, hlo);
+    const bool okR = gc_prim_fast(R, a.g, 0.5 * a.g, hlo);
     const bool ok = gc_riemann_fast(a.g, L, R, W.Z, W.s) & okL & okR & (a.g >= 0x1p-20) & (a.g <= 0x1p20);
     if (!ok) {
         MathIeee mi;
@@ -50,71 +63,171 @@ __device__ __forceinline__ void uns_solve(const UnsArgs &a, const RState &L0, co
 #pragma unroll
         for (int w = 0; w < 3; w++) { W.s[w] = W.s[w] * ef; W.Z[w][0] = W.Z[w][0] * ef; W.Z[w][1] = W.Z[w][1] * ef; W.Z[w][2] = W.Z[w][2] * ef; }
     }
+    return ok;
 }
 
-// grid = patches x chunks of 4096 edges.  DIR 0: edge (j, e), j = 1..ny+2, e = 2..nx+2; DIR 1: edge (e, i), i = 1..nx+2, e = 2..ny+2
-template <int DIR>
-__global__ void __launch_bounds__(128) k_uns_edges(UnsArgs a)
+// (3)-(5) of one edge and its three planes of each kind, at offset o of plane set T
+__device__ __forceinline__ void uns_finish(const UnsArgs &a, const Waves &We, bool stdE, const double (&dlo)[3], const double (&dhi)[3],
+                                           double rdL, double rdR, double *T)
 {
-    const PatchDesc pd = a.pat[blockIdx.x];
-    const int nl = (DIR == 0 ? pd.ny : pd.nx) + 2;            // lines
-    const int ne = (DIR == 0 ? pd.nx : pd.ny) + 1;            // edges per line
-    const int n = nl * ne;
-    double cfl = 0.0;
-    for (int t = blockIdx.y * 4096 + threadIdx.x; t < min(n, (int)(blockIdx.y + 1) * 4096); t += blockDim.x) {
-        int line, e;
-        if (DIR == 0) { line = 1 + t / ne; e = 2 + t % ne; } else { e = 2 + t / nl; line = 1 + t % nl; }   // x: e fastest; y: column fastest
-        const int64_t str = DIR == 0 ? 1 : pd.pitch;
-        const int64_t o = DIR == 0 ? pd.off + (int64_t)line * pd.pitch + e : pd.off + (int64_t)e * pd.pitch + line;
-        const RState c0 = uns_cell(a, o - 2 * str, DIR), c1 = uns_cell(a, o - str, DIR), c2 = uns_cell(a, o, DIR), c3 = uns_cell(a, o + str, DIR);
-        double ef0, ef1, ef2, rdL, rdR;
-        if (DIR == 0) { ef0 = ef1 = ef2 = a.ex; rdL = rdR = a.rdx[pd.j0 + line]; }
-        else { ef0 = a.ey[pd.j0 + e - 1]; ef1 = a.ey[pd.j0 + e]; ef2 = a.ey[pd.j0 + e + 1]; rdL = a.rdy[pd.j0 + e - 1]; rdR = a.rdy[pd.j0 + e]; }
-        Waves Wl, We, Wh;
-        uns_solve(a, c0, c1, ef0, Wl); uns_solve(a, c1, c2, ef1, We); uns_solve(a, c2, c3, ef2, Wh);
-        double dlo[3], dhi[3], am[3], ap[3], F[3];
-        gc_wave_dots(We, Wl, dlo);
-        gc_wave_dots(Wh, We, dhi);
-        MathIeee mi;
-        gc_edge_terms(mi, We, dlo, dhi, a.limiter, a.dt, rdL, rdR, am, ap, F);
-        double *T = a.T + (int64_t)(DIR == 0 ? 0 : 9) * a.tot + o;
+    double am[3], ap[3], F[3];
+    bool done = false;
+    if (stdE && a.limiter != 0) done = gc_edge_terms_std(We, dlo, dhi, 0.5 * __fma_rn(a.dt, rdL, a.dt * rdR), am, ap, F);
+    if (!done) { MathIeee mi; gc_edge_terms(mi, We, dlo, dhi, a.limiter, a.dt, rdL, rdR, am, ap, F); }
 #pragma unroll
-        for (int k = 0; k < 3; k++) { T[(int64_t)k * a.tot] = am[k]; T[(int64_t)(3 + k) * a.tot] = ap[k]; T[(int64_t)(6 + k) * a.tot] = F[k]; }
-        const bool interior = DIR == 0 ? (line >= 2 && line < pd.ny + 2) : (line >= 2 && line < pd.nx + 2);
-        if (interior) cfl = dmax(cfl, gc_edge_cfl(We, rdL, rdR));
-    }
+    for (int k = 0; k < 3; k++) { T[(int64_t)k * a.tot] = am[k]; T[(int64_t)(3 + k) * a.tot] = ap[k]; T[(int64_t)(6 + k) * a.tot] = F[k]; }
+}
+
+__device__ __forceinline__ void uns_cfl_out(const UnsArgs &a, double cfl)
+{
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) cfl = dmax(cfl, __longlong_as_double(__shfl_xor_sync(0xffffffffu, __double_as_longlong(cfl), s)));
     if ((threadIdx.x & 31) == 0 && cfl > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(cfl));
 }
 
-// split of a (target frame: depth, momentum along the target direction, momentum across it) by the target
-// direction's Jacobian at the cell state (h, pn, pt); IEEE operators, the specification's order
-__device__ __forceinline__ void gc_transverse(double g, double eps, double h, double pn, double pt, const double (&a)[3],
-                                              double (&bm)[3], double (&bp)[3])
+// grid = patches x groups of UNS_WPB windows.  Flat index t of a solved edge: row 1 + t / (nx+3), edge e = 1 + t % (nx+3).
+__global__ void __launch_bounds__(128) k_uns_xedges(UnsArgs a)
 {
-#pragma unroll
-    for (int k = 0; k < 3; k++) { bm[k] = 0.0; bp[k] = 0.0; }
-    if (!(h > eps)) return;
-    const double rh = 1.0 / h;
-    const double w = pn * rh, z = pt * rh, c = sqrt(g * h);
-    const double l1 = w - c, l2 = w, l3 = w + c;
-    const double rho = 1.0 / (l3 - l1);
-    const double b1 = __fma_rn(l3, a[0], -a[1]) * rho;
-    const double b3 = __fma_rn(-l1, a[0], a[1]) * rho;
-    const double b2 = __fma_rn(-z, a[0], a[2]);
-    double lam[3] = { l1, l2, l3 };
-    double V[3][3];
-    V[0][0] = l1 * b1; V[0][1] = V[0][0] * l1; V[0][2] = V[0][0] * z;
-    V[1][0] = 0.0;     V[1][1] = 0.0;          V[1][2] = l2 * b2;
-    V[2][0] = l3 * b3; V[2][1] = V[2][0] * l3; V[2][2] = V[2][0] * z;
-#pragma unroll
-    for (int p = 0; p < 3; p++)
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
-            if (lam[p] < 0.0) bm[k] = bm[k] + V[p][k];
-            else if (lam[p] > 0.0) bp[k] = bp[k] + V[p][k];
+    __shared__ double sZ[2][9][128];
+    const PatchDesc pd = a.pat[blockIdx.x];
+    const int k = threadIdx.x;
+    const int ne2 = pd.nx + 3, nflat = (pd.ny + 2) * ne2;
+    const int nwin = (nflat + UNS_WIN - 1) / UNS_WIN;
+    const int w0 = blockIdx.y * UNS_WPB, w1 = min(nwin, w0 + UNS_WPB);
+    double cfl = 0.0;
+    // where thread k stands in window w; a thread outside the sequence loads the patch's first edge and solves nothing
+    auto locate = [&](int w, int &line, int &e, int64_t &o) -> bool {
+        const int t = UNS_WIN * w - 1 + k;
+        const bool act = t >= 0 && t < nflat;
+        line = act ? 1 + t / ne2 : 1;
+        e = act ? 1 + (t - (line - 1) * ne2) : 1;
+        o = pd.off + (int64_t)line * pd.pitch + e;
+        return act;
+    };
+    int line, e; int64_t o;
+    bool active = locate(w0, line, e, o);
+    RState cL = uns_cell(a, o - 1, 0), cR = uns_cell(a, o, 0);
+    for (int w = w0; w < w1; w++) {
+        const int buf = w & 1;
+        int line2 = line, e2 = e; int64_t o2 = o; bool act2 = false;
+        RState nL = cL, nR = cR;
+        if (w + 1 < w1) {                                       // the next window's cells, loaded a window ahead of their use
+            act2 = locate(w + 1, line2, e2, o2);
+            nL = uns_cell(a, o2 - 1, 0); nR = uns_cell(a, o2, 0);
         }
+        Waves We;
+        bool stdE = false;
+        if (active) stdE = uns_solve(a, cL, cR, a.ex, We);
+        else gc_waves_zero(We);
+#pragma unroll
+        for (int q = 0; q < 3; q++) { sZ[buf][3 * q][k] = We.Z[q][0]; sZ[buf][3 * q + 1][k] = We.Z[q][1]; sZ[buf][3 * q + 2][k] = We.Z[q][2]; }
+        __syncthreads();
+        if (active && k >= 1 && k <= UNS_WIN && e >= 2 && e <= pd.nx + 2) {
+            double dlo[3], dhi[3];
+#pragma unroll
+            for (int q = 0; q < 3; q++) {                      // gc_wave_dots with the neighbour's waves read from shared memory
+                dlo[q] = __fma_rn(We.Z[q][2], sZ[buf][3 * q + 2][k - 1], __fma_rn(We.Z[q][1], sZ[buf][3 * q + 1][k - 1], We.Z[q][0] * sZ[buf][3 * q][k - 1]));
+                dhi[q] = __fma_rn(sZ[buf][3 * q + 2][k + 1], We.Z[q][2], __fma_rn(sZ[buf][3 * q + 1][k + 1], We.Z[q][1], sZ[buf][3 * q][k + 1] * We.Z[q][0]));
+            }
+            const double rd = a.rdx[pd.j0 + line];
+            uns_finish(a, We, stdE, dlo, dhi, rd, rd, a.T + o);
+            if (line >= 2 && line < pd.ny + 2) cfl = dmax(cfl, gc_edge_cfl(We, rd, rd));
+        }
+        active = act2; line = line2; e = e2; o = o2; cL = nL; cR = nR;
+    }
+    uns_cfl_out(a, cfl);
+}
+
+// grid = patches x groups of 4 tasks (one per warp); task = (32 columns of 1..nx+2) x (UNS_SEG edges of e = 2..ny+2)
+__global__ void __launch_bounds__(128) k_uns_yedges(UnsArgs a)
+{
+    const PatchDesc pd = a.pat[blockIdx.x];
+    const int lane = threadIdx.x & 31;
+    const int ncw = (pd.nx + 2 + 31) / 32, nsg = (pd.ny + 1 + UNS_SEG - 1) / UNS_SEG;
+    const int task = blockIdx.y * 4 + (threadIdx.x >> 5);
+    if (task >= ncw * nsg) return;
+    const int cw = task % ncw, sg = task / ncw;
+    const int col0 = 1 + cw * 32 + lane;
+    const bool valid = col0 <= pd.nx + 2;
+    const int col = valid ? col0 : pd.nx + 2;                   // lanes past the patch repeat its last column and store nothing
+    const int ea = 2 + sg * UNS_SEG, eb = min(ea + UNS_SEG, pd.ny + 3);
+    const bool counted = valid && col >= 2 && col < pd.nx + 2;
+    int64_t o = pd.off + (int64_t)(ea - 2) * pd.pitch + col;
+    RState cprev = uns_cell(a, o, 1);
+    RState cnext = uns_cell(a, o + pd.pitch, 1);               // loaded one iteration ahead of its use
+    Waves Wc;
+    gc_waves_zero(Wc);
+    double dlo[3] = {0.0, 0.0, 0.0};
+    bool stdc = false;
+    double cfl = 0.0;
+    for (int m = ea - 1; m <= eb; m++) {                        // solves edge m (cells m-1 | m); finishes edge m-1
+        o += pd.pitch;
+        const RState cnew = cnext;
+        if (m < eb) cnext = uns_cell(a, o + pd.pitch, 1);
+        Waves Wn;
+        const bool stdn = uns_solve(a, cprev, cnew, a.ey[pd.j0 + m], Wn);
+        double dhi[3];
+        gc_wave_dots(Wn, Wc, dhi);
+        if (m >= ea + 1) {
+            const double rdL = a.rdy[pd.j0 + m - 2], rdR = a.rdy[pd.j0 + m - 1];
+            if (valid) uns_finish(a, Wc, stdc, dlo, dhi, rdL, rdR, a.T + 9 * a.tot + (o - pd.pitch));
+            if (counted) cfl = dmax(cfl, gc_edge_cfl(Wc, rdL, rdR));
+        }
+        Wc = Wn; stdc = stdn; cprev = cnew;
+#pragma unroll
+        for (int q = 0; q < 3; q++) dlo[q] = dhi[q];
+    }
+    uns_cfl_out(a, cfl);
+}
+
+// the target direction's Jacobian at the cell state (h, pn, pt): what its split needs, once per cell and
+// direction; IEEE operators, the specification's order
+struct UnsJac { double l1, l2, l3, z, rho; bool n1, p1, n2, p2, n3, p3; };     // the sign flags are false in a dry cell
+// Both Jacobians of a cell (x: along hu, y: along hv) share 1/h and sqrt(g h).  FAST: the reciprocals and the root by the
+// unchecked correctly rounded sequences of gc_math.cuh; returns false if a wet cell has an operand outside their window (the
+// caller then calls the IEEE version: same bits wherever both apply).
+template <bool FAST>
+__device__ __forceinline__ bool uns_jac2(double g, double eps, double h, double hu, double hv, UnsJac &Jx, UnsJac &Jy)
+{
+    const bool wet = h > eps;
+    const double gh = g * h;
+    const double rh = FAST ? gc_frcp(h) : 1.0 / h;
+    const double c = FAST ? gc_fsqrt(gh) : sqrt(gh);
+    const double wx = hu * rh, wy = hv * rh;
+    Jx.z = wy; Jy.z = wx;
+    Jx.l1 = wx - c; Jx.l2 = wx; Jx.l3 = wx + c;
+    Jy.l1 = wy - c; Jy.l2 = wy; Jy.l3 = wy + c;
+    const double dx = Jx.l3 - Jx.l1, dy = Jy.l3 - Jy.l1;
+    Jx.rho = FAST ? gc_frcp(dx) : 1.0 / dx;
+    Jy.rho = FAST ? gc_frcp(dy) : 1.0 / dy;
+    Jx.n1 = wet & (Jx.l1 < 0.0); Jx.p1 = wet & (Jx.l1 > 0.0); Jx.n2 = wet & (Jx.l2 < 0.0); Jx.p2 = wet & (Jx.l2 > 0.0);
+    Jx.n3 = wet & (Jx.l3 < 0.0); Jx.p3 = wet & (Jx.l3 > 0.0);
+    Jy.n1 = wet & (Jy.l1 < 0.0); Jy.p1 = wet & (Jy.l1 > 0.0); Jy.n2 = wet & (Jy.l2 < 0.0); Jy.p2 = wet & (Jy.l2 > 0.0);
+    Jy.n3 = wet & (Jy.l3 < 0.0); Jy.p3 = wet & (Jy.l3 > 0.0);
+    return !wet | (gc_in_window(h) & gc_in_window(gh) & (gh > 0.0) & gc_in_window(dx) & gc_in_window(dy));
+}
+// split of a (target frame: depth, momentum along the target direction, momentum across it) into the parts travelling down
+// (bm) and up (bp) the target direction; a dry cell passes nothing on.  Written without control flow: the specification adds
+// family p's vector to bm if lambda_p < 0, to bp if lambda_p > 0, in the order p = 1, 2, 3, starting from +0.0; here a family
+// that does not take part (every family of a dry cell) is added as +0.0, which changes no bit (a partial sum that starts at +0.0 is never -0.0), and family
+// 2's vector (0, 0, l2 b2) is left out of components 0 and 1 for the same reason.  A dry cell's numbers (1/h of a tiny or zero
+// h) are computed and never selected.
+__device__ __forceinline__ void uns_split(const UnsJac &J, const double (&a)[3], double (&bm)[3], double (&bp)[3])
+{
+    const double b1 = __fma_rn(J.l3, a[0], -a[1]) * J.rho;
+    const double b3 = __fma_rn(-J.l1, a[0], a[1]) * J.rho;
+    const double b2 = __fma_rn(-J.z, a[0], a[2]);
+    double V0[3], V2[3];
+    V0[0] = J.l1 * b1; V0[1] = V0[0] * J.l1; V0[2] = V0[0] * J.z;
+    V2[0] = J.l3 * b3; V2[1] = V2[0] * J.l3; V2[2] = V2[0] * J.z;
+    const double V12 = J.l2 * b2;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        double m = 0.0 + (J.n1 ? V0[k] : 0.0), q = 0.0 + (J.p1 ? V0[k] : 0.0);
+        if (k == 2) { m = m + (J.n2 ? V12 : 0.0); q = q + (J.p2 ? V12 : 0.0); }
+        m = m + (J.n3 ? V2[k] : 0.0); q = q + (J.p3 ? V2[k] : 0.0);
+        bm[k] = m; bp[k] = q;
+    }
 }
 
 // the vector an edge sends into one of its two cells: part 0: a- = A-dQ + F~ (cell on the low side), part 1: a+ = A+dQ - F~,
@@ -128,96 +241,149 @@ __device__ __forceinline__ void uns_vec(const double *T, int64_t tot, int64_t o,
     at[0] = a[0]; at[1] = a[2]; at[2] = a[1];
 }
 
-// G~' of the y-edge at the lower side of cell (row e, column i) [offset o]: G~, then the up-going parts from row e-1, then the
-// down-going parts from row e, each row's x-edges in the order (a+ of the cell's left edge, a- of its right edge)
-__device__ __forceinline__ void uns_G2(const UnsArgs &a, const PatchDesc &pd, int64_t o, int e, double (&G2)[3])
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// ---- k_uns_update -------------------------------------------------------------------------------------------------
+// What a lane needs of row r sits in 21 planes at its own cell: h, hu, hv, and (A-dQ, A+dQ, F~) of the cell's left x-edge and
+// lower y-edge.  Rows are staged two ahead of their use in a ring of three, 8 bytes per lane and plane by cp.async (each warp
+// its own ring: 3 x 21 x 256 bytes), so that the march never waits for memory; the right x-edge's values are the next lane's.
+#define UNS_UPD_WARPS 2
+#define UNS_NPL 21
+#define UNS_RING_DOUBLES (3 * UNS_NPL * 32)
+__device__ __forceinline__ void uns_cpa8(unsigned sdst, const double *gsrc)
 {
-    const double *Tx = a.T, *Ty = a.T + 9 * a.tot;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void uns_stage_row(const UnsArgs &a, int64_t o, unsigned sdst)
+{
+    uns_cpa8(sdst, a.h + o); uns_cpa8(sdst + 256u, a.hu + o); uns_cpa8(sdst + 512u, a.hv + o);
+    const double *T = a.T + o;
 #pragma unroll
-    for (int k = 0; k < 3; k++) G2[k] = Ty[(int64_t)(6 + k) * a.tot + o];
-#pragma unroll
-    for (int r = 0; r < 2; r++) {                               // r = 0: row e-1 (its bp), r = 1: row e (its bm)
-        const int j = e - 1 + r;
-        const int64_t c = o - (int64_t)(1 - r) * pd.pitch;      // the cell of that row in this column
-        const double half = 0.5 * (a.dt * a.rdx[pd.j0 + j]);
-        const double h = a.h[c], pn = a.hv[c], pt = a.hu[c];
-#pragma unroll
-        for (int q = 0; q < 2; q++) {                           // q = 0: a+ of x-edge (j, i) ; q = 1: a- of x-edge (j, i+1)
-            double at[3], bm[3], bp[3];
-            uns_vec(Tx, a.tot, c + q, q == 0 ? 1 : 0, at);
-            gc_transverse(a.g, a.eps, h, pn, pt, at, bm, bp);
-            if (a.coord == 1) {
-#pragma unroll
-                for (int k = 0; k < 3; k++) { bm[k] = bm[k] * a.ey[pd.j0 + j]; bp[k] = bp[k] * a.ey[pd.j0 + j + 1]; }
-            }
-#pragma unroll
-            for (int k = 0; k < 3; k++) G2[k] = __fma_rn(-half, r == 0 ? bp[k] : bm[k], G2[k]);
-        }
-    }
+    for (int p = 0; p < 18; p++) uns_cpa8(sdst + (unsigned)(3 + p) * 256u, T + (int64_t)p * a.tot);
 }
 
-// F~' of the x-edge at the left side of cell (row j, column e) [offset o]: F~, then the right-going parts from column e-1,
-// then the left-going parts from column e, each column's y-edges in the order (b+ of the cell's lower edge, b- of its upper edge)
-__device__ __forceinline__ void uns_F2(const UnsArgs &a, const PatchDesc &pd, int64_t o, int j, double (&F2)[3])
+// grid = patches x groups of UNS_UPD_WARPS tasks; task = (30 updating columns, a halo lane on each side) x (UNS_SEG rows of 2..ny+1).
+// Every row does the same work with no branch around the shuffles (the first and the last row of a segment compute a few numbers
+// nobody uses); SPH: latitude-longitude grid (edge factors applied).
+template <int SPH>
+__global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
 {
-    const double *Tx = a.T, *Ty = a.T + 9 * a.tot;
-#pragma unroll
-    for (int k = 0; k < 3; k++) F2[k] = Tx[(int64_t)(6 + k) * a.tot + o];
-    const double half = 0.5 * (a.dt * a.rdy[pd.j0 + j]);
-#pragma unroll
-    for (int r = 0; r < 2; r++) {                               // r = 0: column e-1 (its cp), r = 1: column e (its cm)
-        const int64_t c = o - (1 - r);
-        const double h = a.h[c], pn = a.hu[c], pt = a.hv[c];
-#pragma unroll
-        for (int q = 0; q < 2; q++) {                           // q = 0: b+ of y-edge (j, .) ; q = 1: b- of y-edge (j+1, .)
-            double at[3], cm[3], cp[3];
-            uns_vec(Ty, a.tot, c + (int64_t)q * pd.pitch, q == 0 ? 1 : 0, at);
-            gc_transverse(a.g, a.eps, h, pn, pt, at, cm, cp);
-            if (a.coord == 1) {
-#pragma unroll
-                for (int k = 0; k < 3; k++) { cm[k] = cm[k] * a.ex; cp[k] = cp[k] * a.ex; }
-            }
-#pragma unroll
-            for (int k = 0; k < 3; k++) F2[k] = __fma_rn(-half, r == 0 ? cp[k] : cm[k], F2[k]);
-        }
-    }
-}
-
-__global__ void __launch_bounds__(128) k_uns_update(UnsArgs a)
-{
+    extern __shared__ double uns_sm[];
     const PatchDesc pd = a.pat[blockIdx.x];
-    const int n = pd.nx * pd.ny;
-    const double *Tx = a.T, *Ty = a.T + 9 * a.tot;
-    for (int t = blockIdx.y * 4096 + threadIdx.x; t < min(n, (int)(blockIdx.y + 1) * 4096); t += blockDim.x) {
-        const int j = 2 + t / pd.nx, i = 2 + t % pd.nx;
-        const int64_t o = pd.off + (int64_t)j * pd.pitch + i;
-        double Fl[3], Fr[3], Gl[3], Gu[3];
-        uns_F2(a, pd, o, j, Fl); uns_F2(a, pd, o + 1, j, Fr);
-        uns_G2(a, pd, o, j, Gl); uns_G2(a, pd, o + pd.pitch, j + 1, Gu);
-        double dfx[3], dgy[3];
+    const int lane = threadIdx.x & 31;
+    const int ncw = (pd.nx + 29) / 30, nsg = (pd.ny + UNS_SEG - 1) / UNS_SEG;
+    const int task = blockIdx.y * UNS_UPD_WARPS + (threadIdx.x >> 5);
+    if (task >= ncw * nsg) return;
+    const int cw = task % ncw, sg = task / ncw;
+    const int col0 = 1 + cw * 30 + lane;                        // lane 0: the column left of the 30; lane 31: the one right of them
+    const int col = min(col0, pd.nx + 2);                       // lanes past the patch repeat its last column and store nothing
+    const bool upd = lane >= 1 && lane <= 30 && col0 <= pd.nx + 1;
+    const int ja = 2 + sg * UNS_SEG, jb = min(ja + UNS_SEG, pd.ny + 2);
+    const double *S = uns_sm + (threadIdx.x >> 5) * UNS_RING_DOUBLES;                       // this warp's ring
+    const unsigned sl = (unsigned)__cvta_generic_to_shared(S) + (unsigned)lane * 8u;        // ... and this lane's column of it
+    const int ln1 = min(lane + 1, 31);
+    int64_t o = pd.off + (int64_t)(ja - 1) * pd.pitch + col;
+    uns_stage_row(a, o, sl);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    uns_stage_row(a, o + pd.pitch, sl + (unsigned)(UNS_NPL * 256));
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    double bpq[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};      // up-going parts of row r-1
+    double dfx[3] = {0.0, 0.0, 0.0}, gp[3] = {0.0, 0.0, 0.0}, qh = 0.0, qu = 0.0, qv = 0.0;   // of cell r-1
+    int st = 0;                                                 // ring stage of row r
+    for (int r = ja - 1; r <= jb; r++, o += pd.pitch) {
+        const int st1 = st == 2 ? 0 : st + 1, st2 = st1 == 2 ? 0 : st1 + 1;
+        __syncwarp();                                           // every lane has finished with row r-1, whose stage is refilled
+        if (r + 2 <= jb) uns_stage_row(a, o + 2 * (int64_t)pd.pitch, sl + (unsigned)(st2 * UNS_NPL * 256));
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");    // rows r and r+1 have arrived
+        __syncwarp();
+        const double *R0 = S + st * (UNS_NPL * 32), *R1 = S + st1 * (UNS_NPL * 32);
+        const double h = R0[lane], hu = R0[32 + lane], hv = R0[64 + lane];
+        double amx1[3], apx[3], Fx[3], Fx1[3], amy[3], apy[3], Gy[3], amu[3], Gu[3];
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            const double fm = Fr[k] + Tx[(int64_t)k * a.tot + o + 1], fp = Fl[k] - Tx[(int64_t)(3 + k) * a.tot + o];
-            const double gm = Gu[k] + Ty[(int64_t)k * a.tot + o + pd.pitch], gp = Gl[k] - Ty[(int64_t)(3 + k) * a.tot + o];
-            dfx[k] = fm - fp; dgy[k] = gm - gp;
+            amx1[k] = R0[(3 + k) * 32 + ln1]; apx[k] = R0[(6 + k) * 32 + lane]; Fx[k] = R0[(9 + k) * 32 + lane]; Fx1[k] = R0[(9 + k) * 32 + ln1];
+            amy[k] = R0[(12 + k) * 32 + lane]; apy[k] = R0[(15 + k) * 32 + lane]; Gy[k] = R0[(18 + k) * 32 + lane];
+            amu[k] = R1[(12 + k) * 32 + lane]; Gu[k] = R1[(18 + k) * 32 + lane];      // of the cell's upper y-edge: the next row's
         }
-        const double dtdx = a.dt * a.rdx[pd.j0 + j], dtdy = a.dt * a.rdy[pd.j0 + j];
-        double hh = __fma_rn(-dtdy, dgy[0], __fma_rn(-dtdx, dfx[0], a.h[o]));
-        double uu = __fma_rn(-dtdy, dgy[2], __fma_rn(-dtdx, dfx[1], a.hu[o]));
-        double vv = __fma_rn(-dtdy, dgy[1], __fma_rn(-dtdx, dfx[2], a.hv[o]));
-        if (hh < a.eps && a.write_out) {                                                 // dry clean-up (S-9)
-            if (hh < 0.0) {
-                atomicAdd(&a.stats->nclip, 1ull);
-                atomicAdd(&a.stats->clipped, (-hh) * (a.kappa[pd.j0 + j] * a.dxdy));
+        UnsJac Jx, Jy;
+        if (!uns_jac2<true>(a.g, a.eps, h, hu, hv, Jx, Jy)) uns_jac2<false>(a.g, a.eps, h, hu, hv, Jx, Jy);
+        // a+ of the cell's left and a- of its right x-edge (target frame: components 1 and 2 swapped), split by the y-Jacobian;
+        // b+ of its lower and b- of its upper y-edge, split by the x-Jacobian
+        double bm[2][3], bp[2][3], cm[2][3], cp[2][3];
+        {
+            const double a0[3] = { apx[0] - Fx[0], apx[2] - Fx[2], apx[1] - Fx[1] };
+            const double a1[3] = { amx1[0] + Fx1[0], amx1[2] + Fx1[2], amx1[1] + Fx1[1] };
+            const double b0[3] = { apy[0] - Gy[0], apy[2] - Gy[2], apy[1] - Gy[1] };
+            const double b1[3] = { amu[0] + Gu[0], amu[2] + Gu[2], amu[1] + Gu[1] };
+            uns_split(Jy, a0, bm[0], bp[0]);
+            uns_split(Jy, a1, bm[1], bp[1]);
+            uns_split(Jx, b0, cm[0], cp[0]);
+            uns_split(Jx, b1, cm[1], cp[1]);
+        }
+        if (SPH) {
+            const double e0 = a.ey[pd.j0 + r], e1 = a.ey[pd.j0 + r + 1];
+#pragma unroll
+            for (int q = 0; q < 2; q++)
+#pragma unroll
+                for (int k = 0; k < 3; k++) { bm[q][k] = bm[q][k] * e0; bp[q][k] = bp[q][k] * e1; cm[q][k] = cm[q][k] * a.ex; cp[q][k] = cp[q][k] * a.ex; }
+        }
+        // F~' of the cell's left x-edge: F~, the right-going parts from the column to the left (the lane below), the left-going
+        // parts from this column; the right edge's F~' is the next lane's
+        const double hf = 0.5 * (a.dt * a.rdy[pd.j0 + r]);
+        double F2[3], dfn[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            double v = Fx[k];
+            v = __fma_rn(-hf, shfl_up1(cp[0][k]), v); v = __fma_rn(-hf, shfl_up1(cp[1][k]), v);
+            v = __fma_rn(-hf, cm[0][k], v);           v = __fma_rn(-hf, cm[1][k], v);
+            F2[k] = v;
+        }
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const double fm = shfl_dn1(F2[k]) + amx1[k], fp = F2[k] - apx[k];
+            dfn[k] = fm - fp;
+        }
+        // G~' of the y-edge below cell r: G~, the up-going parts from row r-1, the down-going parts from row r (3.13's order)
+        double G2[3];
+        const double hb = 0.5 * (a.dt * a.rdx[pd.j0 + r - 1]), hr = 0.5 * (a.dt * a.rdx[pd.j0 + r]);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            double v = Gy[k];
+            v = __fma_rn(-hb, bpq[0][k], v); v = __fma_rn(-hb, bpq[1][k], v);
+            v = __fma_rn(-hr, bm[0][k], v);  v = __fma_rn(-hr, bm[1][k], v);
+            G2[k] = v;
+        }
+        if (r > ja) {                                           // it closes cell r-1
+            const int j = r - 1;
+            double dgy[3];
+#pragma unroll
+            for (int k = 0; k < 3; k++) { const double gm = G2[k] + amy[k]; dgy[k] = gm - gp[k]; }
+            const double dtdx = a.dt * a.rdx[pd.j0 + j], dtdy = a.dt * a.rdy[pd.j0 + j];
+            double hh = __fma_rn(-dtdy, dgy[0], __fma_rn(-dtdx, dfx[0], qh));
+            double uu = __fma_rn(-dtdy, dgy[2], __fma_rn(-dtdx, dfx[1], qu));
+            double vv = __fma_rn(-dtdy, dgy[1], __fma_rn(-dtdx, dfx[2], qv));
+            if (upd) {
+                if (hh < a.eps && a.write_out) {                                             // dry clean-up (S-9)
+                    if (hh < 0.0) {
+                        atomicAdd(&a.stats->nclip, 1ull);
+                        atomicAdd(&a.stats->clipped, (-hh) * (a.kappa[pd.j0 + j] * a.dxdy));
+                    }
+                    hh = dmax(hh, 0.0); uu = 0.0; vv = 0.0;
+                }
+                if (a.friction && a.write_out) {
+                    const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, a.dt, hh, uu, vv);
+                    uu = q.x; vv = q.y;
+                }
+                if (hh != hh || uu != uu || vv != vv) a.stats->nan_seen = 1;
+                if (a.write_out) { const int64_t oc = o - pd.pitch; a.oh[oc] = hh; a.ohu[oc] = uu; a.ohv[oc] = vv; }
             }
-            hh = dmax(hh, 0.0); uu = 0.0; vv = 0.0;
         }
-        if (a.friction && a.write_out) {
-            const double2 q = gc_friction_apply(a.gn2, a.eps, a.fdepth, a.dt, hh, uu, vv);
-            uu = q.x; vv = q.y;
-        }
-        if (hh != hh || uu != uu || vv != vv) a.stats->nan_seen = 1;
-        if (a.write_out) { a.oh[o] = hh; a.ohu[o] = uu; a.ohv[o] = vv; }
+#pragma unroll
+        for (int k = 0; k < 3; k++) { gp[k] = G2[k] - apy[k]; dfx[k] = dfn[k]; bpq[0][k] = bp[0][k]; bpq[1][k] = bp[1][k]; }
+        qh = h; qu = hu; qv = hv;
+        st = st1;
     }
 }
 
@@ -240,14 +406,18 @@ int gc_launch_unsplit(gc_level *L, double dt, int write_out)
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out;
     a.gn2 = P.g * (P.manning_n * P.manning_n); a.fdepth = P.friction_depth; a.friction = P.manning_n > 0.0 ? 1 : 0;
     a.stats = L->d_stats;
-    int64_t me = 1, mc = 1;
+    int64_t wx = 1, ty = 1, tu = 1;                            // windows of k_uns_xedges, tasks of k_uns_yedges / k_uns_update
     for (const gc_patch &Q : L->pat) {
-        me = std::max<int64_t>(me, std::max<int64_t>((int64_t)(Q.ny + 2) * (Q.nx + 1), (int64_t)(Q.nx + 2) * (Q.ny + 1)));
-        mc = std::max<int64_t>(mc, (int64_t)Q.nx * Q.ny);
+        wx = std::max<int64_t>(wx, ((int64_t)(Q.ny + 2) * (Q.nx + 3) + UNS_WIN - 1) / UNS_WIN);
+        ty = std::max<int64_t>(ty, (int64_t)((Q.nx + 2 + 31) / 32) * ((Q.ny + 1 + UNS_SEG - 1) / UNS_SEG));
+        tu = std::max<int64_t>(tu, (int64_t)((Q.nx + 29) / 30) * ((Q.ny + UNS_SEG - 1) / UNS_SEG));
     }
-    const dim3 ge((unsigned)L->np, (unsigned)((me + 4095) / 4096)), gc((unsigned)L->np, (unsigned)((mc + 4095) / 4096));
-    { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_uns_edges<0><<<ge, 128, 0, L->ctx->stream>>>(a); }
-    { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_uns_edges<1><<<ge, 128, 0, L->ctx->stream>>>(a); }
-    { ProfScope ps(L->ctx, GC_SLOT_FUSED); k_uns_update<<<gc, 128, 0, L->ctx->stream>>>(a); }
+    const dim3 gx((unsigned)L->np, (unsigned)((wx + UNS_WPB - 1) / UNS_WPB)), gy((unsigned)L->np, (unsigned)((ty + 3) / 4)),
+               gu((unsigned)L->np, (unsigned)((tu + UNS_UPD_WARPS - 1) / UNS_UPD_WARPS));
+    { ProfScope ps(L->ctx, GC_SLOT_XSWEEP); k_uns_xedges<<<gx, 128, 0, L->ctx->stream>>>(a); }
+    { ProfScope ps(L->ctx, GC_SLOT_YSWEEP); k_uns_yedges<<<gy, 128, 0, L->ctx->stream>>>(a); }
+    { ProfScope ps(L->ctx, GC_SLOT_FUSED); const size_t sm = UNS_UPD_WARPS * UNS_RING_DOUBLES * sizeof(double);
+      if (P.coord == 1) k_uns_update<1><<<gu, 32 * UNS_UPD_WARPS, sm, L->ctx->stream>>>(a);
+      else k_uns_update<0><<<gu, 32 * UNS_UPD_WARPS, sm, L->ctx->stream>>>(a); }
     return GC_OK;
 }
