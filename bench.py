@@ -141,7 +141,7 @@ def host_fields(wl, n):
     return out
 
 
-def oracle_leg(wl, n, side, fields, steps, warmup, threads, budget_s=None):
+def oracle_leg(wl, n, side, fields, steps, warmup, threads, budget_s=None, unsplit=False):
     """The oracle as it stands on the bench workload (n x n in patches of `side`), its loop over patches on `threads` host
     cores (0 = all).  steps = None: as many steps as fit budget_s after the first.  -> (updates/s, seconds, steps, threads)"""
     import workloads
@@ -155,7 +155,7 @@ def oracle_leg(wl, n, side, fields, steps, warmup, threads, budget_s=None):
 
     def one(dt):
         L.fill_ghost(None, 1.0)
-        return wl.cfl / L.step(dt)["s_over_dx_max"]
+        return wl.cfl / (L.step_unsplit(dt) if unsplit else L.step(dt))["s_over_dx_max"]
     for _ in range(warmup):
         dt = one(dt)
     t0 = time.time()
@@ -180,7 +180,7 @@ def run_reference(args):
     n, side = args.n, args.side
     wl = workloads.cfg5(n)
     fields = host_fields(wl, n)
-    rate, el, k, nt = oracle_leg(wl, n, side, fields, max(args.steps, 1), args.warmup, 0)
+    rate, el, k, nt = oracle_leg(wl, n, side, fields, max(args.steps, 1), args.warmup, 0, unsplit=args.scheme == "unsplit")
     sample = "cfg5 spherical %dx%d in patches of side %d (the whole workload), %d steps after %d warm-up, loop over patches on %d threads" \
              % (n, n, side, k, args.warmup, nt)
     print(json.dumps({
@@ -206,6 +206,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-tilings", action="store_true", help="skip config.tilings (sides 16 ... 256)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end legs")
+    ap.add_argument("--scheme", default="split", choices=("split", "unsplit"),
+                    help="split: the paper's dimensionally split step (the headline); unsplit: the step with transverse Riemann solves "
+                         "(DESIGN.md 3.13; fixed dt, no tilings / e2e legs)")
     ap.add_argument("--gauges", type=int, default=0,
                     help="bind this many seeded gauges and record them into a device-resident series every step (DESIGN.md 3.10)")
     ap.add_argument("--manning", type=float, default=0.0,
@@ -223,6 +226,9 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     rank, world, local, dist = init_ranks("nccl", torch.device("cuda", local))
+    unsplit = args.scheme == "unsplit"
+    if unsplit:
+        args.no_tilings = args.no_e2e = True
     assert args.gpus == world, "--gpus %d but WORLD_SIZE %d: launch N > 1 with torch.distributed.run (one rank per GPU)" % (args.gpus, world)
     dev = "cuda:%d" % local
     W = args.warmup
@@ -259,7 +265,10 @@ def main():
             L.fill_ghost(None, 1.0)
             if series is not None:
                 L.gauges_sample_into(series[k])      # one record per step, straight into the device-resident series
-            L.step_auto(dt_dev, wl.cfl)
+            if unsplit:
+                L.step_unsplit(dt0)                  # fixed dt (gc_level_step_unsplit returns its statistics to the host)
+            else:
+                L.step_auto(dt_dev, wl.cfl)
         for k in range(warm):
             one_step(k)
         torch.cuda.synchronize()
@@ -388,8 +397,17 @@ def main():
     share = {k: v[0] / max(sum(x[0] for x in prof.values()), 1e-12) for k, v in prof.items() if v[1]}
     # cells one launch of the dominant kernel updates: the x-sweep also covers the 4 ghost rows of every patch (S-5)
     per_launch = {"xsweep": cells * (1.0 + 4.0 / args.side), "ysweep": float(cells)}.get(dom, float(cells))
-    kc = counts["kernels"].get(dom) if counts else None
-    if kc:
+    kc = counts["kernels"].get(dom) if counts and not unsplit else None
+    if unsplit:
+        # planes of 8 bytes per cell the kernels of DESIGN.md 3.13 must move: the edge kernels read h, hu, hv, b and write
+        # (A-dQ, A+dQ, F~); the update reads those 18 and h, hu, hv and writes the new state
+        ub = {"xsweep": 104.0, "ysweep": 104.0, "fused": 192.0}.get(dom, 56.0)
+        gbs = ub * cells / (dom_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": {"xsweep": "k_uns_xedges", "ysweep": "k_uns_yedges", "fused": "k_uns_update"}.get(dom, dom),
+                    "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
+                    "peak_source": "MEASURED_PEAKS.json" if which == "measured" else "fallback 6650 GB/s",
+                    "bytes_per_cell": ub, "cells_per_launch": float(cells), "kernel_ms": dom_ms, "kernel_share_of_step": share}
+    elif kc:
         achieved = kc["flop_per_cell"] * per_launch / (dom_ms * 1e-3) / 1e12
         traffic = kc["dram_bytes_per_launch"] if (n, args.side) == (counts.get("n"), counts.get("side")) else None
         roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
@@ -415,7 +433,8 @@ def main():
                                % (n, n, n // args.side, n // args.side, args.side),
                    "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (cells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl,
-                   "fma": "explicit, where DESIGN.md 3 writes it (both sides)", "manning_n": args.manning, "gauges": args.gauges},
+                   "fma": "explicit, where DESIGN.md 3 writes it (both sides)", "manning_n": args.manning, "gauges": args.gauges,
+                   "scheme": args.scheme},
         "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
         "hbm": {"achieved_gbs": BYTES_PER_UPDATE * value / world / 1e9, "peak_gbs": hbm_peak,
                 "frac": BYTES_PER_UPDATE * value / world / 1e9 / hbm_peak, "of": which, "bytes_per_update": BYTES_PER_UPDATE},
@@ -427,8 +446,8 @@ def main():
     if not args.no_cpu and world == 1:
         if L is not None:
             L.destroy()
-        rate, el, k, nt = oracle_leg(wl, n, args.side, fields, None, 0, 0, budget_s=12.0)
-        rate1, el1, k1, _ = oracle_leg(wl, n, args.side, fields, 1, 0, 1)
+        rate, el, k, nt = oracle_leg(wl, n, args.side, fields, None, 0, 0, budget_s=12.0, unsplit=unsplit)
+        rate1, el1, k1, _ = oracle_leg(wl, n, args.side, fields, 1, 0, 1, unsplit=unsplit)
         out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": nt, "kind": "oracle",
                                "sample": "the bench workload itself (%dx%d in patches of side %d): %d steps in %.1f s, loop over patches on "
                                          "%d threads" % (n, n, args.side, k, el, nt),

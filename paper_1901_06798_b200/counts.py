@@ -20,11 +20,11 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def source_hash():
-    """sha256 over the kernel sources and the ABI headers"""
+    """sha256 over what the sweep kernels are compiled from: gc_sweep.cu, every header beside it, the ABI headers"""
     h = hashlib.sha256()
     for d in (os.path.join(ROOT, "paper_1901_06798_b200", "csrc"), os.path.join(ROOT, "include")):
         for f in sorted(os.listdir(d)):
-            if f.endswith((".cu", ".cuh", ".h")):
+            if f == "gc_sweep.cu" or f.endswith((".cuh", ".h")):
                 h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()
 

@@ -78,6 +78,11 @@ __device__ __forceinline__ void uns_finish(const UnsArgs &a, const Waves &We, bo
     for (int k = 0; k < 3; k++) { T[(int64_t)k * a.tot] = am[k]; T[(int64_t)(3 + k) * a.tot] = ap[k]; T[(int64_t)(6 + k) * a.tot] = F[k]; }
 }
 
+__device__ __forceinline__ void uns_cpa8(unsigned sdst, const double *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
+}
+
 __device__ __forceinline__ void uns_cfl_out(const UnsArgs &a, double cfl)
 {
 #pragma unroll
@@ -107,13 +112,16 @@ __global__ void __launch_bounds__(128) k_uns_xedges(UnsArgs a)
     int line, e; int64_t o;
     bool active = locate(w0, line, e, o);
     RState cL = uns_cell(a, o - 1, 0), cR = uns_cell(a, o, 0);
+    double rd = a.rdx[pd.j0 + line];
     for (int w = w0; w < w1; w++) {
         const int buf = w & 1;
         int line2 = line, e2 = e; int64_t o2 = o; bool act2 = false;
         RState nL = cL, nR = cR;
+        double rd2 = rd;
         if (w + 1 < w1) {                                       // the next window's cells, loaded a window ahead of their use
             act2 = locate(w + 1, line2, e2, o2);
             nL = uns_cell(a, o2 - 1, 0); nR = uns_cell(a, o2, 0);
+            rd2 = a.rdx[pd.j0 + line2];
         }
         Waves We;
         bool stdE = false;
@@ -129,11 +137,10 @@ __global__ void __launch_bounds__(128) k_uns_xedges(UnsArgs a)
                 dlo[q] = __fma_rn(We.Z[q][2], sZ[buf][3 * q + 2][k - 1], __fma_rn(We.Z[q][1], sZ[buf][3 * q + 1][k - 1], We.Z[q][0] * sZ[buf][3 * q][k - 1]));
                 dhi[q] = __fma_rn(sZ[buf][3 * q + 2][k + 1], We.Z[q][2], __fma_rn(sZ[buf][3 * q + 1][k + 1], We.Z[q][1], sZ[buf][3 * q][k + 1] * We.Z[q][0]));
             }
-            const double rd = a.rdx[pd.j0 + line];
             uns_finish(a, We, stdE, dlo, dhi, rd, rd, a.T + o);
             if (line >= 2 && line < pd.ny + 2) cfl = dmax(cfl, gc_edge_cfl(We, rd, rd));
         }
-        active = act2; line = line2; e = e2; o = o2; cL = nL; cR = nR;
+        active = act2; line = line2; e = e2; o = o2; cL = nL; cR = nR; rd = rd2;
     }
     uns_cfl_out(a, cfl);
 }
@@ -152,30 +159,60 @@ __global__ void __launch_bounds__(128) k_uns_yedges(UnsArgs a)
     const int col = valid ? col0 : pd.nx + 2;                   // lanes past the patch repeat its last column and store nothing
     const int ea = 2 + sg * UNS_SEG, eb = min(ea + UNS_SEG, pd.ny + 3);
     const bool counted = valid && col >= 2 && col < pd.nx + 2;
+    // the column's cells are staged three rows ahead of their use, 8 bytes per lane and plane by cp.async into the warp's ring
+    // of four rows (a DRAM round trip under this load outlasts an iteration, and plain loads two ahead would still be waited
+    // for at the top of every iteration: they share a scoreboard); metric terms are loaded one iteration ahead
+    __shared__ double ring[4][4][4][32];                        // warp, stage, plane (h, hu, hv, b), lane
+    const int wp = threadIdx.x >> 5;
+    const unsigned sl = (unsigned)__cvta_generic_to_shared(&ring[wp][0][0][lane]);
     int64_t o = pd.off + (int64_t)(ea - 2) * pd.pitch + col;
     RState cprev = uns_cell(a, o, 1);
-    RState cnext = uns_cell(a, o + pd.pitch, 1);               // loaded one iteration ahead of its use
+#pragma unroll
+    for (int q = 0; q < 3; q++) {                               // rows ea-1, ea, ea+1 into stages 0, 1, 2
+        if (ea - 1 + q <= eb) {
+            const int64_t oq = o + (int64_t)(q + 1) * pd.pitch;
+            uns_cpa8(sl + q * 1024u, a.h + oq); uns_cpa8(sl + q * 1024u + 256u, a.hu + oq);
+            uns_cpa8(sl + q * 1024u + 512u, a.hv + oq); uns_cpa8(sl + q * 1024u + 768u, a.b + oq);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    double efn = a.ey[pd.j0 + ea - 1], rd0 = a.rdy[pd.j0 + ea - 3 >= 0 ? pd.j0 + ea - 3 : 0], rd1 = a.rdy[pd.j0 + ea - 2], rdn = a.rdy[pd.j0 + ea - 1];
     Waves Wc;
     gc_waves_zero(Wc);
     double dlo[3] = {0.0, 0.0, 0.0};
     bool stdc = false;
     double cfl = 0.0;
+    int st = 0;                                                 // ring stage of row m
     for (int m = ea - 1; m <= eb; m++) {                        // solves edge m (cells m-1 | m); finishes edge m-1
         o += pd.pitch;
-        const RState cnew = cnext;
-        if (m < eb) cnext = uns_cell(a, o + pd.pitch, 1);
+        {
+            const int s3 = (st + 3) & 3;
+            if (m + 3 <= eb) {
+                const int64_t oq = o + 3 * (int64_t)pd.pitch;
+                uns_cpa8(sl + s3 * 1024u, a.h + oq); uns_cpa8(sl + s3 * 1024u + 256u, a.hu + oq);
+                uns_cpa8(sl + s3 * 1024u + 512u, a.hv + oq); uns_cpa8(sl + s3 * 1024u + 768u, a.b + oq);
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 3;" ::: "memory"); // row m has arrived
+        }
+        RState cnew;
+        cnew.h = ring[wp][st][0][lane]; cnew.p = ring[wp][st][2][lane]; cnew.t = ring[wp][st][1][lane]; cnew.b = ring[wp][st][3][lane];
+        cnew.u = 0.0; cnew.v = 0.0; cnew.phi = 0.0; cnew.c = 0.0;
+        const double ef = efn, rdL = rd0, rdR = rd1;            // ey[j0 + m], rdy[j0 + m - 2], rdy[j0 + m - 1]
+        rd0 = rd1; rd1 = rdn;
+        if (m < eb) { efn = a.ey[pd.j0 + m + 1]; rdn = a.rdy[pd.j0 + m + 1]; }
         Waves Wn;
-        const bool stdn = uns_solve(a, cprev, cnew, a.ey[pd.j0 + m], Wn);
+        const bool stdn = uns_solve(a, cprev, cnew, ef, Wn);
         double dhi[3];
         gc_wave_dots(Wn, Wc, dhi);
         if (m >= ea + 1) {
-            const double rdL = a.rdy[pd.j0 + m - 2], rdR = a.rdy[pd.j0 + m - 1];
             if (valid) uns_finish(a, Wc, stdc, dlo, dhi, rdL, rdR, a.T + 9 * a.tot + (o - pd.pitch));
             if (counted) cfl = dmax(cfl, gc_edge_cfl(Wc, rdL, rdR));
         }
         Wc = Wn; stdc = stdn; cprev = cnew;
 #pragma unroll
         for (int q = 0; q < 3; q++) dlo[q] = dhi[q];
+        st = (st + 1) & 3;
     }
     uns_cfl_out(a, cfl);
 }
@@ -251,10 +288,6 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0
 #define UNS_UPD_WARPS 2
 #define UNS_NPL 21
 #define UNS_RING_DOUBLES (3 * UNS_NPL * 32)
-__device__ __forceinline__ void uns_cpa8(unsigned sdst, const double *gsrc)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
-}
 __device__ __forceinline__ void uns_stage_row(const UnsArgs &a, int64_t o, unsigned sdst)
 {
     uns_cpa8(sdst, a.h + o); uns_cpa8(sdst + 256u, a.hu + o); uns_cpa8(sdst + 512u, a.hv + o);
@@ -291,7 +324,11 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
     double bpq[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};      // up-going parts of row r-1
     double dfx[3] = {0.0, 0.0, 0.0}, gp[3] = {0.0, 0.0, 0.0}, qh = 0.0, qu = 0.0, qv = 0.0;   // of cell r-1
     int st = 0;                                                 // ring stage of row r
+    // metric terms of rows r-1, r (and the edge factors of edges r, r+1), loaded a row ahead of their use
+    double ey0 = a.ey[pd.j0 + ja - 1], ey1 = a.ey[pd.j0 + ja], rxm = a.rdx[pd.j0 + ja - 2], rx0 = a.rdx[pd.j0 + ja - 1],
+           rym = a.rdy[pd.j0 + ja - 2], ry0 = a.rdy[pd.j0 + ja - 1];
     for (int r = ja - 1; r <= jb; r++, o += pd.pitch) {
+        const double ey2 = a.ey[pd.j0 + r + 2], rx1 = a.rdx[pd.j0 + r + 1], ry1 = a.rdy[pd.j0 + r + 1];
         const int st1 = st == 2 ? 0 : st + 1, st2 = st1 == 2 ? 0 : st1 + 1;
         __syncwarp();                                           // every lane has finished with row r-1, whose stage is refilled
         if (r + 2 <= jb) uns_stage_row(a, o + 2 * (int64_t)pd.pitch, sl + (unsigned)(st2 * UNS_NPL * 256));
@@ -323,7 +360,7 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
             uns_split(Jx, b1, cm[1], cp[1]);
         }
         if (SPH) {
-            const double e0 = a.ey[pd.j0 + r], e1 = a.ey[pd.j0 + r + 1];
+            const double e0 = ey0, e1 = ey1;
 #pragma unroll
             for (int q = 0; q < 2; q++)
 #pragma unroll
@@ -331,7 +368,7 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
         }
         // F~' of the cell's left x-edge: F~, the right-going parts from the column to the left (the lane below), the left-going
         // parts from this column; the right edge's F~' is the next lane's
-        const double hf = 0.5 * (a.dt * a.rdy[pd.j0 + r]);
+        const double hf = 0.5 * (a.dt * ry0);
         double F2[3], dfn[3];
 #pragma unroll
         for (int k = 0; k < 3; k++) {
@@ -347,7 +384,7 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
         }
         // G~' of the y-edge below cell r: G~, the up-going parts from row r-1, the down-going parts from row r (3.13's order)
         double G2[3];
-        const double hb = 0.5 * (a.dt * a.rdx[pd.j0 + r - 1]), hr = 0.5 * (a.dt * a.rdx[pd.j0 + r]);
+        const double hb = 0.5 * (a.dt * rxm), hr = 0.5 * (a.dt * rx0);
 #pragma unroll
         for (int k = 0; k < 3; k++) {
             double v = Gy[k];
@@ -360,7 +397,7 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
             double dgy[3];
 #pragma unroll
             for (int k = 0; k < 3; k++) { const double gm = G2[k] + amy[k]; dgy[k] = gm - gp[k]; }
-            const double dtdx = a.dt * a.rdx[pd.j0 + j], dtdy = a.dt * a.rdy[pd.j0 + j];
+            const double dtdx = a.dt * rxm, dtdy = a.dt * rym;
             double hh = __fma_rn(-dtdy, dgy[0], __fma_rn(-dtdx, dfx[0], qh));
             double uu = __fma_rn(-dtdy, dgy[2], __fma_rn(-dtdx, dfx[1], qu));
             double vv = __fma_rn(-dtdy, dgy[1], __fma_rn(-dtdx, dfx[2], qv));
@@ -383,6 +420,7 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
 #pragma unroll
         for (int k = 0; k < 3; k++) { gp[k] = G2[k] - apy[k]; dfx[k] = dfn[k]; bpq[0][k] = bp[0][k]; bpq[1][k] = bp[1][k]; }
         qh = h; qu = hu; qv = hv;
+        ey0 = ey1; ey1 = ey2; rxm = rx0; rx0 = rx1; rym = ry0; ry0 = ry1;
         st = st1;
     }
 }
