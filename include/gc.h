@@ -200,7 +200,8 @@ int gc_level_init_from(gc_level *newfine, const gc_level *oldfine, const gc_leve
 
 /* A8 (P:146 step 5): flux registers on the boundary of the fine region.  attach builds and zeroes them
  * (and makes both levels record what the registers need during gc_level_step); fixup applies
- * Q_C += side * delta / area to the uncovered coarse neighbours, then the clean-up rule, and re-zeroes. */
+ * Q_C += side * delta / area to the uncovered coarse neighbours, then the clean-up rule, and re-zeroes.
+ * GC_ERR_BADARG for a refinement ratio above 128, GC_ERR_STATE if the fine level is not nested in the coarse one. */
 int gc_flux_attach(gc_level *coarse, gc_level *fine);
 int gc_flux_fixup(gc_level *coarse, gc_level *fine);
 

@@ -354,21 +354,26 @@ __global__ void __launch_bounds__(64) k_flux_coarse(FluxArgs a)
 
 __device__ __forceinline__ double p_used(double h, double p, double eps) { return (h <= eps) ? 0.0 : p; }
 
-// the fine level has just stepped: delta -= dt l (F_k + e J_k) for the r fine cells along the coarse edge, in order
-__global__ void __launch_bounds__(64) k_flux_fine(FluxArgs a)
+// the fine level has just stepped: delta -= dt l (F_k + e J_k) for the r fine cells along the coarse edge, in order.
+// Thread <-> (register, fine cell k): the r terms of a register -- four Riemann problems each -- are computed side by side,
+// then the register's first thread subtracts them in order.  Block = FLUX_FINE_BLOCK threads = floor(block / r) registers.
+#define FLUX_FINE_BLOCK 128
+__global__ void __launch_bounds__(FLUX_FINE_BLOCK) k_flux_fine(FluxArgs a)
 {
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= a.nreg) return;
-    const FluxReg R = a.reg[n];
-    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
-    double d0 = a.delta[3 * n + 0], d1 = a.delta[3 * n + 1], d2 = a.delta[3 * n + 2];
-    RState B; B.h = a.base[4 * n + 0]; B.p = a.base[4 * n + 1]; B.t = a.base[4 * n + 2]; B.b = a.base[4 * n + 3];
-    B.u = 0.0; B.v = 0.0; B.phi = 0.0; B.c = 0.0;
-    const double sg = (R.side > 0) ? 1.0 : -1.0;
-    LineAcc A;
-    if (R.dir == 0) { A.h = a.qn0; A.p = a.qn1; A.t = a.qn2; A.b = a.b; A.str = 1; }
-    else            { A.h = a.qs0; A.p = a.qs2; A.t = a.qs1; A.b = a.b; A.str = R.fpitch; }
-    for (int m = 0; m < a.r; m++) {
+    __shared__ double term[3][FLUX_FINE_BLOCK];
+    const int per = FLUX_FINE_BLOCK / a.r;
+    const int li = threadIdx.x / a.r, m = threadIdx.x - li * a.r;
+    const int n = blockIdx.x * per + li;
+    const bool act = li < per && n < a.nreg;
+    if (act) {
+        const FluxReg R = a.reg[n];
+        const double dt = a.dt_dev ? *a.dt_dev : a.dt;
+        RState B; B.h = a.base[4 * n + 0]; B.p = a.base[4 * n + 1]; B.t = a.base[4 * n + 2]; B.b = a.base[4 * n + 3];
+        B.u = 0.0; B.v = 0.0; B.phi = 0.0; B.c = 0.0;
+        const double sg = (R.side > 0) ? 1.0 : -1.0;
+        LineAcc A;
+        if (R.dir == 0) { A.h = a.qn0; A.p = a.qn1; A.t = a.qn2; A.b = a.b; A.str = 1; }
+        else            { A.h = a.qs0; A.p = a.qs2; A.t = a.qs1; A.b = a.b; A.str = R.fpitch; }
         const int64_t c = R.fcell + (R.dir == 0 ? (int64_t)m * R.fpitch : (int64_t)m);
         double fm[3], fp[3], len, efJ;
         if (R.dir == 0) {
@@ -394,11 +399,18 @@ __global__ void __launch_bounds__(64) k_flux_fine(FluxArgs a)
         const double J1 = sg * ((Z[0][1] + Z[1][1]) + Z[2][1]);
         const double J2 = sg * ((Z[0][2] + Z[1][2]) + Z[2][2]);
         const double F0 = R.side > 0 ? fp[0] : fm[0], F1 = R.side > 0 ? fp[1] : fm[1], F2 = R.side > 0 ? fp[2] : fm[2];
-        d0 = d0 - dt * len * (F0 + efJ * J0);
-        d1 = d1 - dt * len * (F1 + efJ * J1);
-        d2 = d2 - dt * len * (F2 + efJ * J2);
+        term[0][threadIdx.x] = dt * len * (F0 + efJ * J0);
+        term[1][threadIdx.x] = dt * len * (F1 + efJ * J1);
+        term[2][threadIdx.x] = dt * len * (F2 + efJ * J2);
     }
-    a.delta[3 * n + 0] = d0; a.delta[3 * n + 1] = d1; a.delta[3 * n + 2] = d2;
+    __syncthreads();
+    if (act && m == 0) {
+        double d0 = a.delta[3 * n + 0], d1 = a.delta[3 * n + 1], d2 = a.delta[3 * n + 2];
+        for (int k = 0; k < a.r; k++) {
+            d0 = d0 - term[0][threadIdx.x + k]; d1 = d1 - term[1][threadIdx.x + k]; d2 = d2 - term[2][threadIdx.x + k];
+        }
+        a.delta[3 * n + 0] = d0; a.delta[3 * n + 1] = d1; a.delta[3 * n + 2] = d2;
+    }
 }
 
 static void fill_flux_args(FluxArgs &a, const gc_level *S, const gc_level *Creg, double dt, const double *dt_dev)
@@ -428,7 +440,8 @@ void gc_launch_flux_fine(gc_level *F, double dt, const double *dt_dev)
     if (!C || C->nreg == 0) return;
     FluxArgs a; fill_flux_args(a, F, C, dt, dt_dev);
     ProfScope ps(F->ctx, GC_SLOT_FLUX);
-    k_flux_fine<<<(C->nreg + 63) / 64, 64, 0, F->ctx->stream>>>(a);
+    const int per = FLUX_FINE_BLOCK / a.r;                      // registers per block (a.r <= FLUX_FINE_BLOCK: checked at attach)
+    k_flux_fine<<<(C->nreg + per - 1) / per, FLUX_FINE_BLOCK, 0, F->ctx->stream>>>(a);
 }
 
 // fix-up: one thread per corrected coarse cell, its registers applied in list order, then the clean-up rule

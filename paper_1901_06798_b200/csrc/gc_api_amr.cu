@@ -277,6 +277,7 @@ extern "C" int gc_flux_attach(gc_level *C, gc_level *F)
     if (!C || !F || C->ctx != F->ctx || C == F) return gc_fail(C ? C->ctx : nullptr, GC_ERR_BADARG, "gc_flux_attach: bad argument");
     gc_ctx *ctx = C->ctx;
     const int r = F->ratio;
+    if (r < 1 || r > 128) return gc_fail(ctx, GC_ERR_BADARG, "gc_flux_attach: refinement ratio outside 1..128");
     std::vector<FluxReg> regs;
     for (int p = 0; p < F->np; p++) {
         const gc_patch &P = F->pat[p];

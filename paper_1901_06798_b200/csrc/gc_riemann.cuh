@@ -26,12 +26,13 @@ __device__ __forceinline__ void gc_prim(M &m, RState &S, double g, double eps)
     if (S.h < 0.0) { S.h = 0.0; S.p = 0.0; S.t = 0.0; }      // R0
     if (S.h <= eps) {
         S.h = 0.0; S.p = 0.0; S.t = 0.0; S.u = 0.0; S.v = 0.0; S.phi = 0.0;
-    } else {
+        S.c = g * S.h;                                        // sqrt(g * 0) = sqrt(+-0) = +-0 = g * 0 itself: no call of the root, whose
+    } else {                                                  // zero operand takes the IEEE sequence's out-of-line path (land cells)
         double rh = m.rcp(S.h);
         S.u = S.p * rh; S.v = S.t * rh;
         S.phi = __fma_rn(S.p, S.u, 0.5 * g * (S.h * S.h));
+        S.c = m.sqrt_(g * S.h);
     }
-    S.c = m.sqrt_(g * S.h);
 }
 
 // R5: flat-bottom two-wave middle state M(hL, hR, uL, uR) -> (hm, sigma1, sigma2)

@@ -269,6 +269,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     RState Lst; Lst.h = 0.0; Lst.p = 0.0; Lst.t = 0.0; Lst.b = 0.0; Lst.u = 0.0; Lst.v = 0.0; Lst.phi = 0.0; Lst.c = 0.0;
     bool Lok = false;                                            // cell r-1 passed gc_prim_fast
     double cflm = 0.0;
+    unsigned fb_iters = 0u, fb_solves = 0u, fb_fluxes = 0u;
 
     // staging: thread-private slots, filled by cp.async one group (x: 2 cells, y: 1 cell) ahead of their use
     const unsigned st0 = (DIR == 0) ? sm0 + PK_XST * PK_SL : (unsigned)__cvta_generic_to_shared(dsm) + PK_YSTAGE * PK_SL + threadIdx.x * 8u;
@@ -346,14 +347,11 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         const bool badA = live & !(r >= 1 ? okR : okP);
         const bool badB = needB & !okB;
         if (__any_sync(0xffffffffu, badA | badB)) {
-            {   // P:345 accounting: one lane per warp, only on this (rare in open ocean) path
-                const unsigned ma = __ballot_sync(0xffffffffu, badA), mb = __ballot_sync(0xffffffffu, badB);
-                if ((threadIdx.x & 31) == 0) {
-                    atomicAdd(&a.stats->fb_warp_iters, 1ull);
-                    atomicAdd(&a.stats->fb_solves, (unsigned long long)__popc(ma));
-                    atomicAdd(&a.stats->fb_fluxes, (unsigned long long)__popc(mb));
-                }
-            }
+            // P:345 accounting: kept in registers, added to the level's counters once per warp at the end (three atomics on the
+            // same addresses from every such iteration serialise in L2 where land makes this path common)
+            fb_iters += 1u;
+            fb_solves += (unsigned)__popc(__ballot_sync(0xffffffffu, badA));
+            fb_fluxes += (unsigned)__popc(__ballot_sync(0xffffffffu, badB));
             if (badA) {
                 MathIeee mi;
                 R.h = qh; R.p = qp; R.t = qt; R.b = qb;
@@ -448,6 +446,11 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     if ((threadIdx.x & 31) == 0) {
         if (cflm > 0.0) atomicMax(&a.stats->sdx_bits, (unsigned long long)__double_as_longlong(cflm));
         atomicAdd(&a.stats->warp_iters, (unsigned long long)(nst_warp + 1));
+        if (fb_iters) {
+            atomicAdd(&a.stats->fb_warp_iters, (unsigned long long)fb_iters);
+            atomicAdd(&a.stats->fb_solves, (unsigned long long)fb_solves);
+            atomicAdd(&a.stats->fb_fluxes, (unsigned long long)fb_fluxes);
+        }
     }
 }
 
