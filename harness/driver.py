@@ -441,9 +441,13 @@ class Hierarchy:
     """The AMR recursion of P:140-146 (steps 1-5) with regridding every `regrid_interval` steps of a level,
     driving one backend through the C-ABI calls.  Bookkeeping only."""
 
-    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7, gauges=None, keep_unchanged=True):
+    def __init__(self, ctx, wl, max_levels=None, reflux=True, patches1=None, efficiency=0.7, gauges=None, keep_unchanged=True,
+                 accumulate=True):
         self.ctx, self.wl, self.reflux, self.eff = ctx, wl, reflux, efficiency
         self.gauges = gauges             # GaugeRecorder or None (DESIGN.md 3.10)
+        # a backend with step_accum / stats_reset (the CUDA path) is not waited for step by step: the levels' statistics accumulate
+        # on the device and are read once per coarse step and before a level is replaced (same numbers: a max of maxima)
+        self.accumulate = accumulate
         self.keep_unchanged = keep_unchanged   # keep a level whose regrid reproduces its patch list (bit-identical to recreating it)
         self.reuse_box_flags = keep_unchanged  # and do not re-flag a level whose flags can only come from unchanged forced boxes
         self._boxflag_cache = {}
@@ -513,6 +517,19 @@ class Hierarchy:
         boxes = cluster_native(fl, valid=ok, efficiency=self.eff, max_side=max(1, self.wl.patch_max // r))
         return np.array([[(b[0] + bbox[0]) * r, (b[1] + bbox[1]) * r, b[2] * r, b[3] * r] for b in boxes], dtype=np.int32)
 
+    def _accum(self, L):
+        return self.accumulate and hasattr(L, "step_accum")
+
+    def _harvest(self, k, L):
+        """the statistics level k's steps left on the device since the last harvest -> self.sdx[k]"""
+        if not self._accum(L):
+            return
+        st = L.stats()
+        if st["nan_seen"]:
+            raise RuntimeError("NaN in the updated state of level %d" % (k + 1))
+        self.sdx[k] = max(self.sdx[k], st["s_over_dx_max"])
+        L.stats_reset()
+
     def _regrid(self, k0, initial=False, t=None):
         """rebuild levels k0+1.. from the flags of the level below each; t = the time the levels k0.. have reached
         (a level regrids at the end of one of its own steps, when it and every finer level stand at the same time)"""
@@ -548,6 +565,8 @@ class Hierarchy:
                 C.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
                 N.init_from(old, C)
             if old is not None:
+                if not initial:
+                    self._harvest(k + 1, old)
                 old.destroy()
                 self.levels[k + 1] = N
             else:
@@ -574,8 +593,11 @@ class Hierarchy:
         L.fill_ghost(self.levels[k - 1] if k > 0 else None, alpha)
         if self.gauges is not None:
             self.gauges.record(k, L, t)
-        st = L.step(dt)
-        self.sdx[k] = max(self.sdx[k], st["s_over_dx_max"])
+        if self._accum(L):
+            L.step_accum(dt)
+        else:
+            st = L.step(dt)
+            self.sdx[k] = max(self.sdx[k], st["s_over_dx_max"])
         self.steps[k] += 1
         self.updates += L.ncells
         # the step wrote interior cells only: bring the new buffer's ghost ring to the new state's time before the finer level's
@@ -598,10 +620,15 @@ class Hierarchy:
         """one step of level 1 (and everything above it); returns the next dt of level 1"""
         self.sdx = [0.0] * len(self.levels)
         self.alpha_now[0] = 1.0
+        for L in self.levels:
+            if self._accum(L):
+                L.stats_reset()
         self._advance(0, dt, 1.0, self.t)
         self.t += dt
         if len(self.ratios) > 0 and self.steps[0] % self.wl.regrid_interval == 0:
             self._regrid(0)
+        for k, L in enumerate(self.levels):
+            self._harvest(k, L)
         m, R = 0.0, 1
         for k in range(len(self.sdx)):
             R = R * (self.ratios[k - 1] if k > 0 else 1)

@@ -175,6 +175,12 @@ int gc_level_step(gc_level *L, double dt, gc_step_stats *out);
  * capturable. */
 int gc_level_step_auto(gc_level *L, double *dt_dev, double cfl_target);
 int gc_level_stats(const gc_level *, gc_step_stats *out /*HOST*/);
+/* For the subcycled levels of the AMR recursion, whose steps the host has no reason to wait for one by one:
+ * gc_level_step_accum is gc_level_step(L, dt, NULL) with dt > 0 WITHOUT zeroing the level's statistics first, so that over a run of
+ * steps s_over_dx_max becomes their maximum (exact: a max of bit images), n_clipped and clipped_mass their sums, nan_seen their
+ * OR; gc_level_stats reads them (and waits), gc_level_stats_reset zeroes them (no wait).  cfl_max is not formed (0). */
+int gc_level_step_accum(gc_level *L, double dt);
+int gc_level_stats_reset(gc_level *L);
 /* The same level step by the UNSPLIT wave-propagation method with transverse Riemann solves -- "the original GeoClaw ... with the
  * unsplit algorithm" that the paper simplifies to dimensional splitting and validates against (DESIGN.md 3.13,
  * reading S-21): every edge's fluctuations and limited correction flux from Q^n, each edge's vectors A-dQ + F~ and A+dQ - F~ split

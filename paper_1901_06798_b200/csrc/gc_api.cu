@@ -335,7 +335,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
         rrange[(size_t)p] = make_int2((int)first, (int)(rects.size() - first));
         if (need_mask) {   // in-domain ghost cells without a same-level source come from the coarser level (A3)
             for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < P.nx + 4; i++) {
-                if (i >= 2 && i < P.nx + 2 && j >= 2 && j < P.ny + 2) continue;
+                if (i == 2 && j >= 2 && j < P.ny + 2) i = P.nx + 2;              // the ghost ring only: skip the row's interior
                 int64_t gi = (int64_t)P.i0 + i - 2, gj = (int64_t)P.j0 + j - 2;
                 if (gi < 0 || gi >= nxl || gj < 0 || gj >= nyl) continue;
                 if (mask[(size_t)j * D.pitch + i]) continue;
@@ -627,6 +627,23 @@ extern "C" int gc_level_step(gc_level *L, double dt, gc_step_stats *out)
         if (out->nan_seen) return gc_fail(L->ctx, GC_ERR_NAN, "gc_level_step: NaN in the updated state");
     }
     return GC_OK;
+}
+
+extern "C" int gc_level_stats_reset(gc_level *L)
+{
+    if (!L) return GC_ERR_BADARG;
+    gc_launch_stats_reset(L);
+    return gc_cuda_check(L->ctx, "gc_level_stats_reset");
+}
+
+extern "C" int gc_level_step_accum(gc_level *L, double dt)
+{
+    if (!L || !(dt > 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step_accum: bad argument");
+    gc_launch_sweeps(L, dt, nullptr, 1);
+    L->cur = 1 - L->cur;
+    int rc = gc_flux_after_step(L, dt, nullptr);
+    if (rc) return rc;
+    return gc_cuda_check(L->ctx, "gc_level_step_accum");
 }
 
 extern "C" int gc_level_step_unsplit(gc_level *L, double dt, gc_step_stats *out)

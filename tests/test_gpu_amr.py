@@ -233,3 +233,30 @@ def test_flux_fixup_requires_attach_and_nesting_errors(gc):
         F.fill_ghost(C, 1.0)
     with pytest.raises(RuntimeError):
         C.average_down_from(F)
+
+
+def test_step_accum_leaves_the_maximum_and_the_sums_of_a_run_of_steps(gc):
+    """gc_level_step_accum / gc_level_stats_reset (the subcycled levels of the recursion are not waited for step by step): same state
+    as gc_level_step, and the statistics read afterwards are the maximum (s_over_dx_max), the sums (n_clipped, clipped_mass) and the
+    OR (nan_seen) of the steps since the reset"""
+    wl = workloads.cfg2(96)
+    La = driver.setup_level(gc.Context(**wl.params), wl, patches=workloads.tile(96, 96, 32))
+    Lb = driver.setup_level(gc.Context(**wl.params), wl, patches=workloads.tile(96, 96, 32))
+    La.fill_ghost(None, 1.0)
+    dt = 0.8 / La.step(0.0)["s_over_dx_max"]
+    Lb.fill_ghost(None, 1.0); Lb.step(0.0)
+    Lb.stats_reset()
+    assert Lb.stats()["s_over_dx_max"] == 0.0
+    sd, nc, cm = [], 0, 0.0
+    for k in range(30):
+        La.fill_ghost(None, 1.0); Lb.fill_ghost(None, 1.0)
+        st = La.step(dt)
+        Lb.step_accum(dt)
+        sd.append(st["s_over_dx_max"]); nc += st["n_clipped"]; cm += st["clipped_mass"]
+    sb = Lb.stats()
+    assert sb["s_over_dx_max"] == max(sd) and max(sd) > min(sd) and sb["n_clipped"] == nc and sb["nan_seen"] == 0
+    assert abs(sb["clipped_mass"] - cm) <= 1e-12 * abs(cm) + 1e-300
+    for f in ("h", "hu", "hv"):
+        assert np.array_equal(La.get_global(f), Lb.get_global(f))
+    Lb.stats_reset()
+    assert Lb.stats()["s_over_dx_max"] == 0.0 and Lb.stats()["n_clipped"] == 0
