@@ -327,9 +327,16 @@ class Context:
         self._chk(lib().gc_ctx_set_option(self.h, int(key), C.c_int64(int(value))), "gc_ctx_set_option")
 
     def _alloc(self, nbytes, user):
+        # large requests are rounded up to one of eight size classes per octave (<= 12.5 % more): the levels of an AMR run are
+        # recreated at every regrid with slightly different sizes, and a request that misses torch's cache of freed blocks costs a
+        # cudaMalloc (5-100 ms, and a device synchronisation)
+        nbytes = int(nbytes)
+        if nbytes >= (1 << 20):
+            q = 1 << max(nbytes.bit_length() - 4, 21)
+            nbytes = (nbytes + q - 1) // q * q
         try:
             with self.torch.cuda.stream(self.stream):
-                t = self.torch.empty(int(nbytes), dtype=self.torch.uint8, device=self.device)
+                t = self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
         except Exception:
             return None
         self._bufs[t.data_ptr()] = t
