@@ -194,6 +194,14 @@ static void build_tiles(gc_level *L, std::vector<SweepTile> &xt, std::vector<Swe
 // `seg` cells whose boundaries are multiples of 4 cells, so that an x segment starts on a 32-byte boundary of its row
 static void build_lines(gc_level *L, int seg, std::vector<LineDesc> &xl, std::vector<LineDesc> &yl)
 {
+    {
+        size_t nx_ = 0, ny_ = 0;
+        for (const gc_patch &P : L->pat) {
+            nx_ += (size_t)(P.ny + 4) * (size_t)std::max(1, (P.nx + seg - 1) / seg);
+            ny_ += (size_t)P.nx * (size_t)std::max(1, (P.ny + seg - 1) / seg);
+        }
+        xl.reserve(nx_); yl.reserve(ny_);
+    }
     for (int p = 0; p < L->np; p++) {
         const gc_patch &P = L->pat[p];
         for (int dir = 0; dir < 2; dir++) {
@@ -274,14 +282,15 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     build_metric(L);
     L->d_kappa = upload(L, L->kappa); L->d_rdx = upload(L, L->rdx); L->d_rdy = upload(L, L->rdy); L->d_ey = upload(L, L->ey);
     L->d_pat = upload(L, L->hpat);
-    std::vector<SweepTile> xt, yt;
-    build_tiles(L, xt, yt);
-    L->nxt = (int)xt.size(); L->nyt = (int)yt.size();
-    L->d_xt = upload(L, xt); L->d_yt = upload(L, yt);
-    {   // sweep kernel family: marching lines for large levels, edge-parallel tiles for small ones (gc_ctx_set_option overrides)
+    {   // sweep kernel family: marching lines for large levels, edge-parallel tiles for small ones (gc_ctx_set_option overrides);
+        // only the family's own work list is built
         L->use_march = L->ncells >= (int64_t)GC_MARCH_MIN_CELLS;
         if (ctx->opt_family == 1) L->use_march = 0;
         if (ctx->opt_family == 2) L->use_march = 1;
+        std::vector<SweepTile> xt, yt;
+        if (!L->use_march) build_tiles(L, xt, yt);
+        L->nxt = (int)xt.size(); L->nyt = (int)yt.size();
+        L->d_xt = upload(L, xt); L->d_yt = upload(L, yt);
         int seg = (int)std::min<int64_t>(128, std::max<int64_t>(16, (L->ncells / 400000 + 3) / 4 * 4));
         if (ctx->opt_seg >= 4) seg = ctx->opt_seg / 4 * 4;
         std::vector<LineDesc> xl, yl;

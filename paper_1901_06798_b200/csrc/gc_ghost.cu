@@ -44,12 +44,16 @@ __global__ void __launch_bounds__(256, 5) k_copy_rects(const CopyRect *rects, co
             r.w = __shfl_sync(0xffffffffu, mine.w, i); r.h = __shfl_sync(0xffffffffu, mine.h, i);
             r.dpitch = __shfl_sync(0xffffffffu, mine.dpitch, i); r.spitch = __shfl_sync(0xffffffffu, mine.spitch, i);
             if (r.w >= 32) {                                               // (row pair, 32-column chunk) items dealt round the patch's warps
-                const int nxc = (r.w + 31) >> 5, nit = nxc * ((r.h + 1) >> 1);
-                for (int q = sub; q < nit; q += wpp) {
-                    const int yp = q / nxc, x = (q - yp * nxc) * 32 + lane, y = 2 * yp;
+                const int nxc = (r.w + 31) >> 5;
+                int y = 0, xc = sub;                                       // item sub, sub + wpp, ...: no division
+                while (xc >= nxc) { xc -= nxc; y += 2; }
+                while (y < r.h) {
+                    const int x = xc * 32 + lane;
                     if (x < r.w)
                         copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
                                       r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, y + 1 < r.h);
+                    xc += wpp;
+                    while (xc >= nxc) { xc -= nxc; y += 2; }
                 }
             } else {
                 int rpp, ly, lx;                                           // rows per pass; this lane's row and column in a pass
