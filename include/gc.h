@@ -188,6 +188,19 @@ int gc_level_stats_reset(gc_level *L);
  * Same arguments, statistics and dt = 0 probe as gc_level_step.  Flux registers (gc_flux_attach) are defined for the split step
  * only: GC_ERR_STATE on a level that has any.  First use allocates 18 planes of scratch (released with the level). */
 int gc_level_step_unsplit(gc_level *L, double dt, gc_step_stats *out);
+/* The same step for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * identical arithmetic and results, but the 18 scratch planes live in a file-scope device array inside the library instead of
+ * being allocated at the level's first unsplit step.  The entry point calls no cudaMalloc / cudaFree and no allocator callback.
+ * Limit: the level's storage cells (every patch's (nx + 4 rounded up to a multiple of 4) x (ny + 4), summed) must not exceed
+ * GC_UNS_STATIC_MAX_CELLS, else GC_ERR_BADARG and nothing changes; gc_unsplit_static_max_cells() returns the limit.  The array
+ * (18 x GC_UNS_STATIC_MAX_CELLS doubles = 37.75 MB) is held by every GPU that loads the library until the process exits.  Its
+ * address is resolved once per device at gc_ctx_create (GC_ERR_CUDA here if that failed).  All calls on a device share the array,
+ * which keeps the last call's contents (nothing in it has to start at zero: every value used is written by the same call first):
+ * calls that overlap on the GPU -- other streams, other contexts -- race; calls on one stream do not.  out as for gc_level_step
+ * (NULL: no synchronisation). */
+#define GC_UNS_STATIC_MAX_CELLS (1 << 18)
+int gc_level_step_unsplit_static(gc_level *L, double dt, gc_step_stats *out);
+int64_t gc_unsplit_static_max_cells(void);
 
 /* wet mask (h > dry_tol) of the current state: one byte per interior cell, patch after patch, row-major. */
 int gc_wet_mask(const gc_level *, uint8_t *mask, int is_device);

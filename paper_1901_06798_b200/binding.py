@@ -19,7 +19,7 @@ SYMBOLS = [
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
     "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update", "gc_level_fallback_counts", "gc_level_step_unsplit",
-    "gc_level_step_accum", "gc_level_stats_reset",
+    "gc_level_step_accum", "gc_level_stats_reset", "gc_level_step_unsplit_static", "gc_unsplit_static_max_cells",
 ]
 
 
@@ -84,6 +84,8 @@ def lib():
     L.gc_level_step_auto.argtypes = [vp, vp, d]
     L.gc_level_step_unsplit.argtypes = [vp, d, vp]
     L.gc_level_step_accum.argtypes = [vp, d]
+    L.gc_level_step_unsplit_static.argtypes = [vp, d, vp]
+    L.gc_unsplit_static_max_cells.argtypes = []; L.gc_unsplit_static_max_cells.restype = C.c_int64
     L.gc_level_stats_reset.argtypes = [vp]
     L.gc_level_stats.argtypes = [vp, vp]
     L.gc_wet_mask.argtypes = [vp, vp, i]
@@ -187,6 +189,17 @@ class Level:
 
     def stats_reset(self):
         self.ctx._chk(lib().gc_level_stats_reset(self.h), "gc_level_stats_reset")
+
+    def step_unsplit_static(self, dt, sync=True):
+        """gc_level_step_unsplit_static: the unsplit step with its scratch in the library's static device array (allocates nothing;
+        levels of at most gc_unsplit_static_max_cells() storage cells)"""
+        if not sync:
+            self.ctx._chk(lib().gc_level_step_unsplit_static(self.h, dt, None), "gc_level_step_unsplit_static")
+            return None
+        st = StepStats()
+        self.ctx._chk(lib().gc_level_step_unsplit_static(self.h, dt, C.byref(st)), "gc_level_step_unsplit_static")
+        return dict(cfl_max=st.cfl_max, s_over_dx_max=st.s_over_dx_max, clipped_mass=st.clipped_mass,
+                    n_clipped=st.n_clipped, nan_seen=st.nan_seen)
 
     def step_unsplit(self, dt):
         """gc_level_step_unsplit: one unsplit level step with transverse Riemann solves"""

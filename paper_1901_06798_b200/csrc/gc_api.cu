@@ -65,6 +65,7 @@ extern "C" int gc_ctx_create(const gc_params *P, void *stream, gc_alloc_fn alloc
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return GC_ERR_CUDA; }   // no CPU fallback
     gc_ctx *c = new gc_ctx();
     c->P = *P; c->stream = (cudaStream_t)stream; c->alloc = alloc; c->free_ = free_; c->user = user;
+    gc_unsplit_static_setup();        // gc_level_step_unsplit_static: address of its scratch array, once per device (a failure is reported there)
     *out = c;
     return GC_OK;
 }

@@ -180,6 +180,7 @@ void gc_launch_math_selftest(cudaStream_t s, const double *a, const double *b, i
 void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, int threads);
 // gc_unsplit.cu
 int gc_launch_unsplit(gc_level *L, double dt, int write_out);
+void gc_unsplit_static_setup(void);   // resolves the static scratch array's device address on the current device (once per device)
 // gc_ghost.cu
 void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);
 void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int is_state);

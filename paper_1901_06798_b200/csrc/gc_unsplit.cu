@@ -16,6 +16,8 @@
 //                 in registers, the right- and left-going parts reach the neighbour columns by warp shuffles; G~' of the lower
 //                 edge, F~' of the left edge (the right one from the next lane), then the update of cell r-1, clean-up, friction.
 // Every expression in the order of the specification (bit-identical to the oracle, tests/test_gpu_unsplit.py).
+#include <mutex>
+#include <string>
 #include "gc_internal.h"
 #include "gc_scheme.cuh"
 
@@ -425,20 +427,15 @@ __global__ void __launch_bounds__(32 * UNS_UPD_WARPS) k_uns_update(UnsArgs a)
     }
 }
 
-int gc_launch_unsplit(gc_level *L, double dt, int write_out)
+// the three launches of one unsplit step with the 18 scratch planes at T (plane stride L->tot doubles)
+static void uns_run(gc_level *L, double dt, int write_out, double *T)
 {
     const gc_params &P = L->ctx->P;
-    if (!L->d_uns) {                                            // 18 planes of scratch, allocated at the first unsplit step
-        L->d_uns = (double *)gc_dev_alloc(L->ctx, (size_t)18 * (size_t)L->tot * sizeof(double));
-        if (!L->d_uns) return GC_ERR_NOMEM;
-        L->allocs.push_back(L->d_uns);
-    }
-    if (L->np == 0) return GC_OK;
     const int cur = L->cur, nxt = 1 - cur;
     UnsArgs a;
     a.pat = L->d_pat; a.h = L->q[cur][0]; a.hu = L->q[cur][1]; a.hv = L->q[cur][2]; a.b = L->b;
     a.oh = L->q[nxt][0]; a.ohu = L->q[nxt][1]; a.ohv = L->q[nxt][2];
-    a.T = L->d_uns; a.tot = L->tot;
+    a.T = T; a.tot = L->tot;
     a.rdx = L->d_rdx; a.rdy = L->d_rdy; a.ey = L->d_ey; a.kappa = L->d_kappa;
     a.ex = L->ex; a.g = P.g; a.eps = P.dry_tol; a.dt = dt; a.dxdy = L->dx * L->dy;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out;
@@ -457,5 +454,81 @@ int gc_launch_unsplit(gc_level *L, double dt, int write_out)
     { ProfScope ps(L->ctx, GC_SLOT_FUSED); const size_t sm = UNS_UPD_WARPS * UNS_RING_DOUBLES * sizeof(double);
       if (P.coord == 1) k_uns_update<1><<<gu, 32 * UNS_UPD_WARPS, sm, L->ctx->stream>>>(a);
       else k_uns_update<0><<<gu, 32 * UNS_UPD_WARPS, sm, L->ctx->stream>>>(a); }
+}
+
+int gc_launch_unsplit(gc_level *L, double dt, int write_out)
+{
+    if (!L->d_uns) {                                            // 18 planes of scratch, allocated at the first unsplit step
+        L->d_uns = (double *)gc_dev_alloc(L->ctx, (size_t)18 * (size_t)L->tot * sizeof(double));
+        if (!L->d_uns) return GC_ERR_NOMEM;
+        L->allocs.push_back(L->d_uns);
+    }
+    if (L->np == 0) return GC_OK;
+    uns_run(L, dt, write_out, L->d_uns);
+    return GC_OK;
+}
+
+// ---- gc_level_step_unsplit_static: the same step for callers that may not allocate (CUDA graph capture, serving loops) ------
+// The 18 scratch planes live in a file-scope device array of GC_UNS_STATIC_MAX_CELLS storage cells per plane (gc.h): 37.75 MB that
+// every GPU which loads the library holds until the process exits.  In host code `g_uns_static` is a host-side stand-in, not a
+// device address; the address is resolved with cudaGetSymbolAddress once per device, with that device current (at gc_ctx_create;
+// here, should the device not have seen one), and that pointer goes to the kernels.  Nothing in the array has to start at zero:
+// every value k_uns_update uses was written by the two edge kernels of the same call (what it reads beyond that -- the x-edge
+// planes of column 1, the y-edge planes of row 1 -- feeds halo lanes and rows whose results are discarded), so the previous call's
+// contents do no harm.  Every call on a device shares the array: calls that overlap on the GPU (two streams, two contexts) race.
+static __device__ __align__(256) double g_uns_static[(size_t)18 * GC_UNS_STATIC_MAX_CELLS];
+
+#define GC_UNS_MAX_DEV 64
+static double *g_uns_static_addr[GC_UNS_MAX_DEV];       // per device: the array's device address, resolved once
+static cudaError_t g_uns_static_rc[GC_UNS_MAX_DEV];
+static bool g_uns_static_tried[GC_UNS_MAX_DEV];
+static std::mutex g_uns_static_mx;
+
+// resolves the array's address on the CURRENT device; returns it, or nullptr (the CUDA error kept for the entry point's message)
+static double *uns_static_resolve(cudaError_t *rc_out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= GC_UNS_MAX_DEV) { cudaGetLastError(); if (rc_out) *rc_out = e != cudaSuccess ? e : cudaErrorInvalidDevice; return nullptr; }
+    std::lock_guard<std::mutex> lk(g_uns_static_mx);
+    if (!g_uns_static_tried[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_uns_static);
+        if (e != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+        g_uns_static_addr[dev] = (double *)p; g_uns_static_rc[dev] = e; g_uns_static_tried[dev] = true;
+    }
+    if (rc_out) *rc_out = g_uns_static_rc[dev];
+    return g_uns_static_addr[dev];
+}
+
+void gc_unsplit_static_setup(void) { uns_static_resolve(nullptr); }   // gc_ctx_create: set-up time, the context's device current
+
+extern "C" int64_t gc_unsplit_static_max_cells(void) { return (int64_t)GC_UNS_STATIC_MAX_CELLS; }
+
+extern "C" int gc_level_step_unsplit_static(gc_level *L, double dt, gc_step_stats *out)
+{
+    if (!L || !(dt >= 0.0)) return gc_fail(L ? L->ctx : nullptr, GC_ERR_BADARG, "gc_level_step_unsplit_static: bad argument");
+    if (L->reg_fine || L->reg_coarse)
+        return gc_fail(L->ctx, GC_ERR_STATE, "gc_level_step_unsplit_static: flux registers are defined for the split step only");
+    if (L->tot > (int64_t)GC_UNS_STATIC_MAX_CELLS)
+        return gc_fail(L->ctx, GC_ERR_BADARG, "gc_level_step_unsplit_static: level larger than GC_UNS_STATIC_MAX_CELLS storage cells "
+                                              "(patch cells incl. ghost cells and row padding); use gc_level_step_unsplit");
+    cudaError_t e = cudaSuccess;
+    double *T = uns_static_resolve(&e);
+    if (!T) {
+        L->ctx->err = std::string("gc_level_step_unsplit_static: cudaGetSymbolAddress of the static scratch failed: ") + cudaGetErrorString(e);
+        return GC_ERR_CUDA;
+    }
+    gc_launch_stats_reset(L);
+    if (L->np > 0) uns_run(L, dt, dt > 0.0 ? 1 : 0, T);
+    if (dt > 0.0) L->cur = 1 - L->cur;
+    int rc = gc_cuda_check(L->ctx, "gc_level_step_unsplit_static");
+    if (rc) return rc;
+    if (out) {
+        rc = gc_level_stats(L, out);
+        if (rc) return rc;
+        out->cfl_max = dt * out->s_over_dx_max;
+        if (out->nan_seen) return gc_fail(L->ctx, GC_ERR_NAN, "gc_level_step_unsplit_static: NaN in the updated state");
+    }
     return GC_OK;
 }
