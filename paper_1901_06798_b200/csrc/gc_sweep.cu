@@ -279,6 +279,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
 
+#pragma unroll 2
     for (int r = 0; r <= nst_warp; r++) {
         const bool live = r < nst;
         // ---- cell r arrives; the next group is requested
