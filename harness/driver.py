@@ -601,8 +601,11 @@ class Hierarchy:
         self.steps[k] += 1
         self.updates += L.ncells
         # the step wrote interior cells only: bring the new buffer's ghost ring to the new state's time before the finer level's
-        # substeps read it as slope neighbours on patch seams; alpha_now[k] is that time as a fraction
-        L.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
+        # substeps read it as slope neighbours on patch seams; alpha_now[k] is that time as a fraction.  The finest
+        # level has no such reader: its ring is next read by its own next step, whose fill rewrites it (and a regrid that puts a
+        # level on top of it fills first), so the fill is left out there -- same numbers, a fifth of that level's launches
+        if k + 1 < len(self.levels):
+            L.fill_ghost(self.levels[k - 1] if k > 0 else None, self.alpha_now[k])
         if k + 1 < len(self.levels):
             r = self.ratios[k]
             for s in range(r):
