@@ -206,6 +206,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-tilings", action="store_true", help="skip config.tilings (sides 16 ... 256)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end legs")
+    ap.add_argument("--no-chains", action="store_true", help="marching lines stop at every patch boundary (GC_OPT_CHAINS = 1): same bits")
     ap.add_argument("--scheme", default="split", choices=("split", "unsplit"),
                     help="split: the paper's dimensionally split step (the headline); unsplit: the step with transverse Riemann solves "
                          "(DESIGN.md 3.13; fixed dt, no tilings / e2e legs)")
@@ -236,6 +237,8 @@ def main():
     wl = workloads.cfg5(n)
     if args.manning > 0.0:
         wl.params = dict(wl.params, manning_n=args.manning)
+    if args.no_chains:
+        binding.DEFAULT_OPTIONS[binding.OPT_CHAINS] = 1
     ctx = binding.Context(device=dev, **wl.params)
     fields = host_fields(wl, n)
 

@@ -97,8 +97,9 @@ const char *gc_last_error(const gc_ctx *);
 /* Tuning knobs; none changes a result bit (all sweep kernel families compute the same bits).  Read when a level
  * is created.  GC_OPT_SWEEP_FAMILY: 0 = by level size (default), 1 = edge-parallel tiles, 2 = line marching.
  * GC_OPT_MARCH_SEG: cells per marching segment, 4..4096 (rounded down to a multiple of 4); 0 = by level size (default).
+ * GC_OPT_CHAINS: 0 = marching lines run through same-level patches that continue each other (default), 1 = every patch on its own.
  * Unknown key or value out of range: GC_ERR_BADARG, nothing changes. */
-enum { GC_OPT_SWEEP_FAMILY = 0, GC_OPT_MARCH_SEG = 1 };
+enum { GC_OPT_SWEEP_FAMILY = 0, GC_OPT_MARCH_SEG = 1, GC_OPT_CHAINS = 2 };
 int gc_ctx_set_option(gc_ctx *, int key, int64_t value);
 
 /* A1: one level = one device pool with all its patches, a patch-descriptor table,

@@ -291,7 +291,7 @@ class Level:
         self.ctx._chk(lib().gc_flux_fixup(self.h, fine.h), "gc_flux_fixup")
 
 
-OPT_SWEEP_FAMILY, OPT_MARCH_SEG = 0, 1          # gc_ctx_set_option keys (include/gc.h)
+OPT_SWEEP_FAMILY, OPT_MARCH_SEG, OPT_CHAINS = 0, 1, 2          # gc_ctx_set_option keys (include/gc.h)
 SWEEP_AUTO, SWEEP_EDGE, SWEEP_MARCH = 0, 1, 2
 DEFAULT_OPTIONS = {}                            # applied to every new Context (tests select a sweep kernel family here)
 
@@ -336,7 +336,7 @@ class Context:
             canvas[j0:j0 + block.shape[0], i0:i0 + block.shape[1]].copy_(self.torch.from_numpy(np.ascontiguousarray(block)))
 
     def set_option(self, key, value):
-        """gc_ctx_set_option: tuning knobs that change no result bit (OPT_SWEEP_FAMILY, OPT_MARCH_SEG); read at level creation."""
+        """gc_ctx_set_option: tuning knobs that change no result bit (OPT_SWEEP_FAMILY, OPT_MARCH_SEG, OPT_CHAINS); read at level creation."""
         self._chk(lib().gc_ctx_set_option(self.h, int(key), C.c_int64(int(value))), "gc_ctx_set_option")
 
     def _alloc(self, nbytes, user):

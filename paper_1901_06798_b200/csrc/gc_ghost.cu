@@ -24,8 +24,25 @@ __device__ __forceinline__ void copy_pair(double *f0, double *f1, double *f2, in
     if (two) { f0[d1] = b0; if (NF > 1) { f1[d1] = b1; f2[d1] = b2; } }
 }
 
+__device__ __forceinline__ CopyRect rect_from_lane(const CopyRect &mine, int i)
+{
+    CopyRect r;
+    r.dst = __shfl_sync(0xffffffffu, mine.dst, i); r.src = __shfl_sync(0xffffffffu, mine.src, i);
+    r.w = __shfl_sync(0xffffffffu, mine.w, i); r.h = __shfl_sync(0xffffffffu, mine.h, i);
+    r.dpitch = __shfl_sync(0xffffffffu, mine.dpitch, i); r.spitch = __shfl_sync(0xffffffffu, mine.spitch, i);
+    return r;
+}
+// lane -> (row, column) inside one pass over a rectangle narrower than 32 cells; rpp = rows per pass (0: a wide rectangle)
+__device__ __forceinline__ void narrow_map(int w, int lane, int &rpp, int &ly, int &lx)
+{
+    if (w == 2) { rpp = 16; ly = lane >> 1; lx = lane & 1; }                     // x faces, corners: no division
+    else if (w == 16) { rpp = 2; ly = lane >> 4; lx = lane & 15; }
+    else if (w < 32) { rpp = 32 / w; ly = lane / w; lx = lane - ly * w; }
+    else { rpp = 0; ly = 0; lx = 0; }
+}
+
 template <int NF>
-__global__ void __launch_bounds__(256, 5) k_copy_rects(const CopyRect *rects, const int2 *range, int np, int wpp, double *f0, double *f1, double *f2)
+__global__ void __launch_bounds__(256, 2) k_copy_rects(const CopyRect *rects, const int2 *range, int np, int wpp, double *f0, double *f1, double *f2)
 {
     const int gw = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5);
     const int lane = threadIdx.x & 31;
@@ -38,33 +55,61 @@ __global__ void __launch_bounds__(256, 5) k_copy_rects(const CopyRect *rects, co
         CopyRect mine; mine.dst = 0; mine.src = 0; mine.w = 0; mine.h = 0; mine.dpitch = 0; mine.spitch = 0;
         if (i0 + lane < pr.y) mine = rects[pr.x + i0 + lane];
         const int cnt = min(32, pr.y - i0);
-        for (int i = 0; i < cnt; i++) {
-            CopyRect r;
-            r.dst = __shfl_sync(0xffffffffu, mine.dst, i); r.src = __shfl_sync(0xffffffffu, mine.src, i);
-            r.w = __shfl_sync(0xffffffffu, mine.w, i); r.h = __shfl_sync(0xffffffffu, mine.h, i);
-            r.dpitch = __shfl_sync(0xffffffffu, mine.dpitch, i); r.spitch = __shfl_sync(0xffffffffu, mine.spitch, i);
-            if (r.w >= 32) {                                               // (row pair, 32-column chunk) items dealt round the patch's warps
-                const int nxc = (r.w + 31) >> 5;
-                int y = 0, xc = sub;                                       // item sub, sub + wpp, ...: no division
-                while (xc >= nxc) { xc -= nxc; y += 2; }
-                while (y < r.h) {
-                    const int x = xc * 32 + lane;
-                    if (x < r.w)
-                        copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
-                                      r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, y + 1 < r.h);
-                    xc += wpp;
-                    while (xc >= nxc) { xc -= nxc; y += 2; }
+        for (int i = 0; i < cnt; i += 4) {
+            // Narrow rectangles (faces and corners of small patches) four at a time: the first two passes of each -- all of it
+            // for a patch of side <= 32 -- are loaded before anything is stored, 24 loads in flight per lane.  One rectangle
+            // after the other left a warp waiting one DRAM round trip per rectangle (side 16: 8 of them per patch).
+            int64_t da[4], sa[4], db[4], sb[4];
+            bool va[4], vb[4];
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const CopyRect r = rect_from_lane(mine, min(i + k, cnt - 1));      // past the end: the last one again, masked out
+                int rpp, ly, lx;
+                narrow_map(r.w, lane, rpp, ly, lx);
+                const int y = 2 * sub * rpp + ly;
+                va[k] = (i + k < cnt) & (ly < rpp) & (y < r.h);
+                vb[k] = va[k] & (y + rpp < r.h);
+                da[k] = r.dst + (int64_t)y * r.dpitch + lx; sa[k] = r.src + (int64_t)y * r.spitch + lx;
+                db[k] = da[k] + (int64_t)rpp * r.dpitch; sb[k] = sa[k] + (int64_t)rpp * r.spitch;
+            }
+            double a[4][3], b[4][3];
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                a[k][0] = va[k] ? __ldg(f0 + sa[k]) : 0.0; b[k][0] = vb[k] ? __ldg(f0 + sb[k]) : 0.0;
+                if (NF > 1) {
+                    a[k][1] = va[k] ? __ldg(f1 + sa[k]) : 0.0; a[k][2] = va[k] ? __ldg(f2 + sa[k]) : 0.0;
+                    b[k][1] = vb[k] ? __ldg(f1 + sb[k]) : 0.0; b[k][2] = vb[k] ? __ldg(f2 + sb[k]) : 0.0;
                 }
-            } else {
-                int rpp, ly, lx;                                           // rows per pass; this lane's row and column in a pass
-                if (r.w == 2) { rpp = 16; ly = lane >> 1; lx = lane & 1; }                 // x faces, corners: no division
-                else if (r.w == 16) { rpp = 2; ly = lane >> 4; lx = lane & 15; }
-                else { rpp = 32 / r.w; ly = lane / r.w; lx = lane - ly * r.w; }
-                if (ly < rpp) {
-                    for (int y = 2 * sub * rpp + ly; y < r.h; y += 2 * wpp * rpp) {
-                        const bool two = y + rpp < r.h;
-                        copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + lx, r.src + (int64_t)y * r.spitch + lx,
-                                      r.dst + (int64_t)(y + rpp) * r.dpitch + lx, r.src + (int64_t)(y + rpp) * r.spitch + lx, two);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                if (va[k]) { f0[da[k]] = a[k][0]; if (NF > 1) { f1[da[k]] = a[k][1]; f2[da[k]] = a[k][2]; } }
+                if (vb[k]) { f0[db[k]] = b[k][0]; if (NF > 1) { f1[db[k]] = b[k][1]; f2[db[k]] = b[k][2]; } }
+            }
+            // what is left: the later passes of a tall narrow rectangle, and the wide rectangles
+            for (int k = 0; k < 4 && i + k < cnt; k++) {
+                const CopyRect r = rect_from_lane(mine, i + k);
+                if (r.w >= 32) {                                           // (row pair, 32-column chunk) items dealt round the patch's warps
+                    const int nxc = (r.w + 31) >> 5;
+                    int y = 0, xc = sub;                                   // item sub, sub + wpp, ...: no division
+                    while (xc >= nxc) { xc -= nxc; y += 2; }
+                    while (y < r.h) {
+                        const int x = xc * 32 + lane;
+                        if (x < r.w)
+                            copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + x, r.src + (int64_t)y * r.spitch + x,
+                                          r.dst + (int64_t)(y + 1) * r.dpitch + x, r.src + (int64_t)(y + 1) * r.spitch + x, y + 1 < r.h);
+                        xc += wpp;
+                        while (xc >= nxc) { xc -= nxc; y += 2; }
+                    }
+                } else {
+                    int rpp, ly, lx;
+                    narrow_map(r.w, lane, rpp, ly, lx);
+                    if (ly < rpp) {
+                        for (int y = 2 * (sub + wpp) * rpp + ly; y < r.h; y += 2 * wpp * rpp) {
+                            const bool two = y + rpp < r.h;
+                            copy_pair<NF>(f0, f1, f2, r.dst + (int64_t)y * r.dpitch + lx, r.src + (int64_t)y * r.spitch + lx,
+                                          r.dst + (int64_t)(y + rpp) * r.dpitch + lx, r.src + (int64_t)(y + rpp) * r.spitch + lx, two);
+                        }
                     }
                 }
             }

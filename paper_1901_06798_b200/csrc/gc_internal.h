@@ -14,9 +14,9 @@
 // patch descriptor as the kernels see it (A1): interior box, element offset of the patch in a field plane, row pitch
 struct PatchDesc {
     int32_t i0, j0, nx, ny;
-    int64_t off;     // element offset in every field plane of the pool
+    int64_t off;     // element offset in every field plane of the pool; off % 4 == 2: storage column 2 of every row starts a 32-byte sector
     int64_t ioff;    // offset in interior-packed arrays (masks, flags)
-    int32_t pitch;   // row pitch in elements: nx + 4 rounded up to a multiple of 4 (32-byte aligned rows)
+    int32_t pitch;   // row pitch in elements: nx + 4 rounded up to a multiple of 4
     int32_t bcmask;  // bit0 touches xlo, bit1 xhi, bit2 ylo, bit3 yhi
 };
 
@@ -29,8 +29,23 @@ struct SweepTile {
 
 // work item of a marching sweep kernel: ONE thread walks cells [c0-2, c0+nc+2) of a line (row for x, column for y),
 // solving edges c0-1 .. c0+nc+1 and updating cells c0 .. c0+nc-1 (storage indices along the sweep)
+// With chains (below) c0 counts positions along the chain and `patch` is the piece holding position c0 - 2.
 struct LineDesc {
     int32_t patch, line, c0, nc;
+};
+
+// Chains: same-level patches that continue each other along a sweep direction (x: equal j0, ny, side by side; y: equal i0, nx,
+// stacked) are walked by the marching kernels as ONE line, each piece's interior read and written in that patch's own storage --
+// the redundant edges and ghost cells of a patch boundary are paid once per segment instead of once per patch, which is what
+// small patches cost (DESIGN.md 5 "chains").  Position s along a chain = (interior cells of the pieces before
+// the patch) + storage index inside the patch; a position of piece p on line l sits at A + l * pitch + s (x) or A + s * pitch + l
+// (y) in a field plane.  One link per patch and direction; a patch outside any chain is a chain of one (A = off, end = INT_MAX).
+struct ChainLink {
+    int64_t A;          // plane offset of position 0 of line 0, extrapolated back from this piece
+    int32_t end;        // first position of the next piece (= this piece's position of storage index n + 2), INT_MAX in the last piece
+    int32_t next;       // patch index of the next piece, -1 in the last one
+    int32_t pitch;      // row pitch of this piece
+    int32_t org;        // y chains: j0 of the chain's head (global row + 2 of position s is org + s); x chains: j0
 };
 
 // same-level ghost copy: rectangle of w x h cells
@@ -91,7 +106,7 @@ struct gc_ctx {
     void *user;
     std::string err;
     bool prof = false;
-    int opt_family = 0, opt_seg = 0;                 // gc_ctx_set_option: sweep kernel family (0 auto, 1 edge, 2 march), marching segment length
+    int opt_family = 0, opt_seg = 0, opt_chains = 0;                 // gc_ctx_set_option: sweep kernel family (0 auto, 1 edge, 2 march), marching segment length
     void *stage = nullptr; size_t stage_bytes = 0;   // grow-only device staging buffer of the host-pointer paths (gc_stage_get)
     unsigned long long launches = 0;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];
@@ -129,6 +144,9 @@ struct gc_level {
     double *d_kappa, *d_rdx, *d_rdy, *d_ey;
     SweepTile *d_xt, *d_yt; int nxt, nyt;            // edge-parallel tiles (small levels)
     LineDesc *d_xl, *d_yl; int64_t nxl_lines, nyl_lines;   // marching lines (large levels)
+    // chains of patches along x / y (one link per patch); x lines without the ghost rows no y line reads (their patch continues
+    // above / below inside a y chain) -- used when no flux register reads Q* there; chained: 1 = some chain has two pieces
+    ChainLink *d_xlink = nullptr, *d_ylink = nullptr; LineDesc *d_xl_red = nullptr; int64_t nxl_red = 0; int chained = 0;
     int use_march;
     CopyRect *d_copy; int ncopy;                     // same-level copy rectangles, grouped by destination patch
     int2 *d_copy_range; int copy_wpp;               // per patch: (first rectangle, count); warps serving one patch

@@ -26,6 +26,7 @@ struct SweepArgs {
     const PatchDesc *pat;
     const SweepTile *tiles;
     const LineDesc *lines; int64_t nlines;
+    const ChainLink *links;          // marching kernels with chains: one link per patch for this sweep direction
     const double *h, *hu, *hv, *b;   // input planes
     double *oh, *ohu, *ohv;          // output planes
     const double *rd;                // rdx (x-sweep) or rdy (y-sweep), per global row (+2)
@@ -195,7 +196,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
 //   y-sweep: 15-22 ring of the last 4 cells, (h, p) (t, rd) each; 23-26 the next row, 8 bytes per plane and stage (cp.async.ca)
 //   x-sweep: 15-30 four stages of 2 cells x 4 planes (one 16-byte cp.async.cg each): in flight, current, and the two before it
 //            (cell r-3 is read back from them); 31-36 the new values of 4 cells x 3 planes, written to the row with one 256-bit
-//            store per plane (a thread's row accesses touch one sector per lane whatever their width, so wide ones are cheap).
+//            store per plane, one whole sector (a thread's row accesses touch one sector per lane whatever their width).
 #ifndef PARK_MINB
 #define PARK_MINB 3
 #endif
@@ -207,6 +208,7 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
 #define PK_XOUT 31
 #define PARK_BYTES_X ((PK_XOUT + 6) * PK_SL)
 #define PARK_BYTES_Y ((PK_YSTAGE + 4) * PK_SL)
+#define PARK_BYTES_YCH ((PK_YSTAGE + 8) * PK_SL)   // chained variant: four stages, rows requested two ahead
 
 __device__ __forceinline__ void sts2(unsigned addr, double x, double y)
 {
@@ -241,7 +243,10 @@ __device__ __forceinline__ void cpa8(unsigned sdst, const double *gsrc)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(sdst), "l"(gsrc) : "memory");
 }
 
-template <int DIR, int SPH>
+// CH = 1: lines may run through several patches of a chain (gc_internal.h).  Cell r of the line sits at B + r * str, B the base
+// of the piece holding it: Bc for r >= rb (the piece the input has reached), Bp before it (pieces have >= 8 cells, the output runs
+// 5 cells behind the input, so two bases are enough).  The input moves to the next piece when the cell it requests reaches re.
+template <int DIR, int SPH, int CH>
 __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 {
     extern __shared__ __align__(16) double dsm[];
@@ -259,9 +264,20 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
     int64_t base; int64_t str;
     if (DIR == 0) { base = pd.off + (int64_t)ln.line * pd.pitch + cfirst; str = 1; }
     else          { base = pd.off + (int64_t)cfirst * pd.pitch + ln.line; str = pd.pitch; }
+    int jorg = pd.j0;
+    int64_t Bp = 0; int rb = -0x40000000, re = 0x7fffffff, lnext = -1;   // chains: previous piece's base, first r of this piece, of the next, next patch
+    if (CH) {
+        const int4 *lp = reinterpret_cast<const int4 *>(a.links + ln.patch);
+        const int4 v0 = lp[0], v1 = lp[1];
+        const int64_t A = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x);
+        re = v0.z - cfirst; lnext = v0.w;                        // INT_MAX - cfirst stays far beyond any line (cfirst >= 0)
+        if (DIR == 0) base = A + (int64_t)ln.line * v1.x + cfirst;
+        else { base = A + (int64_t)cfirst * v1.x + ln.line; jorg = v1.y; }
+        Bp = base;
+    }
     const bool count = (DIR == 1) || (ln.line >= 2 && ln.line < pd.ny + 2);   // eq. 15 over interior lines only
     const double rdrow = (DIR == 0 && active) ? a.rd[pd.j0 + ln.line] : 0.0;
-    const int jrow = pd.j0 + cfirst;                             // y-sweep: global row (+2) of the first cell read
+    const int jrow = jorg + cfirst;                              // y-sweep: global row (+2) of the first cell read
     const bool mc = a.limiter != 0;
 
 #pragma unroll
@@ -278,6 +294,21 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         else          { cpa8(st0, a.h + base); cpa8(st0 + PK_SL / 2, a.hv + base); cpa8(st0 + 2 * (PK_SL / 2), a.hu + base); cpa8(st0 + 3 * (PK_SL / 2), a.b + base); }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
+    if (DIR == 1 && CH) {                                        // chained y-sweep: rows are requested two ahead (a line through small
+        if (nst > 1) {                                           // patches jumps from patch to patch, and the loads it waits for with it)
+            if (1 >= re) {                                       // cell 0 was the last one of its piece
+                const int4 *lp = reinterpret_cast<const int4 *>(a.links + lnext);
+                const int4 v0 = lp[0], v1 = lp[1];
+                Bp = base; rb = re;
+                base = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x) + (int64_t)cfirst * v1.x + ln.line;
+                re = v0.z - cfirst; lnext = v0.w;
+            }
+            const unsigned sd = st0 + 4 * (PK_SL / 2);
+            const int64_t o = base + str;
+            cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
 
 #pragma unroll 2
     for (int r = 0; r <= nst_warp; r++) {
@@ -288,6 +319,13 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             if ((r & 1) == 0) {
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
                 if (r + 2 < nst) {
+                    if (CH && r + 2 >= re) {                                             // the input enters the next piece of the chain
+                        const int4 *lp = reinterpret_cast<const int4 *>(a.links + lnext);
+                        const int4 v0 = lp[0], v1 = lp[1];
+                        Bp = base; rb = re;
+                        base = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x) + (int64_t)ln.line * v1.x + cfirst;
+                        re = v0.z - cfirst; lnext = v0.w;
+                    }
                     const unsigned sd = st0 + (((r >> 1) + 1) & 3) * (4 * PK_SL);
                     const int64_t o = base + r + 2;
                     cpa16(sd, a.h + o); cpa16(sd + PK_SL, a.hu + o); cpa16(sd + 2 * PK_SL, a.hv + o); cpa16(sd + 3 * PK_SL, a.b + o);
@@ -296,7 +334,7 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             }
             const unsigned sa = st0 + ((r >> 1) & 3) * (4 * PK_SL) + (r & 1) * 8u;
             qh = lds1(sa); qp = lds1(sa + PK_SL); qt = lds1(sa + 2 * PK_SL); qb = lds1(sa + 3 * PK_SL);
-        } else {
+        } else if (!CH) {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             if (r + 1 < nst) {
                 const unsigned sd = st0 + ((r + 1) & 1) * (4 * (PK_SL / 2));
@@ -305,6 +343,23 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
             const unsigned sa = st0 + (r & 1) * (4 * (PK_SL / 2));
+            qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
+        } else {
+            asm volatile("cp.async.wait_group 1;" ::: "memory");                         // all but the newest group: cell r is here
+            if (r + 2 < nst) {
+                if (r + 2 >= re) {                                                       // the input enters the next piece of the chain
+                    const int4 *lp = reinterpret_cast<const int4 *>(a.links + lnext);
+                    const int4 v0 = lp[0], v1 = lp[1];
+                    Bp = base; rb = re;
+                    base = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x) + (int64_t)cfirst * v1.x + ln.line;
+                    re = v0.z - cfirst; lnext = v0.w;
+                }
+                const unsigned sd = st0 + ((r + 2) & 3) * (4 * (PK_SL / 2));
+                const int64_t o = base + (int64_t)(r + 2) * str;
+                cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            const unsigned sa = st0 + (r & 3) * (4 * (PK_SL / 2));
             qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
         }
         double rd0 = rdrow, ef = a.ex;
@@ -396,23 +451,19 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             double up = __fma_rn(-dtdx, fm[1] - fpp[1], q3p);
             double ut = __fma_rn(-dtdx, fm[2] - fpp[2], q3t);
             const int j = r - 3;
-            const int64_t o = base + (int64_t)j * str;
+            const int64_t o = ((CH && j < rb) ? Bp : base) + (int64_t)j * str;
             if (DIR == 0) {
-                // cell j of the row goes to slot (plane, (j >> 1) & 1); a full aligned group of 4 leaves as one store
+                // cell j of the row goes to slot (plane, (j >> 1) & 1).  Cells 4m+2 .. 4m+5 of the line are one 32-byte sector of the
+                // row (a patch's storage column 2 starts a sector, segments and chain pieces start at columns = 2 mod 4) and leave
+                // as one store: cells 4m+2, 4m+3 wait in slot 1, cells 4m+4, 4m+5 in slot 0.  A group never spans two pieces.
                 const unsigned so = sm0 + (PK_XOUT + ((j >> 1) & 1)) * PK_SL + (j & 1) * 8u;
                 sts1(so, uh); sts1(so + 2 * PK_SL, up); sts1(so + 4 * PK_SL, ut);
-                if ((j & 3) == 3) {
+                if ((j & 3) == 1) {
                     const unsigned sf = sm0 + PK_XOUT * PK_SL;
                     double x0, x1, x2, x3;
-                    if (j == 3) {                                                        // cells 0, 1 of the first group are not ours
-                        lds2(sf + PK_SL, x2, x3); stg2(a.oh + o - 1, x2, x3);
-                        lds2(sf + 3 * PK_SL, x2, x3); stg2(a.ohu + o - 1, x2, x3);
-                        lds2(sf + 5 * PK_SL, x2, x3); stg2(a.ohv + o - 1, x2, x3);
-                    } else {
-                        lds2(sf, x0, x1); lds2(sf + PK_SL, x2, x3); stg4(a.oh + o - 3, x0, x1, x2, x3);
-                        lds2(sf + 2 * PK_SL, x0, x1); lds2(sf + 3 * PK_SL, x2, x3); stg4(a.ohu + o - 3, x0, x1, x2, x3);
-                        lds2(sf + 4 * PK_SL, x0, x1); lds2(sf + 5 * PK_SL, x2, x3); stg4(a.ohv + o - 3, x0, x1, x2, x3);
-                    }
+                    lds2(sf + PK_SL, x0, x1); lds2(sf, x2, x3); stg4(a.oh + o - 3, x0, x1, x2, x3);
+                    lds2(sf + 3 * PK_SL, x0, x1); lds2(sf + 2 * PK_SL, x2, x3); stg4(a.ohu + o - 3, x0, x1, x2, x3);
+                    lds2(sf + 5 * PK_SL, x0, x1); lds2(sf + 4 * PK_SL, x2, x3); stg4(a.ohv + o - 3, x0, x1, x2, x3);
                 }
             } else {
                 if (uh < a.eps && a.write_out) {                                        // dry clean-up (S-9)
@@ -434,10 +485,11 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
 
     if (DIR == 0 && nst >= 5) {                                  // x-sweep: the cells of the last, incomplete group
         const int jl = nst - 3;
-        if ((jl & 3) != 3) {
-            for (int j = (jl & ~3) < 2 ? 2 : (jl & ~3); j <= jl; j++) {
+        if ((jl & 3) != 1) {
+            for (int j = ((jl - 2) & ~3) + 2; j <= jl; j++) {
                 const unsigned so = sm0 + (PK_XOUT + ((j >> 1) & 1)) * PK_SL + (j & 1) * 8u;
-                a.oh[base + j] = lds1(so); a.ohu[base + j] = lds1(so + 2 * PK_SL); a.ohv[base + j] = lds1(so + 4 * PK_SL);
+                const int64_t o = ((CH && j < rb) ? Bp : base) + j;
+                a.oh[o] = lds1(so); a.ohu[o] = lds1(so + 2 * PK_SL); a.ohv[o] = lds1(so + 4 * PK_SL);
             }
         }
     }
@@ -471,15 +523,22 @@ template <int DIR>
 static void launch_march(gc_level *L, const SweepArgs &a, unsigned nb)
 {
     static bool attr_done = false;
+    const int bytes = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_Y;
+    const int bytes_ch = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_YCH;
     if (!attr_done) {
-        const int bytes = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_Y;
-        cudaFuncSetAttribute(k_marchp<DIR, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-        cudaFuncSetAttribute(k_marchp<DIR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        cudaFuncSetAttribute(k_marchp<DIR, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        cudaFuncSetAttribute(k_marchp<DIR, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        cudaFuncSetAttribute(k_marchp<DIR, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_ch);
+        cudaFuncSetAttribute(k_marchp<DIR, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_ch);
         attr_done = true;
     }
-    const size_t bytes = DIR == 0 ? PARK_BYTES_X : PARK_BYTES_Y;
-    if (a.coord == 1) k_marchp<DIR, 1><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
-    else k_marchp<DIR, 0><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
+    if (L->chained) {
+        if (a.coord == 1) k_marchp<DIR, 1, 1><<<nb, MARCH_BLOCK, bytes_ch, L->ctx->stream>>>(a);
+        else k_marchp<DIR, 0, 1><<<nb, MARCH_BLOCK, bytes_ch, L->ctx->stream>>>(a);
+    } else {
+        if (a.coord == 1) k_marchp<DIR, 1, 0><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
+        else k_marchp<DIR, 0, 0><<<nb, MARCH_BLOCK, bytes, L->ctx->stream>>>(a);
+    }
 }
 
 void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_out)
@@ -492,13 +551,16 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     a.hlo = (P.g >= 0x1p-20 && P.g <= 0x1p20) ? (P.dry_tol > 0x1p-100 ? P.dry_tol : 0x1p-100) : INFINITY;
     a.coord = P.coord; a.limiter = P.limiter; a.write_out = write_out; a.stats = L->d_stats;
     a.gn2 = P.g * (P.manning_n * P.manning_n); a.fdepth = P.friction_depth; a.friction = P.manning_n > 0.0 ? 1 : 0;
-    a.lines = nullptr; a.nlines = 0;
+    a.lines = nullptr; a.nlines = 0; a.links = nullptr;
     a.ex = L->ex; a.ey = L->d_ey; a.dxdy = L->dx * L->dy; a.kappa = L->d_kappa; a.b = L->b;
     // x-sweep: Q^n -> Q*
     a.tiles = L->d_xt; a.h = L->q[cur][0]; a.hu = L->q[cur][1]; a.hv = L->q[cur][2];
     a.oh = L->qs[0]; a.ohu = L->qs[1]; a.ohv = L->qs[2]; a.rd = L->d_rdx;
     if (L->use_march) {
-        a.lines = L->d_xl; a.nlines = L->nxl_lines;
+        // ghost rows whose patch continues inside a y chain are read by no y line; a flux register may still read Q* there
+        const bool regs = (L->nreg > 0 && L->reg_fine) || L->reg_coarse;
+        a.lines = L->d_xl; a.nlines = L->nxl_lines; a.links = L->d_xlink;
+        if (!regs && L->nxl_red > 0) { a.lines = L->d_xl_red; a.nlines = L->nxl_red; }
         if (a.nlines > 0) {
             ProfScope ps(L->ctx, GC_SLOT_XSWEEP);
             launch_march<0>(L, a, (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK));
@@ -508,7 +570,7 @@ void gc_launch_sweeps(gc_level *L, double dt, const double *dt_dev, int write_ou
     a.tiles = L->d_yt; a.h = L->qs[0]; a.hu = L->qs[1]; a.hv = L->qs[2];
     a.oh = L->q[nxt][0]; a.ohu = L->q[nxt][1]; a.ohv = L->q[nxt][2]; a.rd = L->d_rdy;
     if (L->use_march) {
-        a.lines = L->d_yl; a.nlines = L->nyl_lines;
+        a.lines = L->d_yl; a.nlines = L->nyl_lines; a.links = L->d_ylink;
         if (a.nlines > 0) {
             ProfScope ps(L->ctx, GC_SLOT_YSWEEP);
             launch_march<1>(L, a, (unsigned)((a.nlines + MARCH_BLOCK - 1) / MARCH_BLOCK));
