@@ -4,7 +4,8 @@ one spherical level of NxN cells (default 8192 x 8192, 0.5 arcmin) tiled into sq
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--side S] [--n NCELLS] [--impl reference]
 
-A "step" = gc_fill_ghost + gc_level_step_auto (dt chain on the device, no host sync) over the whole level.
+A "step" = gc_fill_ghost_step + gc_level_step_auto (dt chain on the device, no host sync) over the whole level
+(gc_fill_ghost_step = gc_fill_ghost without the same-level copies the step does not read; --full-fill: gc_fill_ghost).
 metric  = fp64 cell updates/s (interior cells x steps / device time, CUDA events, max over ranks).
 config.tilings = the same step on the five tilings BASELINE.json's configs[4] names (sides 16 ... 256), each with its updates/s,
           HBM GB/s at 56 B per update and fp64-pipe slot fraction (N = 1 only).
@@ -206,7 +207,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-tilings", action="store_true", help="skip config.tilings (sides 16 ... 256)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end legs")
+    ap.add_argument("--full-fill", action="store_true", help="gc_fill_ghost (every ghost cell) instead of gc_fill_ghost_step before each step")
     ap.add_argument("--no-chains", action="store_true", help="marching lines stop at every patch boundary (GC_OPT_CHAINS = 1): same bits")
+    ap.add_argument("--chain-max", type=int, default=0, help="GC_OPT_CHAINS = k: patches of k cells or more are not chained")
     ap.add_argument("--scheme", default="split", choices=("split", "unsplit"),
                     help="split: the paper's dimensionally split step (the headline); unsplit: the step with transverse Riemann solves "
                          "(DESIGN.md 3.13; fixed dt, no tilings / e2e legs)")
@@ -239,6 +242,8 @@ def main():
         wl.params = dict(wl.params, manning_n=args.manning)
     if args.no_chains:
         binding.DEFAULT_OPTIONS[binding.OPT_CHAINS] = 1
+    elif args.chain_max >= 8:
+        binding.DEFAULT_OPTIONS[binding.OPT_CHAINS] = args.chain_max
     ctx = binding.Context(device=dev, **wl.params)
     fields = host_fields(wl, n)
 
@@ -251,7 +256,7 @@ def main():
         L.fill_ghost_b()
         return L
 
-    def timed(L, K, warm, use_dist=True):
+    def timed(L, K, warm, use_dist=True, full_fill=False):
         d = dist if use_dist else None
         dt0 = driver.probe_dt(L, wl.cfl)
         dt_dev = torch.tensor([dt0], dtype=torch.float64, device=dev)
@@ -264,8 +269,15 @@ def main():
             series = torch.empty((max(K, warm, 1), args.gauges, 4), dtype=torch.float64, device=dev)
             torch.cuda.synchronize()
 
+        # gc_fill_ghost_step: the ghost cells the split step reads (where marching lines run through chained patches the copy
+        # between them is dead work; same bits); gauges and the unsplit step read other ghost cells: gc_fill_ghost
+        step_fill = not (full_fill or args.full_fill or unsplit or series is not None)
+
         def one_step(k):
-            L.fill_ghost(None, 1.0)
+            if step_fill:
+                L.fill_ghost_step(None, 1.0)
+            else:
+                L.fill_ghost(None, 1.0)
             if series is not None:
                 L.gauges_sample_into(series[k])      # one record per step, straight into the device-resident series
             if unsplit:
@@ -384,9 +396,12 @@ def main():
                     L.destroy(); L = None
                 Ls = make(side)
                 m, _, pr = timed(Ls, args.steps, W, use_dist=False)
+                if not args.full_fill and not args.no_chains:      # chained sides: the same with every ghost cell filled
+                    mf = timed(Ls, args.steps, W, use_dist=False, full_fill=True)[0]
                 Ls.destroy()
             rate = cells * args.steps / (m * 1e-3)
             tilings[str(side)] = {"updates_per_s": rate, "ms_per_step": m / args.steps,
+                                  "ms_per_step_full_fill": (mf if side != args.side and not args.full_fill and not args.no_chains else m) / args.steps,
                                   "hbm_gbs_at_56B": BYTES_PER_UPDATE * rate / 1e9, "hbm_frac": BYTES_PER_UPDATE * rate / 1e9 / hbm_peak,
                                   "fp64_pipe_slot_frac": slot_fraction(side, rate),
                                   "kernel_ms_per_step": {k: v[0] / args.steps for k, v in pr.items() if v[1]}}

@@ -97,7 +97,8 @@ const char *gc_last_error(const gc_ctx *);
 /* Tuning knobs; none changes a result bit (all sweep kernel families compute the same bits).  Read when a level
  * is created.  GC_OPT_SWEEP_FAMILY: 0 = by level size (default), 1 = edge-parallel tiles, 2 = line marching.
  * GC_OPT_MARCH_SEG: cells per marching segment, 4..4096 (rounded down to a multiple of 4); 0 = by level size (default).
- * GC_OPT_CHAINS: 0 = marching lines run through same-level patches that continue each other (default), 1 = every patch on its own.
+ * GC_OPT_CHAINS: 0 = marching lines run through same-level patches that continue each other (default), 1 = every patch on its own,
+ * k >= 8 = patches of k cells or more along the sweep stay on their own.
  * Unknown key or value out of range: GC_ERR_BADARG, nothing changes. */
 enum { GC_OPT_SWEEP_FAMILY = 0, GC_OPT_MARCH_SEG = 1, GC_OPT_CHAINS = 2 };
 int gc_ctx_set_option(gc_ctx *, int key, int64_t value);
@@ -149,6 +150,14 @@ int gc_level_download_state_async(gc_level *L, double *const host[3] /*HOST, pin
  * gc_fill_ghost_b does same-level copy + physical boundary for the bathymetry (once per regrid). */
 int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha);
 int gc_fill_ghost_b(gc_level *L);
+/* The same, for a caller whose NEXT call on L is a split step (gc_level_step, gc_level_step_auto, gc_level_step_accum): it fills
+ * the ghost cells that step reads and may leave the others as they are.  Where same-level patches continue each other, the
+ * marching sweeps read the neighbour's interior directly (chains) and the copy into the ghost cells between them is
+ * dead work -- on a regular tiling of small patches, all of it.  The step's result is bit-identical to the one after
+ * gc_fill_ghost.  Anything else that reads ghost cells (gc_level_get_field, gc_flag_cells, gc_gauges_sample, a finer level's
+ * gc_fill_ghost or gc_level_init_from, gc_level_step_unsplit) needs gc_fill_ghost.  Levels without chains, or with flux
+ * registers attached, get the full fill. */
+int gc_fill_ghost_step(gc_level *L, const gc_level *coarser, double alpha);
 
 /* Time-dependent bathymetry B(x, y, t) (the seafloor-deformation source that starts both of the paper's tsunamis, P:273
  * "deformation information on uniform grids", "ground deformation file", reading S-20).  dz: vertical

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libgeoclaw_b200.so")
 
 SYMBOLS = [
     "gc_ctx_create", "gc_ctx_destroy", "gc_last_error", "gc_level_create", "gc_level_destroy", "gc_level_ncells",
-    "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost",
+    "gc_level_set_field", "gc_level_get_field", "gc_level_set_global", "gc_level_get_global", "gc_fill_ghost", "gc_fill_ghost_step",
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
@@ -76,6 +76,7 @@ def lib():
     L.gc_level_set_global.argtypes = [vp, i, vp, i, i64, i64, i64, i64, i64]
     L.gc_level_get_global.argtypes = [vp, i, i, vp, i, i64, i64, i64, i64, i64]
     L.gc_fill_ghost.argtypes = [vp, vp, d]
+    L.gc_fill_ghost_step.argtypes = [vp, vp, d]
     L.gc_fill_ghost_b.argtypes = [vp]
     L.gc_level_set_patches.argtypes = [vp, i, vp, i]
     L.gc_gauges_bind.argtypes = [vp, i, vp, vp]
@@ -173,6 +174,10 @@ class Level:
 
     def fill_ghost(self, coarser=None, alpha=1.0):
         self.ctx._chk(lib().gc_fill_ghost(self.h, coarser.h if coarser is not None else None, alpha), "gc_fill_ghost")
+
+    def fill_ghost_step(self, coarser=None, alpha=1.0):
+        """gc_fill_ghost_step: the ghost cells the next split step reads (the rest may stay stale); same result of that step"""
+        self.ctx._chk(lib().gc_fill_ghost_step(self.h, coarser.h if coarser is not None else None, alpha), "gc_fill_ghost_step")
 
     def step(self, dt, sync=True):
         if not sync:

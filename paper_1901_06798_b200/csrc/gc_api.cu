@@ -80,7 +80,7 @@ extern "C" int gc_ctx_set_option(gc_ctx *c, int key, int64_t value)
 {
     if (!c) return GC_ERR_BADARG;
     if (key == GC_OPT_SWEEP_FAMILY && value >= 0 && value <= 2) { c->opt_family = (int)value; return GC_OK; }
-    if (key == GC_OPT_CHAINS && value >= 0 && value <= 1) { c->opt_chains = (int)value; return GC_OK; }
+    if (key == GC_OPT_CHAINS && (value == 0 || value == 1 || (value >= 8 && value <= 1000000))) { c->opt_chains = (int)value; return GC_OK; }
     if (key == GC_OPT_MARCH_SEG && (value == 0 || (value >= 4 && value <= 4096))) { c->opt_seg = (int)value; return GC_OK; }
     return gc_fail(c, GC_ERR_BADARG, "gc_ctx_set_option: unknown key or value out of range");
 }
@@ -196,21 +196,20 @@ static void build_tiles(gc_level *L, std::vector<SweepTile> &xt, std::vector<Swe
 // the same extent across the sweep and starts where the other ends.  Pieces shorter than 8 cells are not chained (the kernels keep
 // the bases of two pieces only, and the output runs 5 cells behind the input); along x every piece but the last must be a multiple
 // of 4 cells long so that the 16-byte loads and the 32-byte stores of the x-sweep keep their alignment across pieces.
-// Pieces of GC_CHAIN_MAX_PIECE cells or more stay on their own: a segment is at most 128 cells long, so there is next to nothing
-// to save, and the chained kernel variant costs about 1 % (measured at side 128 and 256; side 64 gains 3 %, side 16 25 %).
-#define GC_CHAIN_MAX_PIECE 128
+// GC_OPT_CHAINS = k >= 8 keeps pieces of k cells or more on their own (measurements).
 static void build_chains(gc_level *L, int dir, std::vector<int32_t> &succ, std::vector<int32_t> &pred)
 {
     succ.assign((size_t)std::max(L->np, 1), -1); pred.assign((size_t)std::max(L->np, 1), -1);
     if (L->ctx->opt_chains == 1) return;
+    const int maxp = L->ctx->opt_chains >= 8 ? L->ctx->opt_chains : 2147483647;
     for (int p = 0; p < L->np; p++) {
         const gc_patch &P = L->pat[p];
         const int n = dir == 0 ? P.nx : P.ny;
-        if (n < 8 || n >= GC_CHAIN_MAX_PIECE || (dir == 0 && n % 4 != 0)) continue;
+        if (n < 8 || n >= maxp || (dir == 0 && n % 4 != 0)) continue;
         const int q = dir == 0 ? gc_find_patch_host(L, (int64_t)P.i0 + P.nx, P.j0) : gc_find_patch_host(L, P.i0, (int64_t)P.j0 + P.ny);
         if (q < 0) continue;
         const gc_patch &Q = L->pat[q];
-        if ((dir == 0 ? Q.nx : Q.ny) < 8 || (dir == 0 ? Q.nx : Q.ny) >= GC_CHAIN_MAX_PIECE) continue;
+        if ((dir == 0 ? Q.nx : Q.ny) < 8 || (dir == 0 ? Q.nx : Q.ny) >= maxp) continue;
         const bool fits = dir == 0 ? (Q.i0 == P.i0 + P.nx && Q.j0 == P.j0 && Q.ny == P.ny) : (Q.j0 == P.j0 + P.ny && Q.i0 == P.i0 && Q.nx == P.nx);
         if (!fits) continue;
         succ[(size_t)p] = q; pred[(size_t)q] = p;
@@ -220,8 +219,11 @@ static void build_chains(gc_level *L, int dir, std::vector<int32_t> &succ, std::
 // marching lines (k_marchp): every row (x) / interior column (y) of every chain of patches, cut into balanced segments of about
 // `seg` cells whose boundaries are multiples of 4 cells, so that an x segment starts on a 32-byte boundary of its row.
 // xl_red: the x lines without the ghost rows that no y line reads (patches continued inside a y chain on that side).
+// need[p]: which parts of patch p's ghost ring some line reads -- bit 0 the left ghost columns (p heads its x chain), bit 1 the right
+// ones (p ends it), bit 2 the bottom ghost rows (some piece of p's x chain has no patch below in its y chain, so the chain's ghost
+// rows are swept), bit 3 the top ones.  Everything else is reached through the neighbour's interior (gc_fill_ghost_step).
 static void build_lines(gc_level *L, int seg, std::vector<LineDesc> &xl, std::vector<LineDesc> &yl, std::vector<LineDesc> &xl_red,
-                        std::vector<ChainLink> &xlink, std::vector<ChainLink> &ylink)
+                        std::vector<ChainLink> &xlink, std::vector<ChainLink> &ylink, std::vector<uint8_t> &need)
 {
     std::vector<int32_t> succ[2], pred[2];
     build_chains(L, 0, succ[0], pred[0]); build_chains(L, 1, succ[1], pred[1]);
@@ -250,6 +252,9 @@ static void build_lines(gc_level *L, int seg, std::vector<LineDesc> &xl, std::ve
                 if (dir == 0) { lo_ghost |= pred[1][(size_t)p] < 0; hi_ghost |= succ[1][(size_t)p] < 0; }
             }
             if (piece.size() > 1) L->chained = 1;
+            if (dir == 0)
+                for (size_t k = 0; k < piece.size(); k++)
+                    need[(size_t)piece[k]] = (uint8_t)((k == 0 ? 1 : 0) | (k + 1 == piece.size() ? 2 : 0) | (lo_ghost ? 4 : 0) | (hi_ghost ? 8 : 0));
             for (size_t k = 0; k < piece.size(); k++) {
                 const PatchDesc &D = L->hpat[(size_t)piece[k]];
                 ChainLink &K = link[(size_t)piece[k]];
@@ -349,6 +354,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     L->b = L->pool + 6 * plane;
     for (int f = 0; f < 3; f++) L->qs[f] = L->pool + (int64_t)(7 + f) * plane;
 
+    std::vector<uint8_t> need((size_t)std::max(np, 1), 15);   // parts of each ghost ring a sweep reads (build_lines): all of it unless chained
     build_metric(L);
     L->d_kappa = upload(L, L->kappa); L->d_rdx = upload(L, L->rdx); L->d_rdy = upload(L, L->rdy); L->d_ey = upload(L, L->ey);
     L->d_pat = upload(L, L->hpat);
@@ -365,7 +371,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
         if (ctx->opt_seg >= 4) seg = ctx->opt_seg / 4 * 4;
         std::vector<LineDesc> xl, yl, xl_red;
         std::vector<ChainLink> xlink, ylink;
-        if (L->use_march) build_lines(L, seg, xl, yl, xl_red, xlink, ylink);
+        if (L->use_march) build_lines(L, seg, xl, yl, xl_red, xlink, ylink, need);
         if (xl_red.size() == xl.size()) xl_red.clear();                  // nothing to leave out: one list
         L->nxl_lines = (int64_t)xl.size(); L->nyl_lines = (int64_t)yl.size(); L->nxl_red = (int64_t)xl_red.size();
         L->d_xl = upload(L, xl); L->d_yl = upload(L, yl); L->d_xl_red = upload(L, xl_red);
@@ -374,8 +380,8 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     }
 
     // same-level copy rectangles: grown box of p  x  interior of q (A2, incl. corners)
-    std::vector<CopyRect> rects;
-    std::vector<int2> rrange((size_t)std::max(np, 1));
+    std::vector<CopyRect> rects, rects_red;                   // all of them; the ones a split step reads (gc_fill_ghost_step)
+    std::vector<int2> rrange((size_t)std::max(np, 1)), rrange_red((size_t)std::max(np, 1));
     int64_t ghost_cells = 0;
     std::vector<int32_t> bcp;
     std::vector<uint8_t> mask;
@@ -386,7 +392,7 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
         int64_t gx0 = (int64_t)P.i0 - 2, gx1 = (int64_t)P.i0 + P.nx + 2, gy0 = (int64_t)P.j0 - 2, gy1 = (int64_t)P.j0 + P.ny + 2;
         bool need_mask = level > 1;
         if (need_mask) mask.assign((size_t)D.pitch * (P.ny + 4), 0);
-        size_t first = rects.size();
+        size_t first = rects.size(), first_red = rects_red.size();
         int64_t bx0 = std::max<int64_t>(gx0, 0) / L->bsize, bx1 = std::min<int64_t>(gx1 - 1, nxl - 1) / L->bsize;
         int64_t by0 = std::max<int64_t>(gy0, 0) / L->bsize, by1 = std::min<int64_t>(gy1 - 1, nyl - 1) / L->bsize;
         for (int64_t by = by0; by <= by1; by++) for (int64_t bx = bx0; bx <= bx1; bx++) {
@@ -409,12 +415,22 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
                 if (dup) continue;
                 rects.push_back(r);
                 ghost_cells += (int64_t)r.w * r.h;
+                {   // does a sweep line read any cell of it?  (storage coordinates of p; interior = columns 2..nx+1, rows 2..ny+1)
+                    const int64_t rx0 = x0 - P.i0 + 2, rx1 = x1 - P.i0 + 2, ry0 = y0 - P.j0 + 2, ry1 = y1 - P.j0 + 2;
+                    const uint8_t nd = need[(size_t)p];
+                    const bool sideL = rx0 < 2 && (nd & 1), sideR = rx1 > P.nx + 2 && (nd & 2);
+                    const bool cols_in = rx0 < P.nx + 2 && rx1 > 2, rows_in = ry0 < P.ny + 2 && ry1 > 2;
+                    const bool used = (rows_in && (sideL || sideR)) || (ry0 < 2 && (nd & 4) && (cols_in || sideL || sideR))
+                                      || (ry1 > P.ny + 2 && (nd & 8) && (cols_in || sideL || sideR));
+                    if (used) rects_red.push_back(r);
+                }
                 if (need_mask)
                     for (int64_t y = y0; y < y1; y++) for (int64_t x = x0; x < x1; x++)
                         mask[(size_t)(y - P.j0 + 2) * D.pitch + (x - P.i0 + 2)] = 1;
             }
         }
         rrange[(size_t)p] = make_int2((int)first, (int)(rects.size() - first));
+        rrange_red[(size_t)p] = make_int2((int)first_red, (int)(rects_red.size() - first_red));
         if (need_mask) {   // in-domain ghost cells without a same-level source come from the coarser level (A3)
             for (int j = 0; j < P.ny + 4; j++) for (int i = 0; i < P.nx + 4; i++) {
                 if (i == 2 && j >= 2 && j < P.ny + 2) i = P.nx + 2;              // the ghost ring only: skip the row's interior
@@ -428,6 +444,11 @@ extern "C" int gc_level_create(gc_ctx *ctx, int level, double xlo, double ylo, d
     }
     L->ncopy = (int)rects.size(); L->d_copy = upload(L, rects);
     L->d_copy_range = upload(L, rrange);
+    L->ncopy_red = -1;                                            // -1: every rectangle is read by the step, one list
+    if (rects_red.size() < rects.size()) {
+        L->ncopy_red = (int)rects_red.size(); L->d_copy_red = upload(L, rects_red); L->d_copy_range_red = upload(L, rrange_red);
+        if (!L->d_copy_red || !L->d_copy_range_red) L->ncopy_red = -1;
+    }
     {   // warps per patch: about 256 ghost cells per warp, at most 16
         const int64_t per = np > 0 ? ghost_cells / np : 0;
         L->copy_wpp = (int)std::min<int64_t>(16, std::max<int64_t>(1, per / 256));
@@ -623,7 +644,7 @@ extern "C" int gc_level_get_global(const gc_level *L, int field, int which, doub
 extern "C" int gc_fill_ghost_b(gc_level *L)
 {
     if (!L) return GC_ERR_BADARG;
-    gc_launch_copy_rects(L, L->b, nullptr, nullptr, 1);
+    gc_launch_copy_rects(L, L->b, nullptr, nullptr, 1, false);
     gc_launch_bc(L, L->b, nullptr, nullptr, 1, 0);
     return gc_cuda_check(L->ctx, "gc_fill_ghost_b");
 }
@@ -650,11 +671,14 @@ int gc_fill_coarse_ghosts(gc_level *L, const gc_level *C, double alpha);   // gc
 void gc_amr_on_destroy(gc_level *L);                                       // gc_api_amr.cu
 int gc_flux_after_step(gc_level *L, double dt, const double *dt_dev);     // gc_api_amr.cu
 
-extern "C" int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha)
+static int fill_ghost(gc_level *L, const gc_level *coarser, double alpha, bool for_step)
 {
     if (!L) return GC_ERR_BADARG;
     double **q = L->q[L->cur];
-    gc_launch_copy_rects(L, q[0], q[1], q[2], 3);
+    // for_step: only the rectangles a sweep line of the split step reads.  A flux register reads ghost cells of its own, and then
+    // the x-sweep takes every ghost row (gc_launch_sweeps): everything is filled.
+    const bool regs = (L->nreg > 0 && L->reg_fine) || L->reg_coarse;
+    gc_launch_copy_rects(L, q[0], q[1], q[2], 3, for_step && !regs);
     if (coarser) {
         int rc = gc_fill_coarse_ghosts(L, coarser, alpha);
         if (rc) return rc;
@@ -664,6 +688,9 @@ extern "C" int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha)
     gc_launch_bc(L, q[0], q[1], q[2], 3, 1);
     return gc_cuda_check(L->ctx, "gc_fill_ghost");
 }
+
+extern "C" int gc_fill_ghost(gc_level *L, const gc_level *coarser, double alpha) { return fill_ghost(L, coarser, alpha, false); }
+extern "C" int gc_fill_ghost_step(gc_level *L, const gc_level *coarser, double alpha) { return fill_ghost(L, coarser, alpha, true); }
 
 extern "C" int gc_level_stats(const gc_level *L, gc_step_stats *out)
 {

@@ -117,14 +117,17 @@ __global__ void __launch_bounds__(256, 2) k_copy_rects(const CopyRect *rects, co
     }
 }
 
-void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf)
+void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf, bool for_step)
 {
-    if (L->ncopy == 0) return;
+    const bool red = for_step && L->ncopy_red >= 0;
+    if ((red ? L->ncopy_red : L->ncopy) == 0) return;
+    const CopyRect *rects = red ? L->d_copy_red : L->d_copy;
+    const int2 *range = red ? L->d_copy_range_red : L->d_copy_range;
     const int threads = 256, wpp = L->copy_wpp;
     const int64_t blocks = ((int64_t)L->np * wpp * 32 + threads - 1) / threads;
     ProfScope ps(L->ctx, GC_SLOT_COPY);
-    if (nf > 1) k_copy_rects<3><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->d_copy_range, L->np, wpp, f0, f1, f2);
-    else k_copy_rects<1><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(L->d_copy, L->d_copy_range, L->np, wpp, f0, f1, f2);
+    if (nf > 1) k_copy_rects<3><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(rects, range, L->np, wpp, f0, f1, f2);
+    else k_copy_rects<1><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(rects, range, L->np, wpp, f0, f1, f2);
 }
 
 // ---- A4: physical boundary.  pass 0: x faces over rows inside the domain; pass 1: y faces over all columns.

@@ -150,6 +150,7 @@ struct gc_level {
     int use_march;
     CopyRect *d_copy; int ncopy;                     // same-level copy rectangles, grouped by destination patch
     int2 *d_copy_range; int copy_wpp;               // per patch: (first rectangle, count); warps serving one patch
+    CopyRect *d_copy_red = nullptr; int2 *d_copy_range_red = nullptr; int ncopy_red = -1;   // the rectangles a split step reads (gc_fill_ghost_step); -1: all
     int32_t *d_bcp; int nbcp;                       // patches touching the physical boundary
     std::vector<int64_t> coarse_ghost;              // plane offsets + global indices of ghosts to be filled from the coarser level
     std::vector<int32_t> coarse_ghost_ij;           // (gi, gj) pairs
@@ -200,7 +201,7 @@ void gc_launch_fp64_probe(cudaStream_t s, double *out, int iters, int blocks, in
 int gc_launch_unsplit(gc_level *L, double dt, int write_out);
 void gc_unsplit_static_setup(void);   // resolves the static scratch array's device address on the current device (once per device)
 // gc_ghost.cu
-void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf);
+void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int nf, bool for_step);
 void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int is_state);
 void gc_launch_set_patches(gc_level *L, double *plane, const int64_t *goff, const double *src);
 void gc_launch_set_global(gc_level *L, double *plane, const double *src, int64_t ld, int64_t gi0, int64_t gj0, int64_t gnx, int64_t gny);

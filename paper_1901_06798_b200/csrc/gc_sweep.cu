@@ -208,7 +208,6 @@ __global__ void __launch_bounds__(SW_BLOCK) k_sweep(SweepArgs a)
 #define PK_XOUT 31
 #define PARK_BYTES_X ((PK_XOUT + 6) * PK_SL)
 #define PARK_BYTES_Y ((PK_YSTAGE + 4) * PK_SL)
-#define PARK_BYTES_YCH ((PK_YSTAGE + 8) * PK_SL)   // chained variant: four stages, rows requested two ahead
 
 __device__ __forceinline__ void sts2(unsigned addr, double x, double y)
 {
@@ -294,22 +293,6 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
         else          { cpa8(st0, a.h + base); cpa8(st0 + PK_SL / 2, a.hv + base); cpa8(st0 + 2 * (PK_SL / 2), a.hu + base); cpa8(st0 + 3 * (PK_SL / 2), a.b + base); }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
-    if (DIR == 1 && CH) {                                        // chained y-sweep: rows are requested two ahead (a line through small
-        if (nst > 1) {                                           // patches jumps from patch to patch, and the loads it waits for with it)
-            if (1 >= re) {                                       // cell 0 was the last one of its piece
-                const int4 *lp = reinterpret_cast<const int4 *>(a.links + lnext);
-                const int4 v0 = lp[0], v1 = lp[1];
-                Bp = base; rb = re;
-                base = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x) + (int64_t)cfirst * v1.x + ln.line;
-                re = v0.z - cfirst; lnext = v0.w;
-            }
-            const unsigned sd = st0 + 4 * (PK_SL / 2);
-            const int64_t o = base + str;
-            cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    }
-
 #pragma unroll 2
     for (int r = 0; r <= nst_warp; r++) {
         const bool live = r < nst;
@@ -334,32 +317,22 @@ __global__ void __launch_bounds__(MARCH_BLOCK, PARK_MINB) k_marchp(SweepArgs a)
             }
             const unsigned sa = st0 + ((r >> 1) & 3) * (4 * PK_SL) + (r & 1) * 8u;
             qh = lds1(sa); qp = lds1(sa + PK_SL); qt = lds1(sa + 2 * PK_SL); qb = lds1(sa + 3 * PK_SL);
-        } else if (!CH) {
+        } else {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             if (r + 1 < nst) {
-                const unsigned sd = st0 + ((r + 1) & 1) * (4 * (PK_SL / 2));
-                const int64_t o = base + (int64_t)(r + 1) * str;
-                cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
-            }
-            asm volatile("cp.async.commit_group;" ::: "memory");
-            const unsigned sa = st0 + (r & 1) * (4 * (PK_SL / 2));
-            qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
-        } else {
-            asm volatile("cp.async.wait_group 1;" ::: "memory");                         // all but the newest group: cell r is here
-            if (r + 2 < nst) {
-                if (r + 2 >= re) {                                                       // the input enters the next piece of the chain
+                if (CH && r + 1 >= re) {                                                 // the input enters the next piece of the chain
                     const int4 *lp = reinterpret_cast<const int4 *>(a.links + lnext);
                     const int4 v0 = lp[0], v1 = lp[1];
                     Bp = base; rb = re;
                     base = (int64_t)(((unsigned long long)(unsigned)v0.y << 32) | (unsigned)v0.x) + (int64_t)cfirst * v1.x + ln.line;
                     re = v0.z - cfirst; lnext = v0.w;
                 }
-                const unsigned sd = st0 + ((r + 2) & 3) * (4 * (PK_SL / 2));
-                const int64_t o = base + (int64_t)(r + 2) * str;
+                const unsigned sd = st0 + ((r + 1) & 1) * (4 * (PK_SL / 2));
+                const int64_t o = base + (int64_t)(r + 1) * str;
                 cpa8(sd, a.h + o); cpa8(sd + PK_SL / 2, a.hv + o); cpa8(sd + 2 * (PK_SL / 2), a.hu + o); cpa8(sd + 3 * (PK_SL / 2), a.b + o);
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
-            const unsigned sa = st0 + (r & 3) * (4 * (PK_SL / 2));
+            const unsigned sa = st0 + (r & 1) * (4 * (PK_SL / 2));
             qh = lds1(sa); qp = lds1(sa + PK_SL / 2); qt = lds1(sa + 2 * (PK_SL / 2)); qb = lds1(sa + 3 * (PK_SL / 2));
         }
         double rd0 = rdrow, ef = a.ex;
@@ -524,7 +497,7 @@ static void launch_march(gc_level *L, const SweepArgs &a, unsigned nb)
 {
     static bool attr_done = false;
     const int bytes = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_Y;
-    const int bytes_ch = DIR == 0 ? (int)PARK_BYTES_X : (int)PARK_BYTES_YCH;
+    const int bytes_ch = bytes;
     if (!attr_done) {
         cudaFuncSetAttribute(k_marchp<DIR, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         cudaFuncSetAttribute(k_marchp<DIR, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);

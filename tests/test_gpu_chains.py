@@ -25,13 +25,15 @@ def grid(xs, ys):
     return np.array(out, dtype=np.int32)
 
 
-def run(gc, gco, wl, pats, nsteps, eta_scale, chains, seg):
+def run(gc, gco, wl, pats, nsteps, eta_scale, chains, seg, step_fill=False):
     from paper_1901_06798_b200 import binding
     cg = gc.Context(**wl.params)
     cg.set_option(binding.OPT_SWEEP_FAMILY, binding.SWEEP_MARCH)
     cg.set_option(binding.OPT_CHAINS, 0 if chains else 1)
     cg.set_option(binding.OPT_MARCH_SEG, seg)
     Lg = driver.setup_level(cg, wl, patches=pats)
+    if step_fill:                                   # gc_fill_ghost_step before every step: only what the step reads is filled
+        Lg.fill_ghost = Lg.fill_ghost_step
     Lo = driver.setup_level(gco.Context(**wl.params), wl)
     lockstep(Lg, Lo, nsteps, wl.cfl, eta_scale)
     return Lg
@@ -89,3 +91,47 @@ def test_chains_friction_and_first_order(gc, gco):
     wl = workloads.cfg2(48)
     wl.params = dict(wl.params, limiter=0)
     run(gc, gco, wl, workloads.tile(48, 48, 8), 25, 2.0, True, 20)
+
+
+@pytest.mark.parametrize("seg", [0, 12, 40])
+def test_fill_ghost_step_same_bits(gc, gco, seg):
+    """gc_fill_ghost_step leaves out the same-level copies no sweep line reads; the steps after it give the oracle's bits --
+    regular tilings (every same-level copy is dead), mixed sizes (chains end in the middle of the level), the L-shaped set."""
+    wl = workloads.cfg2(64)
+    wl.nx, wl.ny = sum(XS), sum(YS)
+    run(gc, gco, wl, grid(XS, YS), 25, 2.0, True, seg, step_fill=True)
+    wl = workloads.cfg2(48)
+    wl.params = dict(wl.params, bc=(1, 0, 0, 1))
+    for side in (8, 16):
+        run(gc, gco, wl, workloads.tile(48, 48, side), 25, 2.0, True, seg, step_fill=True)
+    pats = np.array([[0, 0, 16, 16], [16, 0, 16, 16], [32, 0, 16, 32], [0, 16, 32, 16], [0, 32, 16, 16], [16, 32, 32, 16]], dtype=np.int32)
+    run(gc, gco, wl, pats, 25, 2.0, True, seg, step_fill=True)
+    wl = workloads.cfg5(128)
+    run(gc, gco, wl, workloads.tile(128, 128, 16), 6, 1.0, True, seg, step_fill=True)
+
+
+def test_fill_ghost_step_poisoned_ghosts(gc, gco):
+    """the cells gc_fill_ghost_step does not fill are really not read: NaN in every ghost cell before each fill changes nothing"""
+    from paper_1901_06798_b200 import binding
+    n = 64
+    wl = workloads.cfg2(n)
+    cg = gc.Context(**wl.params)
+    cg.set_option(binding.OPT_SWEEP_FAMILY, binding.SWEEP_MARCH)
+    pats = workloads.tile(n, n, 16)
+    Lg = driver.setup_level(cg, wl, patches=pats)
+    Lo = driver.setup_level(gco.Context(**wl.params), wl)
+    dt = driver.probe_dt(Lo, wl.cfl)
+    for it in range(12):
+        for p in range(len(pats)):
+            for f in ("h", "hu", "hv"):
+                a = Lg.get_field(p, f)
+                keep = a[2:-2, 2:-2].copy()
+                a[:] = np.nan
+                a[2:-2, 2:-2] = keep
+                Lg.set_field(p, f, a)
+        Lg.fill_ghost_step(None, 1.0); Lo.fill_ghost(None, 1.0)
+        sg = Lg.step(dt); so = Lo.step(dt)
+        assert sg["nan_seen"] == 0 and sg["s_over_dx_max"] == so["s_over_dx_max"], it
+        dt = wl.cfl / so["s_over_dx_max"]
+    for f in ("h", "hu", "hv"):
+        assert np.array_equal(Lg.get_global(f), Lo.get_global(f))
