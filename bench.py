@@ -311,6 +311,7 @@ def main():
 
     cells = n * n
     L = make(args.side)
+    xcells_full, xcells_step, ycells = L.sweep_cells()          # cells one launch of each marching sweep updates on this tiling
     sampler = ClockSampler(local)
     time.sleep(0.3)
     t0 = time.time()
@@ -326,12 +327,13 @@ def main():
     slot_peak = nsm * 64.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6      # fp64 pipe: 64 lanes per SM per clock
     counts, counts_src = load_counts()
 
-    def slot_fraction(side, rate):
-        """fp64-pipe issue slots per interior cell update (the x-sweep also covers the 4 ghost rows of every patch, S-5) x rate / peak"""
+    def slot_fraction(xc, rate):
+        """fp64-pipe issue slots per interior cell update (the x-sweep also covers the ghost rows a y line reads: xc cells per
+        launch for n * n interior cells) x rate / peak"""
         if counts is None:
             return None
         kx, ky = counts["kernels"]["xsweep"], counts["kernels"]["ysweep"]
-        return (kx["fp64_slots_per_cell"] * (1.0 + 4.0 / side) + ky["fp64_slots_per_cell"]) * rate / slot_peak
+        return (kx["fp64_slots_per_cell"] * (xc / float(cells)) + ky["fp64_slots_per_cell"]) * rate / slot_peak
 
     # ---- end to end through the C ABI with HOST buffers (pinned): serial, then copies overlapped with the kernels
     e2e = None
@@ -347,7 +349,7 @@ def main():
         for _ in range(Ke):
             for k, f in enumerate(("h", "hu", "hv")):
                 L.set_global(f, hnp_in[k])
-            L.fill_ghost(None, 1.0)
+            L.fill_ghost_step(None, 1.0)
             st = L.step(dt)
             for k, f in enumerate(("h", "hu", "hv")):
                 ctx._chk(binding.lib().gc_level_get_global(L.h, k, 0, hnp_out[k].ctypes.data, 0, n, 0, 0, n, n), "get")
@@ -363,7 +365,7 @@ def main():
             for s in range(K):
                 P = pools[s % 2]
                 P.upload_state_async(hin, s_up)
-                P.fill_ghost(None, 1.0)
+                P.fill_ghost_step(None, 1.0)
                 P.step_auto(dts[s % 2], wl.cfl)
                 P.download_state_async(hout, s_dn)
             s_dn.synchronize(); torch.cuda.synchronize()
@@ -388,22 +390,23 @@ def main():
     tilings = None
     if not args.no_tilings and world == 1:
         tilings = {}
+        if L is not None:
+            L.destroy(); L = None
+        both_fills = not (args.full_fill or args.no_chains or unsplit or args.gauges > 0)
         for side in (16, 32, 64, 128, 256):
+            Ls = make(side)
+            xc = Ls.sweep_cells()[0 if (args.full_fill or unsplit) else 1]
             if side == args.side:
-                m, pr = ms, prof
+                m, pr = ms, prof                                # the headline run above
             else:
-                if L is not None:
-                    L.destroy(); L = None
-                Ls = make(side)
                 m, _, pr = timed(Ls, args.steps, W, use_dist=False)
-                if not args.full_fill and not args.no_chains:      # chained sides: the same with every ghost cell filled
-                    mf = timed(Ls, args.steps, W, use_dist=False, full_fill=True)[0]
-                Ls.destroy()
+            mf = timed(Ls, args.steps, W, use_dist=False, full_fill=True)[0] if both_fills else m   # every ghost cell filled
+            Ls.destroy()
             rate = cells * args.steps / (m * 1e-3)
             tilings[str(side)] = {"updates_per_s": rate, "ms_per_step": m / args.steps,
-                                  "ms_per_step_full_fill": (mf if side != args.side and not args.full_fill and not args.no_chains else m) / args.steps,
+                                  "ms_per_step_full_fill": mf / args.steps,
                                   "hbm_gbs_at_56B": BYTES_PER_UPDATE * rate / 1e9, "hbm_frac": BYTES_PER_UPDATE * rate / 1e9 / hbm_peak,
-                                  "fp64_pipe_slot_frac": slot_fraction(side, rate),
+                                  "fp64_pipe_slot_frac": slot_fraction(xc, rate), "xsweep_cells_per_launch": xc,
                                   "kernel_ms_per_step": {k: v[0] / args.steps for k, v in pr.items() if v[1]}}
 
     if rank != 0:
@@ -413,8 +416,8 @@ def main():
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms = prof[dom][0] / max(prof[dom][1], 1)
     share = {k: v[0] / max(sum(x[0] for x in prof.values()), 1e-12) for k, v in prof.items() if v[1]}
-    # cells one launch of the dominant kernel updates: the x-sweep also covers the 4 ghost rows of every patch (S-5)
-    per_launch = {"xsweep": cells * (1.0 + 4.0 / args.side), "ysweep": float(cells)}.get(dom, float(cells))
+    # cells one launch of the dominant kernel updates: the x-sweep also covers the ghost rows a y line reads (S-5; gc_level_sweep_cells)
+    per_launch = {"xsweep": float(xcells_full if (args.full_fill or unsplit) else xcells_step), "ysweep": float(ycells)}.get(dom, float(cells))
     kc = counts["kernels"].get(dom) if counts and not unsplit else None
     if unsplit:
         # planes of 8 bytes per cell the kernels of DESIGN.md 3.13 must move: the edge kernels read h, hu, hv, b and write
@@ -452,7 +455,10 @@ def main():
                    "l2": "inputs (%.1f GB pool) larger than L2, no flush" % (cells * 8 * 10 * (1 + 4 / args.side) ** 2 / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU", "cfl": wl.cfl,
                    "fma": "explicit, where DESIGN.md 3 writes it (both sides)", "manning_n": args.manning, "gauges": args.gauges,
-                   "scheme": args.scheme},
+                   "scheme": args.scheme,
+                   "ghost_fill": "gc_fill_ghost (every ghost cell)" if (args.full_fill or unsplit or args.gauges > 0) else
+                                 "gc_fill_ghost_step (the ghost cells the step reads: chained patches are read through, DESIGN.md 5); "
+                                 "tilings[side].ms_per_step_full_fill is the same step after gc_fill_ghost"},
         "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
         "hbm": {"achieved_gbs": BYTES_PER_UPDATE * value / world / 1e9, "peak_gbs": hbm_peak,
                 "frac": BYTES_PER_UPDATE * value / world / 1e9 / hbm_peak, "of": which, "bytes_per_update": BYTES_PER_UPDATE},

@@ -27,6 +27,12 @@ int gc_profile_read(gc_ctx *, double *ms /*HOST*/, int64_t *count /*HOST*/);
  * Synchronises the context's stream. */
 int gc_level_fallback_counts(const gc_level *L, int64_t out[4] /*HOST*/);
 
+/* Cells one launch of the marching sweep kernels updates on this level (the unit of bench.py's per-launch roofline figures):
+ * out[0] = x-sweep over every row of every patch (4 ghost rows per patch, S-5), out[1] = x-sweep without the ghost rows no y line
+ * reads (chains; what runs when no flux register is attached), out[2] = y-sweep (= interior cells).  0 for levels swept by the
+ * edge-parallel kernels. */
+int gc_level_sweep_cells(const gc_level *L, int64_t out[3] /*HOST*/);
+
 /* Self-test of the branch-free correctly rounded divide / reciprocal / square root the marching kernels use
  * (csrc/gc_math.cuh) against the IEEE operators: for each i, a[i]/b[i], 1/b[i], sqrt(a[i]) (a, b: HOST arrays of n).
  * nmismatch = results that differ in any bit although the fast path accepted the operands (must be 0);

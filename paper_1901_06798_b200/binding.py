@@ -18,7 +18,7 @@ SYMBOLS = [
     "gc_fill_ghost_b", "gc_level_step", "gc_level_step_auto", "gc_level_stats", "gc_wet_mask", "gc_level_mass",
     "gc_flag_cells", "gc_average_down", "gc_level_init_from", "gc_flux_attach", "gc_flux_fixup", "gc_probe_fp64_peak",
     "gc_launch_count", "gc_profile_enable", "gc_profile_read", "gc_selftest_math", "gc_gauges_bind", "gc_gauges_sample", "gc_level_set_patches",
-    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update", "gc_level_fallback_counts", "gc_level_step_unsplit",
+    "gc_ctx_set_option", "gc_level_upload_state_async", "gc_level_download_state_async", "gc_bathy_update", "gc_level_fallback_counts", "gc_level_sweep_cells", "gc_level_step_unsplit",
     "gc_level_step_accum", "gc_level_stats_reset", "gc_level_step_unsplit_static", "gc_unsplit_static_max_cells",
 ]
 
@@ -65,6 +65,7 @@ def lib():
     L.gc_ctx_set_option.argtypes = [vp, i, i64]
     L.gc_bathy_update.argtypes = [vp, vp, d]
     L.gc_level_fallback_counts.argtypes = [vp, vp]
+    L.gc_level_sweep_cells.argtypes = [vp, vp]
     L.gc_level_upload_state_async.argtypes = [vp, vp, vp]
     L.gc_level_download_state_async.argtypes = [vp, vp, vp]
     L.gc_last_error.argtypes = [vp]; L.gc_last_error.restype = C.c_char_p
@@ -231,6 +232,12 @@ class Level:
     def download_state_async(self, host3, copy_stream):
         ptrs = (C.c_void_p * 3)(*[t.data_ptr() for t in host3])
         self.ctx._chk(lib().gc_level_download_state_async(self.h, ptrs, C.c_void_p(copy_stream.cuda_stream)), "gc_level_download_state_async")
+
+    def sweep_cells(self):
+        """gc_level_sweep_cells -> (x-sweep cells per launch over every row, without the unread ghost rows, y-sweep cells)"""
+        out = (C.c_int64 * 3)()
+        self.ctx._chk(lib().gc_level_sweep_cells(self.h, out), "gc_level_sweep_cells")
+        return tuple(int(v) for v in out)
 
     def fallback_counts(self):
         """gc_level_fallback_counts -> dict(warp_iters, fb_warp_iters, fb_solves, fb_fluxes), cumulative for this level"""

@@ -48,8 +48,11 @@ def main():
     ap.add_argument("--n", type=int, default=8192)
     ap.add_argument("--side", type=int, default=256)
     ap.add_argument("--out", default=os.path.join(ROOT, "profiles", "r02_counts.json"))
+    ap.add_argument("--x-cells", type=float, default=0.0,
+                    help="cells one x-sweep launch updates (bench.py prints it as roofline.cells_per_launch / config.tilings[side]."
+                         "xsweep_cells_per_launch); default: n * (n + 4), the regular tiling with chains (only the level's own 4 ghost rows)")
     a = ap.parse_args()
-    cells = {"xsweep": a.n * a.n * (1.0 + 4.0 / a.side), "ysweep": float(a.n * a.n)}   # the x-sweep also covers 4 ghost rows per patch
+    cells = {"xsweep": a.x_cells if a.x_cells > 0 else float(a.n) * (a.n + 4), "ysweep": float(a.n * a.n)}
 
     raw = list(csv.reader(io.StringIO(_ncu(a.rep, "--page", "raw", "--csv"))))
     hdr = raw[0]

@@ -281,10 +281,10 @@ static void build_lines(gc_level *L, int seg, std::vector<LineDesc> &xl, std::ve
                 for (int l = 0; l < nlines; l++) {
                     const LineDesc d{sp, line0 + l, (int32_t)(2 + b0), (int32_t)(b1 - b0)};
                     if (dir == 0) {
-                        xl.push_back(d);
+                        xl.push_back(d); L->sweep_cells[0] += d.nc;
                         const bool ghost_row = l < 2 || l >= H.ny + 2;
-                        if (!ghost_row || (l < 2 ? lo_ghost : hi_ghost)) xl_red.push_back(d);
-                    } else yl.push_back(d);
+                        if (!ghost_row || (l < 2 ? lo_ghost : hi_ghost)) { xl_red.push_back(d); L->sweep_cells[1] += d.nc; }
+                    } else { yl.push_back(d); L->sweep_cells[2] += d.nc; }
                 }
             }
         }
@@ -702,6 +702,13 @@ extern "C" int gc_level_stats(const gc_level *L, gc_step_stats *out)
     if (rc) return rc;
     double sdx; memcpy(&sdx, &s.sdx_bits, 8);
     out->s_over_dx_max = sdx; out->cfl_max = 0.0; out->clipped_mass = s.clipped; out->n_clipped = (int64_t)s.nclip; out->nan_seen = s.nan_seen;
+    return GC_OK;
+}
+
+extern "C" int gc_level_sweep_cells(const gc_level *L, int64_t out[3])
+{
+    if (!L || !out) return GC_ERR_BADARG;
+    for (int k = 0; k < 3; k++) out[k] = L->sweep_cells[k];
     return GC_OK;
 }
 

@@ -147,6 +147,7 @@ struct gc_level {
     // chains of patches along x / y (one link per patch); x lines without the ghost rows no y line reads (their patch continues
     // above / below inside a y chain) -- used when no flux register reads Q* there; chained: 1 = some chain has two pieces
     ChainLink *d_xlink = nullptr, *d_ylink = nullptr; LineDesc *d_xl_red = nullptr; int64_t nxl_red = 0; int chained = 0;
+    int64_t sweep_cells[3] = {0, 0, 0};             // cells updated per launch: x-sweep over every row, x-sweep without the unread ghost rows, y-sweep
     int use_march;
     CopyRect *d_copy; int ncopy;                     // same-level copy rectangles, grouped by destination patch
     int2 *d_copy_range; int copy_wpp;               // per patch: (first rectangle, count); warps serving one patch

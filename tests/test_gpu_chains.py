@@ -135,3 +135,16 @@ def test_fill_ghost_step_poisoned_ghosts(gc, gco):
         dt = wl.cfl / so["s_over_dx_max"]
     for f in ("h", "hu", "hv"):
         assert np.array_equal(Lg.get_global(f), Lo.get_global(f))
+
+
+def test_sweep_cells_accounting(gc):
+    """gc_level_sweep_cells: a regular tiling with chains sweeps the level's own 4 ghost rows only; without chains 4 per patch"""
+    from paper_1901_06798_b200 import binding
+    n, side = 128, 16
+    wl = workloads.cfg5(n)
+    for chains, want in ((True, (n * (n + 4 * n // side), n * (n + 4), n * n)), (False, (n * (n + 4 * n // side),) * 2 + (n * n,))):
+        ctx = gc.Context(**wl.params)
+        ctx.set_option(binding.OPT_SWEEP_FAMILY, binding.SWEEP_MARCH)
+        ctx.set_option(binding.OPT_CHAINS, 0 if chains else 1)
+        L = driver.setup_level(ctx, wl, patches=workloads.tile(n, n, side))
+        assert L.sweep_cells() == want, (chains, L.sweep_cells(), want)
