@@ -209,6 +209,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end legs")
     ap.add_argument("--full-fill", action="store_true", help="gc_fill_ghost (every ghost cell) instead of gc_fill_ghost_step before each step")
     ap.add_argument("--no-chains", action="store_true", help="marching lines stop at every patch boundary (GC_OPT_CHAINS = 1): same bits")
+    ap.add_argument("--seg", type=int, default=0, help="GC_OPT_MARCH_SEG: cells per marching segment (0: the library's choice)")
     ap.add_argument("--chain-max", type=int, default=0, help="GC_OPT_CHAINS = k: patches of k cells or more are not chained")
     ap.add_argument("--scheme", default="split", choices=("split", "unsplit"),
                     help="split: the paper's dimensionally split step (the headline); unsplit: the step with transverse Riemann solves "
@@ -240,6 +241,8 @@ def main():
     wl = workloads.cfg5(n)
     if args.manning > 0.0:
         wl.params = dict(wl.params, manning_n=args.manning)
+    if args.seg:
+        binding.DEFAULT_OPTIONS[binding.OPT_MARCH_SEG] = args.seg
     if args.no_chains:
         binding.DEFAULT_OPTIONS[binding.OPT_CHAINS] = 1
     elif args.chain_max >= 8:

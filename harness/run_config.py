@@ -42,7 +42,7 @@ def run_single(cfg, wl, patches, max_steps, graph_k, device):
         t_dev = torch.zeros(1, dtype=torch.float64, device=device)
 
         def one():
-            L.fill_ghost(None, 1.0)
+            L.fill_ghost_step(None, 1.0)           # the ghost cells the step reads (every one of them unless patches are chained)
             t_dev.add_(dt_dev)                     # simulated time, accumulated on the device
             L.step_auto(dt_dev, wl.cfl)
 
