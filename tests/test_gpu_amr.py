@@ -10,6 +10,17 @@ from harness import driver
 pytestmark = pytest.mark.gpu
 
 
+@pytest.fixture(autouse=True, params=["by size", "march"])
+def sweep_family(request, monkeypatch):
+    """The levels of these tests are small, so by size they run on the edge-parallel kernels; forced onto the marching kernels
+    they also go through the chains (fine patches that continue each other are walked as one line) next to
+    coarse-fine boundaries, with and without flux registers attached.  Same bits either way."""
+    from paper_1901_06798_b200 import binding
+    if request.param == "march":
+        monkeypatch.setitem(binding.DEFAULT_OPTIONS, binding.OPT_SWEEP_FAMILY, binding.SWEEP_MARCH)
+    return request.param
+
+
 def shore_bathy(X, Y):
     return -8.0 + 11.0 * X / 3200.0 + 1.2 * np.sin(Y / 350.0) + 0.6 * np.cos(X / 170.0 + Y / 260.0)
 
