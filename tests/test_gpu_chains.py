@@ -45,7 +45,7 @@ XS, YS = (8, 12, 20, 9, 3), (8, 24, 11, 5)
 
 
 @pytest.mark.parametrize("chains", [True, False])
-@pytest.mark.parametrize("seg", [0, 8, 12, 16, 28, 4096])
+@pytest.mark.parametrize("seg", [0, 4, 8, 12, 16, 28, 4096])
 def test_chains_wet_dry_mixed_sizes(gc, gco, chains, seg):
     wl = workloads.cfg2(64)
     wl.nx, wl.ny = sum(XS), sum(YS)
