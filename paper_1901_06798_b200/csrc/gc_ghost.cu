@@ -61,11 +61,13 @@ __global__ void __launch_bounds__(256, 2) k_copy_rects(const CopyRect *rects, co
             // after the other left a warp waiting one DRAM round trip per rectangle (side 16: 8 of them per patch).
             int64_t da[4], sa[4], db[4], sb[4];
             bool va[4], vb[4];
+            bool more = false;                                                     // some rectangle of the four is wide, or taller than two passes of the patch's warps
 #pragma unroll
             for (int k = 0; k < 4; k++) {
                 const CopyRect r = rect_from_lane(mine, min(i + k, cnt - 1));      // past the end: the last one again, masked out
                 int rpp, ly, lx;
                 narrow_map(r.w, lane, rpp, ly, lx);
+                more |= (rpp == 0) | (r.h > 2 * wpp * rpp);                        // the same for every lane: it depends on the rectangle only
                 const int y = 2 * sub * rpp + ly;
                 va[k] = (i + k < cnt) & (ly < rpp) & (y < r.h);
                 vb[k] = va[k] & (y + rpp < r.h);
@@ -87,6 +89,7 @@ __global__ void __launch_bounds__(256, 2) k_copy_rects(const CopyRect *rects, co
                 if (vb[k]) { f0[db[k]] = b[k][0]; if (NF > 1) { f1[db[k]] = b[k][1]; f2[db[k]] = b[k][2]; } }
             }
             // what is left: the later passes of a tall narrow rectangle, and the wide rectangles
+            if (!more) continue;
             for (int k = 0; k < 4 && i + k < cnt; k++) {
                 const CopyRect r = rect_from_lane(mine, i + k);
                 if (r.w >= 32) {                                           // (row pair, 32-column chunk) items dealt round the patch's warps
