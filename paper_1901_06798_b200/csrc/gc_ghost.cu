@@ -133,14 +133,15 @@ void gc_launch_copy_rects(gc_level *L, double *f0, double *f1, double *f2, int n
     else k_copy_rects<1><<<(unsigned)blocks, threads, 0, L->ctx->stream>>>(rects, range, L->np, wpp, f0, f1, f2);
 }
 
-// ---- A4: physical boundary.  pass 0: x faces over rows inside the domain; pass 1: y faces over all columns.
+// ---- A4: physical boundary.  pass 0: x faces over rows inside the domain; pass 1: y faces over all columns; pass 2: both, one
+// block per patch doing the one after the other.
 // Wall: mirror cell, normal momentum negated (is_state: f1 = hu, f2 = hv); extrapolation: nearest interior cell.
 __global__ void k_bc(const PatchDesc *pat, const int32_t *list, double *f0, double *f1, double *f2, int nf, int is_state,
                      int pass, int64_t nxl, int64_t nyl, int bc0, int bc1, int bc2, int bc3)
 {
     PatchDesc pd = pat[list[blockIdx.x]];
     int rows = pd.ny + 4;
-    if (pass == 0) {
+    if (pass != 1) {
         // up to 4 ghost columns (2 per side) x rows
         for (int t = threadIdx.x; t < rows * 4; t += blockDim.x) {
             int j = t >> 2, c = t & 3;
@@ -160,7 +161,9 @@ __global__ void k_bc(const PatchDesc *pat, const int32_t *list, double *f0, doub
                 f2[d] = f2[s];
             }
         }
-    } else {
+    }
+    if (pass == 2) __syncthreads();      // both passes in one launch: the y faces read this patch's own x faces, written by this block
+    if (pass != 0) {
         const int W = pd.nx + 4;
         for (int t = threadIdx.x; t < W * 4; t += blockDim.x) {
             int c = t / W, i = t - c * W;
@@ -186,10 +189,8 @@ void gc_launch_bc(gc_level *L, double *f0, double *f1, double *f2, int nf, int i
 {
     if (L->nbcp == 0) return;
     const int *bc = L->ctx->P.bc;
-    ProfScope ps(L->ctx, GC_SLOT_BC, 2);
-    for (int pass = 0; pass < 2; pass++)
-        k_bc<<<L->nbcp, 128, 0, L->ctx->stream>>>(L->d_pat, L->d_bcp, f0, f1, f2, nf, is_state, pass, L->nxl, L->nyl,
-                                                  bc[0], bc[1], bc[2], bc[3]);
+    ProfScope ps(L->ctx, GC_SLOT_BC, 1);
+    k_bc<<<L->nbcp, 128, 0, L->ctx->stream>>>(L->d_pat, L->d_bcp, f0, f1, f2, nf, is_state, 2, L->nxl, L->nyl, bc[0], bc[1], bc[2], bc[3]);
 }
 
 // ---- field transfer.  Grids are patches x chunks of GC_CHUNK cells, so that a level that is one large patch spreads over the
