@@ -294,20 +294,20 @@ def main():
         torch.cuda.synchronize()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         lc0 = ctx.launch_count()
+        # the library brackets each of its kernels with CUDA events on the launching stream during the timed steps themselves
+        # (they cost nothing measurable: plain against bracketed passes alternating, profiles/r02_marchp.md), so that the
+        # per-kernel times of the roofline object come from the same steps, at the same clock, as ms_per_step
+        ctx.profile(True)
         e0.record()
         for k in range(K):
             one_step(k)
         e1.record()
         torch.cuda.synchronize()
+        prof = ctx.profile_read()
+        ctx.profile(False)
         if d: d.barrier()
         ms = e0.elapsed_time(e1)
         launches = ctx.launch_count() - lc0
-        # same K steps again with the library's per-kernel event brackets (separate pass: brackets perturb a little)
-        ctx.profile(True)
-        for k in range(K):
-            one_step(k)
-        prof = ctx.profile_read()
-        ctx.profile(False)
         st = L.stats()
         assert st["nan_seen"] == 0 and np.isfinite(dt_dev.item())
         return ms, launches, prof
