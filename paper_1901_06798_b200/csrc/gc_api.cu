@@ -86,7 +86,7 @@ extern "C" int gc_ctx_set_option(gc_ctx *c, int key, int64_t value)
 }
 
 extern "C" int64_t gc_launch_count(const gc_ctx *c) { return c ? (int64_t)c->launches : 0; }
-extern "C" int gc_profile_enable(gc_ctx *c, int on) { if (!c) return GC_ERR_BADARG; c->prof = on != 0; return GC_OK; }
+extern "C" int gc_profile_enable(gc_ctx *c, int on) { if (!c) return GC_ERR_BADARG; c->prof = on != 0; c->prof_last = nullptr; return GC_OK; }
 extern "C" int gc_profile_read(gc_ctx *c, double *ms, int64_t *count)
 {
     if (!c || !ms || !count) return GC_ERR_BADARG;
@@ -97,10 +97,11 @@ extern "C" int gc_profile_read(gc_ctx *c, double *ms, int64_t *count)
             float t = 0.f;
             cudaEventElapsedTime(&t, p.first, p.second);
             ms[s] += t;
-            cudaEventDestroy(p.first); cudaEventDestroy(p.second);
         }
         c->ev[s].clear();
     }
+    for (cudaEvent_t e : c->ev_own) cudaEventDestroy(e);
+    c->ev_own.clear(); c->prof_last = nullptr;
     return gc_cuda_check(c, "gc_profile_read");
 }
 

@@ -109,18 +109,31 @@ struct gc_ctx {
     int opt_family = 0, opt_seg = 0, opt_chains = 0;                 // gc_ctx_set_option: sweep kernel family (0 auto, 1 edge, 2 march), marching segment length
     void *stage = nullptr; size_t stage_bytes = 0;   // grow-only device staging buffer of the host-pointer paths (gc_stage_get)
     unsigned long long launches = 0;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[GC_NSLOT];     // brackets per slot; the events themselves are owned by ev_own
+    std::vector<cudaEvent_t> ev_own; cudaEvent_t prof_last = nullptr;
 };
 
-// counts kernel launches; when profiling is on, brackets them with CUDA events on the launching stream
+// counts kernel launches; when profiling is on, brackets them with CUDA events on the launching stream.  The event that ends one
+// launch's bracket starts the next one's (the library's launches follow each other on one stream; every recorded event puts a
+// small bubble between two kernels, so there are n + 1 of them for n launches, not 2 n): a launch's time then includes the gap
+// before it, a few microseconds.  gc_profile_enable and gc_profile_read start a new run of brackets.
 struct ProfScope {
-    gc_ctx *c; int slot; cudaEvent_t e0, e1;
-    ProfScope(gc_ctx *c_, int slot_, int nlaunch = 1) : c(c_), slot(slot_), e0(nullptr), e1(nullptr)
+    gc_ctx *c; int slot; cudaEvent_t e0;
+    ProfScope(gc_ctx *c_, int slot_, int nlaunch = 1) : c(c_), slot(slot_), e0(nullptr)
     {
         c->launches += nlaunch;
-        if (c->prof) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventRecord(e0, c->stream); }
+        if (c->prof) {
+            e0 = c->prof_last;
+            if (!e0) { cudaEventCreate(&e0); c->ev_own.push_back(e0); cudaEventRecord(e0, c->stream); }
+        }
     }
-    ~ProfScope() { if (e0) { cudaEventRecord(e1, c->stream); c->ev[slot].push_back({e0, e1}); } }
+    ~ProfScope()
+    {
+        if (e0) {
+            cudaEvent_t e1; cudaEventCreate(&e1); c->ev_own.push_back(e1); cudaEventRecord(e1, c->stream);
+            c->ev[slot].push_back({e0, e1}); c->prof_last = e1;
+        }
+    }
 };
 
 // one bound gauge: pool offsets of stencil cell (i, j) and of the containing cell, the patch's row pitch, the weights
